@@ -1,0 +1,145 @@
+"""ctypes loader for the float64 CPU oracle (oracle/snref.c).
+
+TEST INFRASTRUCTURE: only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+--impl reference legs may import this.  It imports nothing from the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsnref.so")
+_SRC = os.path.join(_HERE, "snref.c")
+_lib: Optional[ctypes.CDLL] = None
+
+
+class SnrefDiag(ctypes.Structure):
+    _fields_ = [("norm", ctypes.c_double), ("e_kin", ctypes.c_double), ("e_nonlocal", ctypes.c_double),
+                ("e_local", ctypes.c_double), ("e_total", ctypes.c_double)]
+
+
+def build(force: bool = False) -> str:
+    """Compile oracle/snref.c -> oracle/libsnref.so (gcc -O2 -fopenmp)."""
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-fopenmp", "-std=gnu99", "-fPIC", "-shared", "-o", _LIB_PATH, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB_PATH
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB_PATH)
+        vp, i64p, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double)
+        L.snref_fft1d.argtypes = [vp, ctypes.c_int64, ctypes.c_int]
+        L.snref_fftn.argtypes = [vp, ctypes.c_int, i64p, ctypes.c_int]
+        L.snref_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_double, ctypes.c_double,
+                                   ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double]
+        L.snref_destroy.argtypes = [vp]
+        L.snref_set_dtau.argtypes = [vp, ctypes.c_double]
+        L.snref_set_state.argtypes = [vp, vp]
+        L.snref_get_state.argtypes = [vp, vp]
+        L.snref_step.argtypes = [vp, ctypes.c_int64]
+        L.snref_potential.argtypes = [vp, vp]
+        L.snref_diagnostics.argtypes = [vp, ctypes.POINTER(SnrefDiag)]
+        L.snref_num_threads.restype = ctypes.c_int
+        L.snref_set_num_threads.argtypes = [ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+class OracleError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        super().__init__(f"{what} failed with oracle code {code}")
+        self.code = code
+
+
+def _chk(rc: int, what: str) -> None:
+    if rc != 0:
+        raise OracleError(rc, what)
+
+
+def fft1d(x: np.ndarray, direction: int) -> np.ndarray:
+    a = np.ascontiguousarray(x, dtype=np.complex128).copy()
+    _chk(lib().snref_fft1d(a.ctypes.data, a.size, direction), "snref_fft1d")
+    return a
+
+
+def fftn(x: np.ndarray, direction: int) -> np.ndarray:
+    a = np.ascontiguousarray(x, dtype=np.complex128).copy()
+    dims = (ctypes.c_int64 * a.ndim)(*a.shape)
+    _chk(lib().snref_fftn(a.ctypes.data, a.ndim, dims, direction), "snref_fftn")
+    return a
+
+
+def num_threads() -> int:
+    return int(lib().snref_num_threads())
+
+
+def set_num_threads(n: int) -> None:
+    lib().snref_set_num_threads(int(n))
+
+
+class Oracle:
+    """One float64 simulation context (snref_ctx)."""
+
+    def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float,
+                 g: Sequence[float], dtau: float):
+        self.dims = tuple(int(n) for n in dims)
+        nd = len(self.dims)
+        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
+        self.L = tuple(Ls)
+        g = [float(v) for v in g]
+        self._h = ctypes.c_void_p()
+        c_dims = (ctypes.c_int64 * nd)(*self.dims)
+        c_L = (ctypes.c_double * nd)(*Ls)
+        c_g = (ctypes.c_double * max(1, len(g)))(*g) if g else (ctypes.c_double * 1)(0.0)
+        _chk(lib().snref_create(ctypes.byref(self._h), nd, c_dims, c_L, A, B, C, D, c_g, len(g), dtau),
+             "snref_create")
+
+    @classmethod
+    def from_config(cls, cfg) -> "Oracle":
+        return cls(cfg.dims, cfg.L, cfg.A, cfg.B, cfg.C, cfg.D, cfg.g, cfg.dtau)
+
+    def close(self) -> None:
+        if self._h:
+            lib().snref_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, psi: np.ndarray) -> None:
+        a = np.ascontiguousarray(psi, dtype=np.complex128)
+        assert a.shape == self.dims, (a.shape, self.dims)
+        _chk(lib().snref_set_state(self._h, a.ctypes.data), "snref_set_state")
+
+    def get_state(self) -> np.ndarray:
+        out = np.empty(self.dims, dtype=np.complex128)
+        _chk(lib().snref_get_state(self._h, out.ctypes.data), "snref_get_state")
+        return out
+
+    def step(self, n: int) -> None:
+        _chk(lib().snref_step(self._h, int(n)), "snref_step")
+
+    def set_dtau(self, dtau: float) -> None:
+        _chk(lib().snref_set_dtau(self._h, float(dtau)), "snref_set_dtau")
+
+    def potential(self) -> np.ndarray:
+        out = np.empty(self.dims, dtype=np.float64)
+        _chk(lib().snref_potential(self._h, out.ctypes.data), "snref_potential")
+        return out
+
+    def diagnostics(self) -> dict:
+        d = SnrefDiag()
+        _chk(lib().snref_diagnostics(self._h, ctypes.byref(d)), "snref_diagnostics")
+        return {k: getattr(d, k) for k, _ in SnrefDiag._fields_}
