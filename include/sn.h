@@ -1,0 +1,108 @@
+/*
+ * sn.h -- C ABI of the B200-native split-step Schroedinger-Newton stepper (libsn.so).
+ *
+ * What the library computes.  The generalized Schroedinger-Newton system of PAPER.md:42-44
+ * (section II, eq. (1),(2))
+ *      i dpsi/dtau = A lap psi + B phi psi + G(|psi|^2) psi            (1)
+ *      lap phi + C phi = D |psi|^2                                      (2)
+ * on a periodic 2D/3D box, advanced with the "Symmetric Split-Step Fourier Method", eq. (2)
+ * "also solved with spectral methods" (section III).  One step is
+ *      K(dtau/2) N(dtau) K(dtau/2),
+ *      K(s): psi^ *= exp(+i A k^2 s) in Fourier space,
+ *      N(s): phi^ = D rho^/(C - k^2) (phi^(0) = 0 when C == 0), psi *= exp(-i s (B phi + G(rho))),
+ * (readings Q1-Q10 of DESIGN.md).  All arithmetic is complex64/float32 on the GPU; every step
+ * of the path runs in hand-written sm_100a kernels (no cuFFT, no CPU fallback).
+ *
+ * Conventions.
+ *   - dims[0] is the slowest axis, dims[ndim-1] the contiguous one (C order).
+ *   - psi is complex64, interleaved (re, im), ndim-dimensional, dense.
+ *   - Pointers are tagged "host" or "device" below.  The library never allocates device
+ *     memory: state, half-spectrum buffer and tables live in the caller's workspace
+ *     (e.g. a torch uint8 tensor), which must stay alive until sn_destroy.
+ *   - Every call returns 0 on success or a negative SN_ERR_* code; nothing throws, nothing
+ *     calls exit.  On error, outputs are untouched and the context state is unchanged.
+ *   - A context is not thread-safe; different contexts are independent.
+ *   - All device work is enqueued on the cudaStream_t given to sn_create.
+ */
+#ifndef SN_H
+#define SN_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SN_OK 0
+#define SN_ERR_NULL -1      /* a required pointer is NULL */
+#define SN_ERR_DIMS -2      /* ndim not 2/3, or an axis length that is not supported */
+#define SN_ERR_PARAM -3     /* non-finite constant, L <= 0, n_g outside [0,4], nsteps < 0 */
+#define SN_ERR_SINGULAR -4  /* C > 0 and C == k^2 for some grid mode: eq. (2) has no solution */
+#define SN_ERR_WORKSPACE -5 /* workspace too small or not 256-byte aligned */
+#define SN_ERR_STATE -6     /* step/get/diagnostics before sn_set_state */
+#define SN_ERR_CUDA -7      /* a CUDA runtime call failed (sticky; text via sn_strerror) */
+
+typedef struct sn_ctx sn_ctx; /* opaque host object, owned by the library */
+
+/* Diagnostics (reading Q10 of DESIGN.md; the paper defines none):
+ *   norm = sum |psi|^2 dV,
+ *   H    = -A sum_k k^2 |psi^_k|^2 dV/prod N + (B/2) sum phi rho dV + sum F(rho) dV,
+ *   F(rho) = sum_j g_j rho^(j+1)/(j+1). */
+typedef struct {
+    double norm, e_kin, e_nonlocal, e_local, e_total;
+} sn_diag;
+
+/* Supported axis lengths: powers of two, 64 <= N <= 4096 (sn_workspace_bytes returns 0 and
+ * sn_create returns SN_ERR_DIMS otherwise).  Bytes of device workspace needed. */
+size_t sn_workspace_bytes(int ndim, const int64_t *dims /* host, ndim entries */);
+
+/* Create a context.
+ *   out          host; receives the context
+ *   dims, L      host; ndim axis lengths and box lengths (dims[0] slowest)
+ *   A,B,C,D      constants of eq. (1),(2)
+ *   g, n_g       host; G(rho) = sum_{j=1..n_g} g[j-1] rho^j, 0 <= n_g <= 4 (g may be NULL if n_g == 0)
+ *   dtau         step; may be negative (time reversal) or zero
+ *   d_workspace  DEVICE; >= sn_workspace_bytes(...) bytes, 256-byte aligned, caller-owned
+ *   cuda_stream  cudaStream_t (0 = legacy default stream) */
+int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C,
+              double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
+              void *cuda_stream);
+
+/* Copy a complex64 state in.  psi: host (src_on_device == 0) or device pointer; prod(dims) complex64. */
+int sn_set_state(sn_ctx *ctx, const void *psi, int src_on_device);
+
+/* Advance nsteps Strang steps (tau += nsteps*dtau).  Enqueues kernels and returns without
+ * synchronising.  Adjacent kinetic half steps are merged inside one call (mathematically identical). */
+int sn_step(sn_ctx *ctx, int64_t nsteps);
+
+/* Copy the state out.  A host destination synchronises the stream. */
+int sn_get_state(sn_ctx *ctx, void *psi_out, int dst_on_device);
+
+/* Norm and energy of the current state (host struct).  Synchronises; the state is unchanged. */
+int sn_diagnostics(sn_ctx *ctx, sn_diag *out);
+
+/* Replace dtau (rebuilds the kinetic phase tables). */
+int sn_set_dtau(sn_ctx *ctx, double dtau);
+
+int sn_destroy(sn_ctx *ctx);
+
+/* Text for an error code; for SN_ERR_CUDA the last CUDA error string seen by this thread. */
+const char *sn_strerror(int code);
+
+/* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
+int64_t sn_launch_count(const sn_ctx *ctx);
+
+/* ---- test hooks (used by the acceptance tests, not by users) ---- */
+
+/* In-place d-dimensional FFT of the internal state: direction +1 forward (e^{-i k x}, unscaled),
+ * -1 inverse (scaled by 1/prod N).  Uses the same line-FFT engine as sn_step. */
+int sn_debug_fft(sn_ctx *ctx, int direction);
+
+/* phi (float32, prod(dims) values, same layout as psi) solving eq. (2) for the current state. */
+int sn_debug_potential(sn_ctx *ctx, float *phi_out, int dst_on_device);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SN_H */

@@ -1,0 +1,521 @@
+// sn_api.cu -- C ABI (include/sn.h), table builder and Strang scheduler of libsn.so.
+//
+// Host-side only: builds the float64 -> hi/lo float tables, lays the caller's workspace out,
+// and enqueues the pass list of one sn_step(n) call on the context's stream.  Every arithmetic
+// step of the path runs in the kernels of sn_kernels.cu; there is no CPU fallback.
+#include "../../include/sn.h"
+#include "sn_launch.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+namespace {
+
+using snk::PassArgs;
+
+thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+inline bool len_ok(int64_t n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+int twiddle_entries(int N)
+{
+    int total = 0, ns = 1;
+    while (ns < N) {
+        const int rem = N / ns, r = rem >= 8 ? 8 : rem;
+        if (ns > 1) total += ns * (r - 1);
+        ns *= r;
+    }
+    return total;
+}
+
+struct Layout {
+    int ndim;
+    int64_t n[3];
+    int64_t cells, cols0, nx, hs_lines, hs_elems;
+    size_t off_psi, off_hs, off_phi, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
+};
+
+bool make_layout(int ndim, const int64_t *dims, Layout &L)
+{
+    if (!dims || (ndim != 2 && ndim != 3)) return false;
+    L.ndim = ndim;
+    L.cells = 1;
+    for (int d = 0; d < ndim; d++) {
+        if (!len_ok(dims[d])) return false;
+        L.n[d] = dims[d];
+        L.cells *= dims[d];
+    }
+    L.cols0 = L.cells / L.n[0];
+    L.nx = L.n[ndim - 1];
+    L.hs_lines = (L.n[0] / 2 + 1) * L.cols0 / L.nx;
+    if (L.hs_lines & 1) L.hs_lines++; // line pairs: one dummy line (2D)
+    L.hs_elems = L.hs_lines * L.nx;
+    size_t o = 0;
+    L.off_psi = o; o = align256(o + (size_t)L.cells * 8);
+    L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
+    L.off_phi = o; o = align256(o + (size_t)L.cells * 4);
+    for (int d = 0; d < ndim; d++) {
+        L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
+        L.off_ph_full[d] = o; o = align256(o + (size_t)L.n[d] * 16);
+        L.off_ph_half[d] = o; o = align256(o + (size_t)L.n[d] * 16);
+        L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
+    }
+    L.off_kother = o; o = align256(o + (size_t)L.hs_lines * 4);
+    L.off_diag = o; o = align256(o + 8 * sizeof(double));
+    L.total = o;
+    return true;
+}
+
+struct f4 { float x, y, z, w; };
+
+inline f4 split_hilo(double re, double im)
+{
+    f4 r;
+    r.x = (float)re; r.y = (float)im;
+    r.z = (float)(re - (double)r.x);
+    r.w = (float)(im - (double)r.y);
+    return r;
+}
+
+inline double kval(int64_t j, int64_t n, double L)
+{
+    const int64_t jj = j < n / 2 ? j : j - n;
+    return 2.0 * M_PI / L * (double)jj;
+}
+
+} // namespace
+
+struct sn_ctx {
+    Layout lay;
+    double L[3];
+    double A, B, C, D, g[4], dtau;
+    int n_g;
+    char *ws;
+    cudaStream_t stream;
+    bool has_state;
+    int64_t launches;
+    snk::NLParams nl;
+    float2 *psi, *hs;
+    float *phi;
+    const float4 *tw[3], *ph_full[3], *ph_half[3];
+    const float *ksq[3], *kother;
+    double *diag;
+};
+
+namespace {
+
+int cuda_fail(cudaError_t e)
+{
+    std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "%s: %s", cudaGetErrorName(e), cudaGetErrorString(e));
+    return SN_ERR_CUDA;
+}
+#define SN_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e_ = (call);                        \
+        if (e_ != cudaSuccess) return cuda_fail(e_);    \
+    } while (0)
+
+int run_pass(sn_ctx *c, int N, PassArgs &a)
+{
+    a.stream = c->stream;
+    int rc;
+    switch (N) {
+    case 64: rc = snk::launch_pass<64>(a); break;
+    case 128: rc = snk::launch_pass<128>(a); break;
+    case 256: rc = snk::launch_pass<256>(a); break;
+    case 512: rc = snk::launch_pass<512>(a); break;
+    case 1024: rc = snk::launch_pass<1024>(a); break;
+    case 2048: rc = snk::launch_pass<2048>(a); break;
+    case 4096: rc = snk::launch_pass<4096>(a); break;
+    default: return SN_ERR_DIMS;
+    }
+    if (rc != 0) return cuda_fail((cudaError_t)rc);
+    c->launches++;
+    return SN_OK;
+}
+
+// kinetic phase tables exp(i A k_a^2 s)/N_a for s = dtau and dtau/2 (S2; reading Q2)
+int upload_phase_tables(sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    for (int d = 0; d < l.ndim; d++) {
+        const int64_t n = l.n[d];
+        std::vector<f4> full(n), half(n);
+        for (int64_t k = 0; k < n; k++) {
+            const double kk = kval(k, n, c->L[d]);
+            const double th = c->A * kk * kk * c->dtau;
+            full[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
+            half[k] = split_hilo(std::cos(0.5 * th) / (double)n, std::sin(0.5 * th) / (double)n);
+        }
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph_full[d], full.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph_half[d], half.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vectors die at the end of this iteration
+    }
+    c->nl.hb = (float)(-0.5 * c->dtau * c->B);
+    for (int j = 0; j < 4; j++) {
+        c->nl.hg[j] = j < c->n_g ? (float)(-0.5 * c->dtau * c->g[j]) : 0.f;
+        c->nl.fg[j] = j < c->n_g ? (float)(c->g[j] / (double)(j + 2)) : 0.f;
+    }
+    return SN_OK;
+}
+
+int upload_static_tables(sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    for (int d = 0; d < l.ndim; d++) {
+        const int N = (int)l.n[d];
+        // twiddles: for each stage (NS, R) with NS > 1: entry [kp][r-1] = exp(-2 pi i r kp/(NS R))
+        std::vector<f4> tw;
+        tw.reserve(twiddle_entries(N));
+        for (int ns = 1; ns < N;) {
+            const int rem = N / ns, r = rem >= 8 ? 8 : rem;
+            if (ns > 1)
+                for (int kp = 0; kp < ns; kp++)
+                    for (int q = 1; q < r; q++) {
+                        const double th = -2.0 * M_PI * (double)((q * kp) % (ns * r)) / (double)(ns * r);
+                        tw.push_back(split_hilo(std::cos(th), std::sin(th)));
+                    }
+            ns *= r;
+        }
+        std::vector<float> ksq(N);
+        for (int k = 0; k < N; k++) {
+            const double kk = kval(k, N, c->L[d]);
+            ksq[k] = (float)(kk * kk);
+        }
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d], tw.data(), tw.size() * 16, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq.data(), (size_t)N * 4, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    // sum of the non-contiguous axes' k^2 for each contiguous line of the half spectrum
+    std::vector<float> ko(l.hs_lines, 0.f);
+    const int64_t h0 = l.n[0] / 2 + 1;
+    if (l.ndim == 2) {
+        for (int64_t k0 = 0; k0 < h0; k0++) {
+            const double a = kval(k0, l.n[0], c->L[0]);
+            ko[k0] = (float)(a * a);
+        }
+    } else {
+        for (int64_t k0 = 0; k0 < h0; k0++)
+            for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
+                const double a = kval(k0, l.n[0], c->L[0]), b = kval(k1, l.n[1], c->L[1]);
+                ko[k0 * l.n[1] + k1] = (float)(a * a + b * b);
+            }
+    }
+    SN_CUDA(cudaMemcpyAsync(c->ws + l.off_kother, ko.data(), ko.size() * 4, cudaMemcpyHostToDevice, c->stream));
+    SN_CUDA(cudaMemsetAsync(c->ws + l.off_hs, 0, (size_t)l.hs_elems * 8, c->stream));
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    return SN_OK;
+}
+
+PassArgs base_args(const sn_ctx *c)
+{
+    PassArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.hilo = 1;
+    a.dir = +1;
+    a.scale = 1.f;
+    a.C = (float)c->C;
+    a.nl = c->nl;
+    a.diag = c->diag;
+    return a;
+}
+
+// geometry of a pass along `axis` of an array shaped like psi but with n0 rows on axis 0
+void set_axis_geometry(const sn_ctx *c, PassArgs &a, int axis, int64_t n0)
+{
+    const Layout &l = c->lay;
+    if (axis == 0) {
+        a.n_outer = 1; a.outer_stride = 0; a.ncols = (int)l.cols0; a.row_stride = l.cols0;
+    } else { // axis 1 of a 3D array
+        a.n_outer = (int)n0; a.outer_stride = l.n[1] * l.n[2]; a.ncols = (int)l.n[2]; a.row_stride = l.n[2];
+    }
+}
+
+// one kinetic sweep over all axes; with_nl fuses the nonlinear phase (and the c2r of phi^) into axis 0
+int kinetic_sweep(sn_ctx *c, bool half, bool with_nl)
+{
+    const Layout &l = c->lay;
+    int rc;
+    for (int d = 0; d < l.ndim; d++) {
+        PassArgs a = base_args(c);
+        a.data = c->psi;
+        a.hs = c->hs;
+        a.tw = c->tw[d];
+        a.phase = half ? c->ph_half[d] : c->ph_full[d];
+        if (d == l.ndim - 1) {
+            a.kind = snk::P_X_KIN;
+            a.nlines = (int)(l.cells / l.nx);
+        } else {
+            a.kind = (d == 0 && with_nl) ? snk::P_H_NLKIN : snk::P_S_KIN;
+            set_axis_geometry(c, a, d, l.n[0]);
+        }
+        if ((rc = run_pass(c, (int)l.n[d], a))) return rc;
+    }
+    return SN_OK;
+}
+
+// phi^ (half spectrum, all scales folded in, ready for the axis-0 c2r) from the current psi
+int potential_spectrum(sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    int rc;
+    {
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_R2C; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+        set_axis_geometry(c, a, 0, l.n[0]);
+        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    }
+    if (l.ndim == 3) {
+        PassArgs a = base_args(c);
+        a.kind = snk::P_S_FFT; a.dir = +1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1];
+        set_axis_geometry(c, a, 1, l.n[0] / 2 + 1);
+        if ((rc = run_pass(c, (int)l.n[1], a))) return rc;
+    }
+    {
+        const int dx = l.ndim - 1;
+        PassArgs a = base_args(c);
+        a.kind = snk::P_X_POISSON; a.data = c->hs; a.tw = c->tw[dx]; a.ksq = c->ksq[dx]; a.kother2 = c->kother;
+        a.nlines = (int)l.hs_lines;
+        a.pscale = (float)(c->D * 0.5 / (double)l.cells);
+        if ((rc = run_pass(c, (int)l.n[dx], a))) return rc;
+    }
+    if (l.ndim == 3) {
+        PassArgs a = base_args(c);
+        a.kind = snk::P_S_FFT; a.dir = -1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1]; a.scale = 1.f;
+        set_axis_geometry(c, a, 1, l.n[0] / 2 + 1);
+        if ((rc = run_pass(c, (int)l.n[1], a))) return rc;
+    }
+    return SN_OK;
+}
+
+} // namespace
+
+// ============================================================================ C ABI
+
+extern "C" {
+
+size_t sn_workspace_bytes(int ndim, const int64_t *dims)
+{
+    Layout l;
+    return make_layout(ndim, dims, l) ? l.total : 0;
+}
+
+int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
+              const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
+{
+    if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
+    Layout l;
+    if (!make_layout(ndim, dims, l)) return SN_ERR_DIMS;
+    if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
+    if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
+        return SN_ERR_PARAM;
+    for (int d = 0; d < ndim; d++)
+        if (!std::isfinite(L[d]) || L[d] <= 0.0) return SN_ERR_PARAM;
+    for (int j = 0; j < n_g; j++)
+        if (!std::isfinite(g[j])) return SN_ERR_PARAM;
+    if (workspace_bytes < l.total || ((uintptr_t)d_workspace & 255) != 0) return SN_ERR_WORKSPACE;
+    if (C > 0.0) { // reading Q5: a grid mode with k^2 == C makes eq. (2) unsolvable
+        const double tol = 1e-12 * std::fmax(1.0, std::fabs(C));
+        const int64_t n0 = l.n[0], n1 = l.n[1], n2 = ndim == 3 ? l.n[2] : 1;
+        for (int64_t i0 = 0; i0 <= n0 / 2; i0++) {
+            const double k0 = kval(i0, n0, L[0]);
+            for (int64_t i1 = 0; i1 <= n1 / 2; i1++) {
+                const double k1 = kval(i1, n1, L[1]);
+                for (int64_t i2 = 0; i2 <= n2 / 2; i2++) {
+                    const double k2 = ndim == 3 ? kval(i2, n2, L[2]) : 0.0;
+                    if (std::fabs(C - (k0 * k0 + k1 * k1 + k2 * k2)) < tol) return SN_ERR_SINGULAR;
+                }
+            }
+        }
+    }
+    sn_ctx *c = new (std::nothrow) sn_ctx;
+    if (!c) return SN_ERR_PARAM;
+    std::memset(c, 0, sizeof(*c));
+    c->lay = l;
+    for (int d = 0; d < ndim; d++) c->L[d] = L[d];
+    c->A = A; c->B = B; c->C = C; c->D = D; c->dtau = dtau; c->n_g = n_g;
+    for (int j = 0; j < n_g; j++) c->g[j] = g[j];
+    c->ws = static_cast<char *>(d_workspace);
+    c->stream = static_cast<cudaStream_t>(cuda_stream);
+    c->psi = reinterpret_cast<float2 *>(c->ws + l.off_psi);
+    c->hs = reinterpret_cast<float2 *>(c->ws + l.off_hs);
+    c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
+    for (int d = 0; d < ndim; d++) {
+        c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
+        c->ph_full[d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph_full[d]);
+        c->ph_half[d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph_half[d]);
+        c->ksq[d] = reinterpret_cast<const float *>(c->ws + l.off_ksq[d]);
+    }
+    c->kother = reinterpret_cast<const float *>(c->ws + l.off_kother);
+    c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
+    int rc = upload_static_tables(c);
+    if (rc == SN_OK) rc = upload_phase_tables(c);
+    if (rc != SN_OK) {
+        delete c;
+        return rc;
+    }
+    *out = c;
+    return SN_OK;
+}
+
+int sn_destroy(sn_ctx *c)
+{
+    if (!c) return SN_ERR_NULL;
+    cudaStreamSynchronize(c->stream);
+    delete c;
+    return SN_OK;
+}
+
+int sn_set_dtau(sn_ctx *c, double dtau)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!std::isfinite(dtau)) return SN_ERR_PARAM;
+    const double old = c->dtau;
+    c->dtau = dtau;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    const int rc = upload_phase_tables(c);
+    if (rc != SN_OK) c->dtau = old;
+    return rc;
+}
+
+int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)
+{
+    if (!c || !psi) return SN_ERR_NULL;
+    SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * 8,
+                            src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+    if (!src_on_device) SN_CUDA(cudaStreamSynchronize(c->stream)); // caller may reuse its host buffer
+    c->has_state = true;
+    return SN_OK;
+}
+
+int sn_get_state(sn_ctx *c, void *psi_out, int dst_on_device)
+{
+    if (!c || !psi_out) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * 8,
+                            dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    if (!dst_on_device) SN_CUDA(cudaStreamSynchronize(c->stream));
+    return SN_OK;
+}
+
+int sn_step(sn_ctx *c, int64_t nsteps)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    if (nsteps < 0) return SN_ERR_PARAM;
+    if (nsteps == 0) return SN_OK;
+    // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
+    int rc = kinetic_sweep(c, /*half=*/true, /*with_nl=*/false);
+    for (int64_t i = 1; rc == SN_OK && i <= nsteps; i++) {
+        rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/i == nsteps, /*with_nl=*/true);
+    }
+    return rc;
+}
+
+int sn_debug_fft(sn_ctx *c, int direction)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    if (direction != 1 && direction != -1) return SN_ERR_PARAM;
+    const Layout &l = c->lay;
+    for (int d = 0; d < l.ndim; d++) {
+        PassArgs a = base_args(c);
+        a.data = c->psi; a.tw = c->tw[d]; a.dir = direction; a.hilo = 1;
+        a.scale = direction < 0 ? (float)(1.0 / (double)l.n[d]) : 1.f;
+        if (d == l.ndim - 1) {
+            a.kind = snk::P_X_FFT;
+            a.nlines = (int)(l.cells / l.nx);
+        } else {
+            a.kind = snk::P_S_FFT;
+            set_axis_geometry(c, a, d, l.n[0]);
+        }
+        const int rc = run_pass(c, (int)l.n[d], a);
+        if (rc) return rc;
+    }
+    return SN_OK;
+}
+
+int sn_debug_potential(sn_ctx *c, float *phi_out, int dst_on_device)
+{
+    if (!c || !phi_out) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    int rc = potential_spectrum(c);
+    if (rc) return rc;
+    PassArgs a = base_args(c);
+    a.kind = snk::P_H_POT; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+    a.phi_out = dst_on_device ? phi_out : c->phi;
+    set_axis_geometry(c, a, 0, c->lay.n[0]);
+    if ((rc = run_pass(c, (int)c->lay.n[0], a))) return rc;
+    if (!dst_on_device) {
+        SN_CUDA(cudaMemcpyAsync(phi_out, c->phi, (size_t)c->lay.cells * 4, cudaMemcpyDeviceToHost, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    return SN_OK;
+}
+
+int sn_diagnostics(sn_ctx *c, sn_diag *out)
+{
+    if (!c || !out) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    const Layout &l = c->lay;
+    SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));
+    int rc = potential_spectrum(c);
+    if (rc) return rc;
+    {
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_DIAG; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+        set_axis_geometry(c, a, 0, l.n[0]);
+        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    }
+    // kinetic energy axis by axis: sum_k k_a^2 |psi^_k|^2 / prod N = sum_lines sum_ka k_a^2 |F_a psi|^2 / N_a
+    // (Parseval along the other axes), so one forward line transform per axis suffices.
+    for (int d = 0; d < l.ndim; d++) {
+        PassArgs a = base_args(c);
+        a.data = c->psi; a.tw = c->tw[d]; a.ksq = c->ksq[d]; a.diag = c->diag + 3 + d;
+        if (d == l.ndim - 1) {
+            a.kind = snk::P_X_KDIAG;
+            a.nlines = (int)(l.cells / l.nx);
+        } else {
+            a.kind = snk::P_S_KDIAG;
+            set_axis_geometry(c, a, d, l.n[0]);
+        }
+        if ((rc = run_pass(c, (int)l.n[d], a))) return rc;
+    }
+    double h[8];
+    SN_CUDA(cudaMemcpyAsync(h, c->diag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    double dV = 1.0;
+    for (int d = 0; d < l.ndim; d++) dV *= c->L[d] / (double)l.n[d];
+    double ek = 0.0;
+    for (int d = 0; d < l.ndim; d++) ek += h[3 + d] / (double)l.n[d];
+    out->norm = h[0] * dV;
+    out->e_kin = -c->A * ek * dV;
+    out->e_nonlocal = 0.5 * c->B * h[1] * dV;
+    out->e_local = h[2] * dV;
+    out->e_total = out->e_kin + out->e_nonlocal + out->e_local;
+    return SN_OK;
+}
+
+int64_t sn_launch_count(const sn_ctx *c) { return c ? c->launches : 0; }
+
+const char *sn_strerror(int code)
+{
+    switch (code) {
+    case SN_OK: return "ok";
+    case SN_ERR_NULL: return "null pointer argument";
+    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths powers of two in [64, 4096])";
+    case SN_ERR_PARAM: return "invalid parameter";
+    case SN_ERR_SINGULAR: return "C > 0 coincides with k^2 of a grid mode: eq. (2) is singular";
+    case SN_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";
+    case SN_ERR_STATE: return "no state set";
+    case SN_ERR_CUDA: return g_cuda_msg;
+    default: return "unknown error code";
+    }
+}
+
+} // extern "C"

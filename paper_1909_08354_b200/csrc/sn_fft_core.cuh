@@ -1,0 +1,268 @@
+// sn_fft_core.cuh -- register/shared-memory Stockham line FFT engine (sm_100a).
+//
+// The "Fourier methods" of PAPER.md:113 (section III) are hand-written here: one line of
+// N = 2^n complex64 points is held by T = N/8 threads, 8 points per thread in registers.
+// Every thread carries TWO independent lines (a[], b[]) so that each twiddle load, each
+// shared-memory instruction (128-bit: one point of each line) and each index computation is
+// amortised over two transforms.  Stages are radix-8 (a trailing radix-2/4 stage when n is
+// not a multiple of 3); between stages the lines are exchanged through shared memory in
+// Stockham (autosort) order, so forward output is in natural order, thread j holding points
+// j + T*m (m = 0..7) -- exactly the operands its first inverse stage needs.  A fused
+// forward -> pointwise -> inverse pass therefore needs no exchange at the junction.
+//
+// Twiddles are stored as hi+lo float pairs (float4 = wr_hi, wi_hi, wr_lo, wi_lo) built in
+// float64 on the host and applied with an FMA chain.  A plain fp32 twiddle has |w| != 1 by a
+// FIXED ~1e-8 relative amount; used by a fixed fraction of the butterflies this gives a
+// systematic, non-averaging gain per transform that breaks norm conservation at the 1e-5
+// level over 10^3 steps.  The lo part enters the FMA chain
+// before the final rounding, which removes the bias.  HILO=false (plain float2 twiddles) is
+// used for the density/potential transforms, where a 1e-7 gain is harmless.
+#pragma once
+#include <cuda_runtime.h>
+
+namespace snk {
+
+constexpr double SQRT_HALF_D = 0.70710678118654752440084436210485;
+constexpr float C8_HI = (float)SQRT_HALF_D;
+constexpr float C8_LO = (float)(SQRT_HALF_D - (double)C8_HI);
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+
+// v * w, w the FORWARD twiddle (e^{-i theta}) as hi/lo; DIR < 0 multiplies by conj(w).
+template <int DIR, bool HILO>
+__device__ __forceinline__ float2 twmul(float2 v, float4 w)
+{
+    const float wi = DIR > 0 ? w.y : -w.y;
+    float2 o;
+    if (HILO) {
+        const float li = DIR > 0 ? w.w : -w.w;
+        o.x = fmaf(v.x, w.x, fmaf(-v.y, wi, fmaf(v.x, w.z, -v.y * li)));
+        o.y = fmaf(v.x, wi, fmaf(v.y, w.x, fmaf(v.x, li, v.y * w.z)));
+    } else {
+        o.x = fmaf(v.x, w.x, -v.y * wi);
+        o.y = fmaf(v.x, wi, v.y * w.x);
+    }
+    return o;
+}
+
+template <bool HILO>
+__device__ __forceinline__ float scale8(float s)
+{
+    return HILO ? fmaf(s, C8_HI, s * C8_LO) : s * C8_HI;
+}
+
+// x *= W8^1 (forward: e^{-i pi/4}; DIR < 0: conjugate)
+template <int DIR, bool HILO>
+__device__ __forceinline__ float2 mul_w8_1(float2 v)
+{
+    return DIR > 0 ? make_float2(scale8<HILO>(v.x + v.y), scale8<HILO>(v.y - v.x))
+                   : make_float2(scale8<HILO>(v.x - v.y), scale8<HILO>(v.x + v.y));
+}
+// x *= W8^3
+template <int DIR, bool HILO>
+__device__ __forceinline__ float2 mul_w8_3(float2 v)
+{
+    return DIR > 0 ? make_float2(scale8<HILO>(v.y - v.x), scale8<HILO>(-v.x - v.y))
+                   : make_float2(scale8<HILO>(-v.x - v.y), scale8<HILO>(v.x - v.y));
+}
+// x *= W4^1 = -i (forward) / +i (inverse)
+template <int DIR>
+__device__ __forceinline__ float2 mul_w4_1(float2 v)
+{
+    return DIR > 0 ? make_float2(v.y, -v.x) : make_float2(-v.y, v.x);
+}
+
+template <int DIR>
+__device__ __forceinline__ void bf2(float2 &x0, float2 &x1)
+{
+    const float2 t = x0;
+    x0 = cadd(t, x1);
+    x1 = csub(t, x1);
+}
+
+// 4-point DFT, natural order in and out
+template <int DIR>
+__device__ __forceinline__ void bf4(float2 &x0, float2 &x1, float2 &x2, float2 &x3)
+{
+    const float2 c0 = cadd(x0, x2), d0 = csub(x0, x2);
+    const float2 c1 = cadd(x1, x3), d1 = mul_w4_1<DIR>(csub(x1, x3));
+    x0 = cadd(c0, c1);
+    x2 = csub(c0, c1);
+    x1 = cadd(d0, d1);
+    x3 = csub(d0, d1);
+}
+
+// 8-point DFT, natural order in and out
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf8(float2 &x0, float2 &x1, float2 &x2, float2 &x3, float2 &x4, float2 &x5,
+                                    float2 &x6, float2 &x7)
+{
+    float2 a0 = cadd(x0, x4), b0 = csub(x0, x4);
+    float2 a1 = cadd(x1, x5), b1 = mul_w8_1<DIR, HILO>(csub(x1, x5));
+    float2 a2 = cadd(x2, x6), b2 = mul_w4_1<DIR>(csub(x2, x6));
+    float2 a3 = cadd(x3, x7), b3 = mul_w8_3<DIR, HILO>(csub(x3, x7));
+    bf4<DIR>(a0, a1, a2, a3); // X0 X2 X4 X6
+    bf4<DIR>(b0, b1, b2, b3); // X1 X3 X5 X7
+    x0 = a0; x1 = b0; x2 = a1; x3 = b1; x4 = a2; x5 = b2; x6 = a3; x7 = b3;
+}
+
+// radix-R butterfly on x[q + r*NB], r = 0..R-1
+template <int R, int NB, int DIR, bool HILO>
+__device__ __forceinline__ void butterfly(float2 (&x)[8], int q)
+{
+    if constexpr (R == 8) {
+        bf8<DIR, HILO>(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7]);
+    } else if constexpr (R == 4) {
+        bf4<DIR>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB]);
+    } else {
+        bf2<DIR>(x[q], x[q + NB]);
+    }
+}
+
+// Number of float4 twiddle entries of the table for length N (all stages with NS > 1).
+constexpr int twiddle_entries(int N)
+{
+    int total = 0, ns = 1;
+    while (ns < N) {
+        const int rem = N / ns;
+        const int r = rem >= 8 ? 8 : rem;
+        if (ns > 1) total += ns * (r - 1);
+        ns *= r;
+    }
+    return total;
+}
+
+// One Stockham stage on both lines: twiddle (if NS > 1) then radix-R butterflies.
+// Butterfly q of thread j is butterfly number bq = j + T*q of the stage; its inputs are the
+// thread's own points j + T*(q + r*NB) = bq + r*N/R; twiddle exp(-/+ 2 pi i r (bq % NS)/(NS R)).
+template <int N, int R, int NS, int DIR, bool HILO>
+__device__ __forceinline__ void stage_compute(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw)
+{
+    constexpr int T = N / 8, NB = 8 / R;
+#pragma unroll
+    for (int q = 0; q < NB; q++) {
+        if constexpr (NS > 1) {
+            const int kp = (j + T * q) & (NS - 1);
+            const float4 *w = tw + kp * (R - 1);
+#pragma unroll
+            for (int r = 1; r < R; r++) {
+                float4 ww;
+                if (HILO) {
+                    ww = __ldg(w + (r - 1));
+                } else {
+                    const float2 h = __ldg(reinterpret_cast<const float2 *>(w + (r - 1)));
+                    ww = make_float4(h.x, h.y, 0.f, 0.f);
+                }
+                a[q + r * NB] = twmul<DIR, HILO>(a[q + r * NB], ww);
+                b[q + r * NB] = twmul<DIR, HILO>(b[q + r * NB], ww);
+            }
+        }
+        butterfly<R, NB, DIR, HILO>(a, q);
+        butterfly<R, NB, DIR, HILO>(b, q);
+    }
+}
+
+// Stockham exchange after a stage (NS, R): output r of butterfly bq goes to position
+// (bq / NS) * NS * R + (bq % NS) + r * NS; afterwards thread j re-reads points j + T*m.
+template <int N, int R, int NS, class SM>
+__device__ __forceinline__ void stage_exchange(float2 (&a)[8], float2 (&b)[8], int j, SM &sm)
+{
+    constexpr int T = N / 8, NB = 8 / R;
+    sm.sync(); // previous readers of the buffer are done
+#pragma unroll
+    for (int q = 0; q < NB; q++) {
+        const int bq = j + T * q;
+        const int base = (bq & ~(NS - 1)) * R + (bq & (NS - 1));
+#pragma unroll
+        for (int r = 0; r < R; r++) sm.st(base + r * NS, a[q + r * NB], b[q + r * NB]);
+    }
+    sm.sync();
+#pragma unroll
+    for (int m = 0; m < 8; m++) sm.ld(j + T * m, a[m], b[m]);
+}
+
+template <int N, int NS, int DIR, bool HILO, class SM>
+__device__ __forceinline__ void fft_stages(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw,
+                                           SM &sm)
+{
+    constexpr int REM = N / NS;
+    constexpr int R = REM >= 8 ? 8 : REM;
+    stage_compute<N, R, NS, DIR, HILO>(a, b, j, tw);
+    if constexpr (NS * R < N) {
+        stage_exchange<N, R, NS, SM>(a, b, j, sm);
+        fft_stages<N, NS * R, DIR, HILO, SM>(a, b, j, tw + (NS > 1 ? NS * (R - 1) : 0), sm);
+    }
+}
+
+// Unscaled DFT of two lines.  In: thread j holds points j + T*m of each line (T = N/8).
+// Out: thread j holds outputs j + T*m.  DIR = +1: sum x e^{-2 pi i jk/N}; DIR = -1: e^{+...}.
+template <int N, int DIR, bool HILO, class SM>
+__device__ __forceinline__ void fft_pair(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw, SM &sm)
+{
+    fft_stages<N, 1, DIR, HILO, SM>(a, b, j, tw, sm);
+}
+
+// ---- shared-memory accessors -------------------------------------------------------------
+// One float4 per point position: (a.re, a.im, b.re, b.im).
+
+// Tile of CP column pairs per row (strided-axis kernels); thread t owns column pair t.  With
+// CP = 8 a row is 128 B = all 32 banks and 8 adjacent lanes cover it, so every 128-bit access
+// phase is conflict-free for any row pattern.  Narrower tiles (long lines) XOR the chunk index
+// with row bits 3.. so that the stride-8 rows written after the first stage spread over banks.
+template <int CP>
+struct SmemTile {
+    float4 *base;
+    int t;
+    __device__ __forceinline__ int idx(int pos) const
+    {
+        if (CP == 8) return pos * 8 + t;
+        if (CP == 4) return (pos * 4 + t) ^ (((pos >> 3) & 1) << 2);
+        if (CP == 2) return (pos * 2 + t) ^ (((pos >> 3) & 3) << 1);
+        return pos ^ ((pos >> 3) & 7);
+    }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const
+    {
+        base[idx(pos)] = make_float4(a.x, a.y, b.x, b.y);
+    }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
+    {
+        const float4 v = base[idx(pos)];
+        a = make_float2(v.x, v.y);
+        b = make_float2(v.z, v.w);
+    }
+    __device__ __forceinline__ void sync() const { __syncthreads(); }
+};
+
+// One line pair per T-thread group, lanes = consecutive j (contiguous-axis kernel).  XOR
+// swizzle of the low 3 position bits with bits 3..5 makes the stride-8 writes of the first
+// stage conflict-free and keeps unit-stride accesses conflict-free.
+template <int T>
+struct SmemLine {
+    float4 *base;
+    int bar_id; // named barrier for this group when T > 32 and the CTA holds several groups
+    bool whole_cta;
+    __device__ __forceinline__ static int sw(int pos) { return pos ^ ((pos >> 3) & 7); }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const
+    {
+        base[sw(pos)] = make_float4(a.x, a.y, b.x, b.y);
+    }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
+    {
+        const float4 v = base[sw(pos)];
+        a = make_float2(v.x, v.y);
+        b = make_float2(v.z, v.w);
+    }
+    __device__ __forceinline__ void sync() const
+    {
+        if (T <= 32) {
+            __syncwarp();
+        } else if (whole_cta) {
+            __syncthreads();
+        } else {
+            asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(T) : "memory");
+        }
+    }
+};
+
+} // namespace snk

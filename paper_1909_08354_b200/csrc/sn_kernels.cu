@@ -1,0 +1,395 @@
+// sn_kernels.cu -- the pass kernels of the split-step path, compiled once per line length
+// (-DSN_LEN=N).  Every kernel is "load a tile of lines -> transform in registers/shared memory
+// with pointwise work fused at both ends -> store"; no standalone elementwise kernel exists.
+//
+// Pass structure of one Strang step (operations S1-S12 of SURVEY.md 8(a)):
+//   the kinetic operator exp(i A k^2 s) = prod_a exp(i A k_a^2 s) is separable, so it is applied
+//   as ONE pass per axis, each doing forward FFT -> phase -> inverse FFT along that axis alone.
+//   The density transform is a packed real-to-complex transform along axis 0 (two real lines
+//   in one complex line); eq. (2) is solved in a fused forward -> D/(C-k^2) -> inverse pass
+//   along the contiguous axis of the half spectrum.
+#include "sn_fft_core.cuh"
+#include "sn_launch.h"
+
+#ifndef SN_LEN
+#error "compile with -DSN_LEN=<line length>"
+#endif
+
+namespace snk {
+
+// ---------------------------------------------------------------------------- helpers
+
+__device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
+__device__ __forceinline__ float4 pack4(float2 a, float2 b) { return make_float4(a.x, a.y, b.x, b.y); }
+__device__ __forceinline__ float abs2(float2 v) { return fmaf(v.x, v.x, v.y * v.y); }
+
+// psi *= exp(i theta), theta/2 = hb*phi + rho*poly(rho).  Written as psi + psi*(e^{i theta}-1)
+// with e^{i theta} - 1 = (-2 sin^2(theta/2), 2 sin(theta/2) cos(theta/2)), so the rounding
+// error of the update scales with |theta| and |e^{i theta}| carries no bias from cos ~ 1.
+__device__ __forceinline__ float2 nl_phase(float2 psi, float phi, const NLParams &nl)
+{
+    const float rho = abs2(psi);
+    const float poly = fmaf(rho, fmaf(rho, fmaf(rho, nl.hg[3], nl.hg[2]), nl.hg[1]), nl.hg[0]);
+    const float th = fmaf(nl.hb, phi, rho * poly);
+    float sh, ch;
+    sincosf(th, &sh, &ch);
+    const float cm1 = -2.f * sh * sh, s = 2.f * sh * ch;
+    return make_float2(psi.x + fmaf(psi.x, cm1, -psi.y * s), psi.y + fmaf(psi.y, cm1, psi.x * s));
+}
+
+// block-wide sum of up to 3 doubles, one atomicAdd per block and value
+template <int NV>
+__device__ __forceinline__ void block_accumulate(double (&v)[NV], double *out)
+{
+    __shared__ double red[NV][32];
+#pragma unroll
+    for (int i = 0; i < NV; i++) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[i] += __shfl_xor_sync(0xffffffffu, v[i], o);
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+    if (lane == 0)
+        for (int i = 0; i < NV; i++) red[i][warp] = v[i];
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int i = 0; i < NV; i++) {
+            double s = lane < nw ? red[i][lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (lane == 0) atomicAdd(out + i, s);
+        }
+    }
+}
+
+__host__ __device__ constexpr int cp_for(int N) { return N <= 512 ? 8 : (4096 / N); }
+
+// ---------------------------------------------------------------------------- strided axis
+// Tile: N rows (points of the line, `row_stride` elements apart) x 2*CP adjacent columns.
+// Thread (t, j): column pair t, points j + T*m.  All global accesses are 128-bit; 8 adjacent
+// lanes read/write one 128-byte row segment.
+
+template <int N, int CP, int MODE, int DIR, bool HILO>
+__global__ void __launch_bounds__(CP *N / 8, 1) k_strided(const PassArgs p)
+{
+    extern __shared__ float4 smem[];
+    constexpr int T = N / 8;
+    const int t = threadIdx.x % CP, j = threadIdx.x / CP;
+    const int tiles_per_outer = p.ncols / (2 * CP);
+    const int outer = blockIdx.x / tiles_per_outer, tile = blockIdx.x % tiles_per_outer;
+    float4 *g4 = reinterpret_cast<float4 *>(p.data + (long long)outer * p.outer_stride + (long long)tile * 2 * CP) + t;
+    const long long rs4 = p.row_stride / 2;
+    SmemTile<CP> sm{smem, t};
+
+    float2 a[8], b[8];
+#pragma unroll
+    for (int m = 0; m < 8; m++) {
+        const float4 v = g4[(long long)(j + T * m) * rs4];
+        a[m] = lo2(v);
+        b[m] = hi2(v);
+    }
+    if (MODE == P_S_FFT) {
+        fft_pair<N, DIR, HILO>(a, b, j, p.tw, sm);
+        const float s = p.scale;
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            if (DIR < 0) {
+                a[m].x *= s; a[m].y *= s; b[m].x *= s; b[m].y *= s;
+            }
+            g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
+        }
+    } else if (MODE == P_S_KIN) {
+        fft_pair<N, +1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 ph = __ldg(p.phase + j + T * m);
+            a[m] = twmul<+1, true>(a[m], ph);
+            b[m] = twmul<+1, true>(b[m], ph);
+        }
+        fft_pair<N, -1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
+    } else { // P_S_KDIAG
+        fft_pair<N, +1, true>(a, b, j, p.tw, sm);
+        float acc = 0.f;
+#pragma unroll
+        for (int m = 0; m < 8; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
+        double v[1] = {(double)acc};
+        block_accumulate<1>(v, p.diag);
+    }
+}
+
+// ---------------------------------------------------------------------------- axis 0 ("h") kernels
+// Tile: N rows x 4*CP columns = two half-tiles of CP column pairs.  Thread (t, j) owns column
+// pairs t (columns 2t, 2t+1) and CP + t of the tile.  Two REAL columns 2t, 2t+1 travel as one
+// complex line re + i im, so the four real columns of a thread are one fft_pair.
+//
+// Packed real transforms (two-for-one trick): Z = FFT(x + i y), x, y real =>
+//   X[k] = (Z[k] + conj Z[N-k])/2,  Y[k] = (Z[k] - conj Z[N-k])/(2i),  k = 0..N/2;
+// inverse: Z[k] = X[k] + i Y[k] (k <= N/2), Z[N-k] = conj X[k] + i conj Y[k].
+// The factor 1/2 is folded into the Poisson multiplier (PassArgs::pscale).
+
+template <int N, int CP, class SM>
+__device__ __forceinline__ void c2r_potential(const PassArgs &p, const float4 *hs4, long long rs4, int t, int j,
+                                              float2 (&fa)[8], float2 (&fb)[8], SM &sm)
+{
+    constexpr int T = N / 8;
+#pragma unroll
+    for (int m = 0; m < 8; m++) {
+        const int km = j + T * m;
+        const int src = m < 4 ? km : N - km; // m >= 4: km >= N/2, mirrored row in [0, N/2]
+        const float4 u = hs4[(long long)src * rs4 + t];
+        const float4 v = hs4[(long long)src * rs4 + CP + t];
+        if (m < 4) {
+            fa[m] = make_float2(u.x - u.w, u.y + u.z);
+            fb[m] = make_float2(v.x - v.w, v.y + v.z);
+        } else {
+            fa[m] = make_float2(u.x + u.w, u.z - u.y);
+            fb[m] = make_float2(v.x + v.w, v.z - v.y);
+        }
+    }
+    fft_pair<N, -1, false>(fa, fb, j, p.tw, sm);
+    // now fa[m] = (phi[col 2t], phi[col 2t+1]), fb[m] = same for column pair CP+t, at row j+T*m
+}
+
+template <int N, int CP, int MODE>
+__global__ void __launch_bounds__(CP *N / 8, 1) k_haxis(const PassArgs p)
+{
+    extern __shared__ float4 smem[];
+    constexpr int T = N / 8;
+    const int t = threadIdx.x % CP, j = threadIdx.x / CP;
+    const long long rs4 = p.row_stride / 2;
+    const long long col4 = (long long)blockIdx.x * 2 * CP; // first column pair of the tile
+    float4 *psi4 = reinterpret_cast<float4 *>(p.data) + col4;
+    float4 *hs4 = reinterpret_cast<float4 *>(p.hs) + col4;
+    SmemTile<CP> sm{smem, t};
+
+    if (MODE == P_H_R2C) {
+        float2 a[8], b[8];
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
+            const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
+            a[m] = make_float2(abs2(lo2(u)), abs2(hi2(u)));
+            b[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+        }
+        fft_pair<N, +1, false>(a, b, j, p.tw, sm);
+        sm.sync();
+#pragma unroll
+        for (int m = 0; m < 8; m++) sm.st(j + T * m, a[m], b[m]);
+        sm.sync();
+#pragma unroll
+        for (int m = 0; m < 5; m++) {
+            if (m < 4 || j == 0) {
+                const int k = j + T * m;
+                float2 ya, yb;
+                sm.ld((N - k) & (N - 1), ya, yb);
+                hs4[(long long)k * rs4 + t] = make_float4(a[m].x + ya.x, a[m].y - ya.y, a[m].y + ya.y, ya.x - a[m].x);
+                hs4[(long long)k * rs4 + CP + t] =
+                    make_float4(b[m].x + yb.x, b[m].y - yb.y, b[m].y + yb.y, yb.x - b[m].x);
+            }
+        }
+        return;
+    }
+
+    float2 fa[8], fb[8];
+    c2r_potential<N, CP>(p, hs4, rs4, t, j, fa, fb, sm);
+
+    if (MODE == P_H_POT) {
+        float2 *out = reinterpret_cast<float2 *>(p.phi_out) + col4;
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            out[(long long)(j + T * m) * rs4 + t] = fa[m];
+            out[(long long)(j + T * m) * rs4 + CP + t] = fb[m];
+        }
+        return;
+    }
+    if (MODE == P_H_DIAG) {
+        float s_rho = 0.f, s_pr = 0.f, s_f = 0.f;
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
+            const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
+            const float r[4] = {abs2(lo2(u)), abs2(hi2(u)), abs2(lo2(v)), abs2(hi2(v))};
+            const float ph[4] = {fa[m].x, fa[m].y, fb[m].x, fb[m].y};
+#pragma unroll
+            for (int c = 0; c < 4; c++) {
+                s_rho += r[c];
+                s_pr = fmaf(ph[c], r[c], s_pr);
+                const float f = fmaf(r[c], fmaf(r[c], fmaf(r[c], p.nl.fg[3], p.nl.fg[2]), p.nl.fg[1]), p.nl.fg[0]);
+                s_f = fmaf(r[c] * r[c], f, s_f);
+            }
+        }
+        double v[3] = {(double)s_rho, (double)s_pr, (double)s_f};
+        block_accumulate<3>(v, p.diag);
+        return;
+    }
+
+    // P_H_NLKIN: nonlinear phase with phi, then the axis-0 kinetic pass, half-tile by half-tile
+#pragma unroll
+    for (int half = 0; half < 2; half++) {
+        float4 *g4 = psi4 + half * CP + t;
+        float2 a[8], b[8];
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 v = g4[(long long)(j + T * m) * rs4];
+            const float2 ph = half == 0 ? fa[m] : fb[m];
+            a[m] = nl_phase(lo2(v), ph.x, p.nl);
+            b[m] = nl_phase(hi2(v), ph.y, p.nl);
+        }
+        fft_pair<N, +1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 ph = __ldg(p.phase + j + T * m);
+            a[m] = twmul<+1, true>(a[m], ph);
+            b[m] = twmul<+1, true>(b[m], ph);
+        }
+        fft_pair<N, -1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
+    }
+}
+
+// ---------------------------------------------------------------------------- contiguous axis
+// A group of T = N/8 threads owns two adjacent lines; lanes are consecutive j, so every global
+// access of a warp is one contiguous 256-byte run of a line.
+
+__host__ __device__ constexpr int xthreads(int N) { return N / 8 >= 256 ? N / 8 : 256; }
+
+template <int N, int MODE, int DIR, bool HILO>
+__global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_contig(const PassArgs p)
+{
+    extern __shared__ float4 smem[];
+    constexpr int T = N / 8, G = xthreads(N) / T;
+    const int j = threadIdx.x % T, grp = threadIdx.x / T;
+    const long long pair = (long long)blockIdx.x * G + grp;
+    const bool active = 2 * pair < p.nlines;
+    if (MODE != P_X_KDIAG && !active) return;
+    float2 *la = p.data + (active ? 2 * pair : 0) * N;
+    float2 *lb = la + N;
+    SmemLine<T> sm{smem + grp * N, 1 + grp, G == 1};
+
+    float2 a[8], b[8];
+#pragma unroll
+    for (int m = 0; m < 8; m++) {
+        a[m] = la[j + T * m];
+        b[m] = lb[j + T * m];
+    }
+    if (MODE == P_X_FFT) {
+        fft_pair<N, DIR, HILO>(a, b, j, p.tw, sm);
+        const float s = p.scale;
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            if (DIR < 0) {
+                a[m].x *= s; a[m].y *= s; b[m].x *= s; b[m].y *= s;
+            }
+            la[j + T * m] = a[m];
+            lb[j + T * m] = b[m];
+        }
+    } else if (MODE == P_X_KIN) {
+        fft_pair<N, +1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 ph = __ldg(p.phase + j + T * m);
+            a[m] = twmul<+1, true>(a[m], ph);
+            b[m] = twmul<+1, true>(b[m], ph);
+        }
+        fft_pair<N, -1, true>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            la[j + T * m] = a[m];
+            lb[j + T * m] = b[m];
+        }
+    } else if (MODE == P_X_POISSON) {
+        // eq. (2) in Fourier space: phi^ = D rho^/(C - k^2); C == 0: phi^(k=0) = 0
+        fft_pair<N, +1, false>(a, b, j, p.tw, sm);
+        const float ka = __ldg(p.kother2 + 2 * pair), kb = __ldg(p.kother2 + 2 * pair + 1);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float kx2 = __ldg(p.ksq + j + T * m);
+            const float da = p.C - kx2 - ka, db = p.C - kx2 - kb;
+            const float ga = da == 0.f ? 0.f : p.pscale / da;
+            const float gb = db == 0.f ? 0.f : p.pscale / db;
+            a[m].x *= ga; a[m].y *= ga; b[m].x *= gb; b[m].y *= gb;
+        }
+        fft_pair<N, -1, false>(a, b, j, p.tw, sm);
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            la[j + T * m] = a[m];
+            lb[j + T * m] = b[m];
+        }
+    } else { // P_X_KDIAG
+        fft_pair<N, +1, true>(a, b, j, p.tw, sm);
+        float acc = 0.f;
+#pragma unroll
+        for (int m = 0; m < 8; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
+        double v[1] = {active ? (double)acc : 0.0};
+        block_accumulate<1>(v, p.diag);
+    }
+}
+
+// ---------------------------------------------------------------------------- launchers
+
+template <class K>
+static int launch_kernel(K kern, unsigned grid, int threads, size_t smem_bytes, const PassArgs &a)
+{
+    if (smem_bytes > 48 * 1024) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return (int)e;
+    }
+    kern<<<grid, threads, smem_bytes, a.stream>>>(a);
+    return (int)cudaGetLastError();
+}
+
+template <int N>
+int launch_pass(const PassArgs &a)
+{
+    constexpr int CP = cp_for(N), T = N / 8;
+    constexpr int ST = CP * T;                       // threads of a strided-axis CTA
+    constexpr size_t SSMEM = (size_t)N * CP * 16;    // one float4 per point and column pair
+    constexpr int XT = xthreads(N), G = XT / T;
+    constexpr size_t XSMEM = (size_t)N * G * 16;
+    switch (a.kind) {
+    case P_S_FFT:
+    case P_S_KIN:
+    case P_S_KDIAG: {
+        const unsigned grid = (unsigned)((long long)a.n_outer * (a.ncols / (2 * CP)));
+        if (a.kind == P_S_KIN) return launch_kernel(k_strided<N, CP, P_S_KIN, +1, true>, grid, ST, SSMEM, a);
+        if (a.kind == P_S_KDIAG) return launch_kernel(k_strided<N, CP, P_S_KDIAG, +1, true>, grid, ST, SSMEM, a);
+        if (a.dir > 0)
+            return a.hilo ? launch_kernel(k_strided<N, CP, P_S_FFT, +1, true>, grid, ST, SSMEM, a)
+                          : launch_kernel(k_strided<N, CP, P_S_FFT, +1, false>, grid, ST, SSMEM, a);
+        return a.hilo ? launch_kernel(k_strided<N, CP, P_S_FFT, -1, true>, grid, ST, SSMEM, a)
+                      : launch_kernel(k_strided<N, CP, P_S_FFT, -1, false>, grid, ST, SSMEM, a);
+    }
+    case P_H_NLKIN:
+    case P_H_R2C:
+    case P_H_POT:
+    case P_H_DIAG: {
+        const unsigned grid = (unsigned)(a.ncols / (4 * CP));
+        if (a.kind == P_H_NLKIN) return launch_kernel(k_haxis<N, CP, P_H_NLKIN>, grid, ST, SSMEM, a);
+        if (a.kind == P_H_R2C) return launch_kernel(k_haxis<N, CP, P_H_R2C>, grid, ST, SSMEM, a);
+        if (a.kind == P_H_POT) return launch_kernel(k_haxis<N, CP, P_H_POT>, grid, ST, SSMEM, a);
+        return launch_kernel(k_haxis<N, CP, P_H_DIAG>, grid, ST, SSMEM, a);
+    }
+    case P_X_FFT:
+    case P_X_KIN:
+    case P_X_POISSON:
+    case P_X_KDIAG: {
+        const long long pairs = a.nlines / 2;
+        const unsigned grid = (unsigned)((pairs + G - 1) / G);
+        if (a.kind == P_X_KIN) return launch_kernel(k_contig<N, P_X_KIN, +1, true>, grid, XT, XSMEM, a);
+        if (a.kind == P_X_POISSON) return launch_kernel(k_contig<N, P_X_POISSON, +1, false>, grid, XT, XSMEM, a);
+        if (a.kind == P_X_KDIAG) return launch_kernel(k_contig<N, P_X_KDIAG, +1, true>, grid, XT, XSMEM, a);
+        return a.dir > 0 ? launch_kernel(k_contig<N, P_X_FFT, +1, true>, grid, XT, XSMEM, a)
+                         : launch_kernel(k_contig<N, P_X_FFT, -1, true>, grid, XT, XSMEM, a);
+    }
+    default:
+        return (int)cudaErrorInvalidValue;
+    }
+}
+
+template int launch_pass<SN_LEN>(const PassArgs &a);
+
+} // namespace snk

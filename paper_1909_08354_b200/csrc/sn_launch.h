@@ -1,0 +1,58 @@
+// sn_launch.h -- internal interface between the scheduler (sn_api.cu) and the per-length kernel
+// translation units (sn_kernels.cu compiled once per line length with -DSN_LEN=N).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace snk {
+
+enum PassKind {
+    P_S_FFT = 0,   // strided axis: plain c2c transform (dir, hilo, scale)
+    P_S_KIN,       // strided axis: forward -> kinetic phase -> inverse            (S1-S3 per axis)
+    P_S_KDIAG,     // strided axis: forward, accumulate sum k_a^2 |psi^|^2         (S12)
+    P_H_NLKIN,     // axis 0: c2r of phi^ -> nonlinear phase -> fwd -> phase -> inv (S7,S8,S1-S3)
+    P_H_R2C,       // axis 0: rho = |psi|^2 -> packed r2c -> half spectrum          (S4,S5)
+    P_H_POT,       // axis 0: c2r of phi^ -> phi (float) out                        (test hook)
+    P_H_DIAG,      // axis 0: c2r of phi^ -> sums of rho, phi rho, F(rho)           (S12)
+    P_X_FFT,       // contiguous axis: plain c2c transform
+    P_X_KIN,       // contiguous axis: forward -> kinetic phase -> inverse
+    P_X_POISSON,   // contiguous axis of the half spectrum: forward -> D/(C-k^2) -> inverse (S5-S7)
+    P_X_KDIAG      // contiguous axis: forward, accumulate sum k_x^2 |psi^|^2
+};
+
+// Nonlinear phase psi *= exp(-i dtau (B phi + sum_j g_j rho^j)), stored as HALF-angle
+// coefficients: theta/2 = hb * phi + rho (hg[0] + rho (hg[1] + rho (hg[2] + rho hg[3]))).
+struct NLParams {
+    float hb;
+    float hg[4];
+    float fg[4]; // F(rho) = rho^2 (fg[0] + rho (fg[1] + ...)), fg[j] = g_j/(j+2)   (diagnostics)
+};
+
+struct PassArgs {
+    int kind;
+    int dir;  // +1 forward, -1 inverse (P_S_FFT / P_X_FFT)
+    int hilo; // 1: hi/lo twiddles (psi transforms); 0: plain (density / potential transforms)
+    float2 *data;      // DEVICE: array transformed in place (psi, or the half spectrum)
+    float2 *hs;        // DEVICE: half-spectrum buffer (P_H_* kinds)
+    long long row_stride;   // elements between consecutive points of a line (strided kinds)
+    long long outer_stride; // elements between outer blocks
+    int ncols;              // contiguous columns per outer block
+    int n_outer;
+    int nlines;             // contiguous kinds: number of lines (even)
+    const float4 *tw;       // DEVICE: twiddle table for this length
+    const float4 *phase;    // DEVICE: kinetic phase table (hi/lo, includes 1/N)
+    const float *ksq;       // DEVICE: k_a^2 per index of this axis
+    const float *kother2;   // DEVICE: P_X_POISSON: sum of the other axes' k^2 per line
+    float scale;            // P_*_FFT: output scale (1/N on inverse)
+    float C;                // eq. (2) constant
+    float pscale;           // P_X_POISSON: D * 0.5 / prod(N)   (0.5 from the packed r2c)
+    NLParams nl;
+    float *phi_out;         // DEVICE: P_H_POT
+    double *diag;           // DEVICE: accumulators
+    cudaStream_t stream;
+};
+
+// Returns cudaError_t as int.  Explicitly instantiated for N in {64,...,4096}.
+template <int N>
+int launch_pass(const PassArgs &a);
+
+} // namespace snk

@@ -1,0 +1,181 @@
+"""Thin ctypes binding of libsn.so (include/sn.h) -- argument marshalling only.
+
+PyTorch is used for exactly two things: the device workspace (one uint8 tensor) and the CUDA
+stream.  Every step of the split-step path (eq. (1),(2)) runs in
+the library's hand-written sm_100a kernels.  There is no CPU fallback: if libsn.so is missing
+or no CUDA device is present this module raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsn.so")
+
+SN_OK = 0
+ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_ERR_SINGULAR",
+             -5: "SN_ERR_WORKSPACE", -6: "SN_ERR_STATE", -7: "SN_ERR_CUDA"}
+
+# every symbol include/sn.h declares
+EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
+           "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_debug_fft", "sn_debug_potential")
+
+
+class SnDiag(ctypes.Structure):
+    _fields_ = [("norm", ctypes.c_double), ("e_kin", ctypes.c_double), ("e_nonlocal", ctypes.c_double),
+                ("e_local", ctypes.c_double), ("e_total", ctypes.c_double)]
+
+
+class SnError(RuntimeError):
+    def __init__(self, code: int, what: str, text: str = ""):
+        super().__init__(f"{what}: {ERR_NAMES.get(code, code)} {text}".strip())
+        self.code = code
+
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+def lib() -> ctypes.CDLL:
+    """Load libsn.so (built by paper_1909_08354_b200.build); fail loudly if it is missing."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_1909_08354_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64p, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_double)
+        L.sn_workspace_bytes.argtypes = [ctypes.c_int, i64p]
+        L.sn_workspace_bytes.restype = ctypes.c_size_t
+        L.sn_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_double, ctypes.c_double,
+                                ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, vp,
+                                ctypes.c_size_t, vp]
+        L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
+        L.sn_step.argtypes = [vp, ctypes.c_int64]
+        L.sn_get_state.argtypes = [vp, vp, ctypes.c_int]
+        L.sn_diagnostics.argtypes = [vp, ctypes.POINTER(SnDiag)]
+        L.sn_set_dtau.argtypes = [vp, ctypes.c_double]
+        L.sn_destroy.argtypes = [vp]
+        L.sn_strerror.argtypes = [ctypes.c_int]
+        L.sn_strerror.restype = ctypes.c_char_p
+        L.sn_launch_count.argtypes = [vp]
+        L.sn_launch_count.restype = ctypes.c_int64
+        L.sn_debug_fft.argtypes = [vp, ctypes.c_int]
+        L.sn_debug_potential.argtypes = [vp, vp, ctypes.c_int]
+        _lib = L
+    return _lib
+
+
+def _chk(rc: int, what: str) -> None:
+    if rc != SN_OK:
+        raise SnError(rc, what, lib().sn_strerror(rc).decode())
+
+
+def workspace_bytes(dims: Sequence[int]) -> int:
+    d = (ctypes.c_int64 * len(dims))(*[int(n) for n in dims])
+    return int(lib().sn_workspace_bytes(len(dims), d))
+
+
+class Simulation:
+    """One sn_ctx plus the torch tensor that backs its workspace."""
+
+    def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float, g: Sequence[float],
+                 dtau: float, device: str = "cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1909_08354_b200 needs a CUDA device (no CPU fallback)")
+        self.dims = tuple(int(n) for n in dims)
+        nd = len(self.dims)
+        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
+        g = [float(v) for v in g]
+        self.device = torch.device(device)
+        nbytes = workspace_bytes(self.dims)
+        if nbytes == 0:
+            raise SnError(-2, "sn_workspace_bytes", lib().sn_strerror(-2).decode())
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._h = ctypes.c_void_p()
+        c_dims = (ctypes.c_int64 * nd)(*self.dims)
+        c_L = (ctypes.c_double * nd)(*Ls)
+        c_g = (ctypes.c_double * max(1, len(g)))(*(g or [0.0]))
+        with torch.cuda.device(self.device):
+            _chk(lib().sn_create(ctypes.byref(self._h), nd, c_dims, c_L, A, B, C, D, c_g, len(g), dtau,
+                                 ctypes.c_void_p(self._ws.data_ptr()), nbytes,
+                                 ctypes.c_void_p(self._stream.cuda_stream)), "sn_create")
+
+    @classmethod
+    def from_config(cls, cfg, **kw) -> "Simulation":
+        return cls(cfg.dims, cfg.L, cfg.A, cfg.B, cfg.C, cfg.D, cfg.g, cfg.dtau, **kw)
+
+    @property
+    def cells(self) -> int:
+        return int(np.prod(self.dims))
+
+    def close(self) -> None:
+        if getattr(self, "_h", None):
+            lib().sn_destroy(self._h)
+            self._h = ctypes.c_void_p()
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- state ------------------------------------------------------------------------------
+    def set_state(self, psi) -> None:
+        """psi: numpy complex64 array (host) or torch complex64 CUDA tensor, shape == dims."""
+        if isinstance(psi, np.ndarray):
+            a = np.ascontiguousarray(psi, dtype=np.complex64)
+            assert a.shape == self.dims, (a.shape, self.dims)
+            _chk(lib().sn_set_state(self._h, ctypes.c_void_p(a.ctypes.data), 0), "sn_set_state")
+        else:
+            import torch
+            if psi.is_cuda:
+                assert psi.dtype == torch.complex64 and psi.is_contiguous() and tuple(psi.shape) == self.dims
+                _chk(lib().sn_set_state(self._h, ctypes.c_void_p(psi.data_ptr()), 1), "sn_set_state")
+            else:  # host torch tensor (e.g. pinned)
+                assert psi.dtype == torch.complex64 and psi.is_contiguous() and tuple(psi.shape) == self.dims
+                _chk(lib().sn_set_state(self._h, ctypes.c_void_p(psi.data_ptr()), 0), "sn_set_state")
+
+    def get_state(self, out=None):
+        """Return the state as a numpy complex64 array, or fill `out` (numpy / torch host or CUDA tensor)."""
+        if out is None:
+            out = np.empty(self.dims, dtype=np.complex64)
+        if isinstance(out, np.ndarray):
+            assert out.dtype == np.complex64 and out.flags.c_contiguous and out.shape == self.dims
+            _chk(lib().sn_get_state(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_get_state")
+        else:
+            _chk(lib().sn_get_state(self._h, ctypes.c_void_p(out.data_ptr()), 1 if out.is_cuda else 0),
+                 "sn_get_state")
+        return out
+
+    # -- the path ---------------------------------------------------------------------------
+    def step(self, n: int) -> None:
+        _chk(lib().sn_step(self._h, int(n)), "sn_step")
+
+    def set_dtau(self, dtau: float) -> None:
+        _chk(lib().sn_set_dtau(self._h, float(dtau)), "sn_set_dtau")
+
+    def diagnostics(self) -> dict:
+        d = SnDiag()
+        _chk(lib().sn_diagnostics(self._h, ctypes.byref(d)), "sn_diagnostics")
+        return {k: getattr(d, k) for k, _ in SnDiag._fields_}
+
+    def launch_count(self) -> int:
+        return int(lib().sn_launch_count(self._h))
+
+    # -- test hooks ---------------------------------------------------------------------------
+    def debug_fft(self, direction: int) -> None:
+        _chk(lib().sn_debug_fft(self._h, int(direction)), "sn_debug_fft")
+
+    def debug_potential(self) -> np.ndarray:
+        out = np.empty(self.dims, dtype=np.float32)
+        _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_debug_potential")
+        return out
