@@ -93,6 +93,21 @@ const char *sn_strerror(int code);
 /* Number of kernels this context has launched since creation (for bench.py's gpu_launches). */
 int64_t sn_launch_count(const sn_ctx *ctx);
 
+/* ---- per-launch timing (bench.py's roofline) ----
+ * With profiling enabled every kernel launch is bracketed by a cudaEvent pair on the context's
+ * stream; sn_profile_read synchronises and returns, per pass kind, the summed device time in
+ * milliseconds and the number of launches since the last reset.  Pass kinds (index):
+ *   0 S_FFT  strided-axis plain transform          1 S_KIN  strided-axis forward-phase-inverse
+ *   2 S_KDIAG strided-axis kinetic-energy sum      3 H_NLKIN axis-0 c2r + nonlinear phase + kinetic
+ *   4 H_R2C  axis-0 density + packed r2c           5 H_POT  axis-0 c2r -> phi (test hook)
+ *   6 H_DIAG axis-0 c2r + energy sums              7 X_FFT  contiguous-axis plain transform
+ *   8 X_KIN  contiguous-axis forward-phase-inverse 9 X_POISSON contiguous-axis forward-D/(C-k^2)-inverse
+ *  10 X_KDIAG contiguous-axis kinetic-energy sum */
+#define SN_NUM_PASS_KINDS 11
+int sn_profile(sn_ctx *ctx, int enable);
+int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 11 */, int64_t *launches_by_kind /* host, 11 */,
+                    int reset);
+
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */
 
 /* In-place d-dimensional FFT of the internal state: direction +1 forward (e^{-i k x}, unscaled),

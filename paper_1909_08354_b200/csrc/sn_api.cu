@@ -104,6 +104,12 @@ struct sn_ctx {
     const float4 *tw[3], *ph_full[3], *ph_half[3];
     const float *ksq[3], *kother;
     double *diag;
+    // optional per-launch timing (sn_profile): event pairs around every launch, summed per pass kind
+    bool profiling;
+    std::vector<cudaEvent_t> *ev;       // pool, pairs (start, stop)
+    std::vector<int> *ev_kind;          // pass kind of each recorded pair
+    double prof_ms[SN_NUM_PASS_KINDS];
+    int64_t prof_launches[SN_NUM_PASS_KINDS];
 };
 
 namespace {
@@ -119,7 +125,44 @@ int cuda_fail(cudaError_t e)
         if (e_ != cudaSuccess) return cuda_fail(e_);    \
     } while (0)
 
+// fold the recorded event pairs into the per-kind sums (synchronises the stream)
+int profile_flush(sn_ctx *c)
+{
+    if (!c->ev || c->ev_kind->empty()) return SN_OK;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    for (size_t i = 0; i < c->ev_kind->size(); i++) {
+        float ms = 0.f;
+        SN_CUDA(cudaEventElapsedTime(&ms, (*c->ev)[2 * i], (*c->ev)[2 * i + 1]));
+        c->prof_ms[(*c->ev_kind)[i]] += ms;
+        c->prof_launches[(*c->ev_kind)[i]]++;
+    }
+    c->ev_kind->clear();
+    return SN_OK;
+}
+
+int run_pass_raw(sn_ctx *c, int N, PassArgs &a);
+
 int run_pass(sn_ctx *c, int N, PassArgs &a)
+{
+    if (!c->profiling) return run_pass_raw(c, N, a);
+    const size_t i = c->ev_kind->size();
+    if (c->ev->size() < 2 * (i + 1)) {
+        cudaEvent_t e0, e1;
+        SN_CUDA(cudaEventCreate(&e0));
+        SN_CUDA(cudaEventCreate(&e1));
+        c->ev->push_back(e0);
+        c->ev->push_back(e1);
+    }
+    SN_CUDA(cudaEventRecord((*c->ev)[2 * i], c->stream));
+    const int rc = run_pass_raw(c, N, a);
+    if (rc) return rc;
+    SN_CUDA(cudaEventRecord((*c->ev)[2 * i + 1], c->stream));
+    c->ev_kind->push_back(a.kind);
+    if (c->ev_kind->size() >= 8192) return profile_flush(c);
+    return SN_OK;
+}
+
+int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
 {
     a.stream = c->stream;
     int rc;
@@ -366,6 +409,11 @@ int sn_destroy(sn_ctx *c)
 {
     if (!c) return SN_ERR_NULL;
     cudaStreamSynchronize(c->stream);
+    if (c->ev) {
+        for (cudaEvent_t e : *c->ev) cudaEventDestroy(e);
+        delete c->ev;
+        delete c->ev_kind;
+    }
     delete c;
     return SN_OK;
 }
@@ -502,6 +550,38 @@ int sn_diagnostics(sn_ctx *c, sn_diag *out)
 }
 
 int64_t sn_launch_count(const sn_ctx *c) { return c ? c->launches : 0; }
+
+int sn_profile(sn_ctx *c, int enable)
+{
+    if (!c) return SN_ERR_NULL;
+    if (enable && !c->ev) {
+        c->ev = new (std::nothrow) std::vector<cudaEvent_t>();
+        c->ev_kind = new (std::nothrow) std::vector<int>();
+        if (!c->ev || !c->ev_kind) return SN_ERR_PARAM;
+    }
+    if (!enable && c->profiling) {
+        const int rc = profile_flush(c);
+        if (rc) return rc;
+    }
+    c->profiling = enable != 0;
+    return SN_OK;
+}
+
+int sn_profile_read(sn_ctx *c, double *ms_by_kind, int64_t *launches_by_kind, int reset)
+{
+    if (!c || !ms_by_kind || !launches_by_kind) return SN_ERR_NULL;
+    const int rc = profile_flush(c);
+    if (rc) return rc;
+    for (int k = 0; k < SN_NUM_PASS_KINDS; k++) {
+        ms_by_kind[k] = c->prof_ms[k];
+        launches_by_kind[k] = c->prof_launches[k];
+        if (reset) {
+            c->prof_ms[k] = 0.0;
+            c->prof_launches[k] = 0;
+        }
+    }
+    return SN_OK;
+}
 
 const char *sn_strerror(int code)
 {

@@ -22,7 +22,11 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
-           "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_debug_fft", "sn_debug_potential")
+           "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
+           "sn_debug_fft", "sn_debug_potential")
+
+PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
+              "X_KDIAG")
 
 
 class SnDiag(ctypes.Structure):
@@ -63,6 +67,8 @@ def lib() -> ctypes.CDLL:
         L.sn_strerror.restype = ctypes.c_char_p
         L.sn_launch_count.argtypes = [vp]
         L.sn_launch_count.restype = ctypes.c_int64
+        L.sn_profile.argtypes = [vp, ctypes.c_int]
+        L.sn_profile_read.argtypes = [vp, dp, i64p, ctypes.c_int]
         L.sn_debug_fft.argtypes = [vp, ctypes.c_int]
         L.sn_debug_potential.argtypes = [vp, vp, ctypes.c_int]
         _lib = L
@@ -170,6 +176,17 @@ class Simulation:
 
     def launch_count(self) -> int:
         return int(lib().sn_launch_count(self._h))
+
+    def profile(self, enable: bool) -> None:
+        _chk(lib().sn_profile(self._h, 1 if enable else 0), "sn_profile")
+
+    def profile_read(self, reset: bool = True) -> dict:
+        """{pass kind: (summed device ms, launches)} for kinds that ran."""
+        n = len(PASS_KINDS)
+        ms = (ctypes.c_double * n)()
+        cnt = (ctypes.c_int64 * n)()
+        _chk(lib().sn_profile_read(self._h, ms, cnt, 1 if reset else 0), "sn_profile_read")
+        return {PASS_KINDS[k]: (float(ms[k]), int(cnt[k])) for k in range(n) if cnt[k]}
 
     # -- test hooks ---------------------------------------------------------------------------
     def debug_fft(self, direction: int) -> None:
