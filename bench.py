@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- split-step cell-updates/s of the B200 Schroedinger-Newton stepper (libsn.so).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5_512] [--impl reference]
+
+A bench "step" is one full Strang step K(dtau/2) N(dtau) K(dtau/2) of PAPER.md:42-44 eq. (1),(2)
+(method: PAPER.md:113) over the whole grid, i.e. one pass of every row S1-S11 of SURVEY.md 8(a).
+The timed region is ONE sn_step(K) call (adjacent half kinetics merged inside the call, as a user
+would run it) bracketed by barrier + synchronize, CUDA events on the stream the kernels run on.
+Default workload: BASELINE.json configs[4] at 512^3 (the size north_star's 60 % HBM target names);
+the state (1 GiB) is far larger than L2 (126 MB), so no L2 flush is needed between steps.
+
+One JSON line on stdout (rank 0).  Extra objects: roofline (dominant kernel, per-launch CUDA
+events measured in a second K-step run right after the timed one), cpu_baseline (the float64
+oracle as it stands, on the host cores, on a bounded sample), e2e (sn_set_state from pinned
+host memory + sn_step(K) + sn_get_state to pinned host memory + sn_diagnostics, all inside the
+timed region), clocks (NVML samples during the timed region).
+
+Multi-GPU: the path does not shard (every transform is global; "replicas only");
+--gpus N runs N independent replicas, one per rank, with no data-path collective.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "split-step cell-updates/sec (complex64)"
+UNIT = "cell-updates/s"
+
+# Algorithmic bytes per cell of each pass kind (complex64 = 8 B, half spectrum
+# = 4 B per cell of the full grid).  hs = the half-spectrum array, (N0/2+1)/N0 of a full complex array.
+PASS_BYTES_PER_CELL = {
+    "H_NLKIN": 20.0,   # read phi^ (4) + read psi (8) + write psi (8)
+    "S_KIN": 16.0,     # read + write psi
+    "X_KIN": 16.0,
+    "H_R2C": 12.0,     # read psi (8) + write rho^ (4)
+    "S_FFT": 8.0,      # read + write half spectrum
+    "X_POISSON": 8.0,
+}
+B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, copy read+write)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """NVML samples of SM clock and throttle reasons while the timed region runs."""
+
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            self._stop.wait(0.01)
+
+    def __enter__(self):
+        if self._nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        return {"sm_mhz": int(statistics.median(self.samples)) if self.samples else None,
+                "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def oracle_rate(cfg_name: str, budget_s: float, inputs):
+    """Time the float64 oracle as it stands on a bounded sample of the workload (host cores)."""
+    from oracle import snref  # test infrastructure: only this leg and --impl reference touch it
+    from oracle.snref import Oracle
+    base = inputs.CONFIGS[cfg_name]
+    # bounded sample: the same recipe (seed, constants, box) resampled so that one step is ~1 s of CPU
+    if base.cells > 128 ** 3 and len(base.dims) == 3:
+        cfg = inputs.scaled(base, (128, 128, 128))
+    elif base.cells > 1024 ** 2 and len(base.dims) == 2:
+        cfg = inputs.scaled(base, (1024, 1024), L=base.L * 1024 / base.dims[0])
+    else:
+        cfg = base
+    psi0 = cfg.initial_state().astype(np.complex128)
+    orc = Oracle.from_config(cfg)
+    orc.set_state(psi0)
+    t0 = time.perf_counter()
+    orc.step(1)
+    t1 = time.perf_counter() - t0
+    k = int(max(2, min(cfg.steps, budget_s / max(t1, 1e-6))))
+    t0 = time.perf_counter()
+    orc.step(k)
+    dt = time.perf_counter() - t0
+    orc.close()
+    return {"value": cfg.cells * k / dt, "unit": UNIT, "cores": snref.num_threads(), "kind": "oracle",
+            "sample": f"{base.name} recipe on a {'x'.join(map(str, cfg.dims))} grid, {k} Strang steps, float64, "
+                      f"{dt:.1f} s wall"}, cfg, k, dt
+
+
+def run_reference(args, inputs):
+    """--impl reference: the oracle (oracle/snref.c) timed on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    base = inputs.CONFIGS[args.workload]
+    from oracle.snref import Oracle
+    from oracle import snref
+    cfg = inputs.scaled(base, (128, 128, 128)) if (len(base.dims) == 3 and base.cells > 128 ** 3) else (
+        inputs.scaled(base, (1024, 1024), L=base.L * 1024 / base.dims[0]) if base.cells > 1024 ** 2 else base)
+    orc = Oracle.from_config(cfg)
+    orc.set_state(cfg.initial_state().astype(np.complex128))
+    orc.step(args.warmup)
+    t0 = time.perf_counter()
+    orc.step(args.steps)
+    dt = time.perf_counter() - t0
+    orc.close()
+    value = cfg.cells * args.steps / dt
+    sample = (f"each step = one float64 Strang step of the {base.name} recipe resampled on a "
+              f"{'x'.join(map(str, cfg.dims))} grid (bounded sample of {'x'.join(map(str, base.dims))})")
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": base.name, "dims": list(base.dims), "sample_dims": list(cfg.dims)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": snref.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--workload", default="C5_512")
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+
+    from paper_1909_08354_b200 import inputs
+    if args.impl == "reference":
+        run_reference(args, inputs)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1909_08354_b200 import sn
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg = inputs.CONFIGS[args.workload]
+    nd = len(cfg.dims)
+    K, W = args.steps, args.warmup
+    psi0 = cfg.initial_state()                          # seeded synthetic state, complex64
+    host_in = torch.from_numpy(psi0).pin_memory()
+    host_out = torch.empty_like(host_in).pin_memory()
+    dev_in = host_in.to(dev, non_blocking=True)
+
+    stream = torch.cuda.current_stream()
+    sim = sn.Simulation.from_config(cfg, device=dev, stream=stream)
+    sim.set_state(dev_in)
+    sim.step(W)                                         # untimed warm-up steps
+    barrier()
+
+    # ---- timed region: exactly K Strang steps, state resident in HBM ----
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = sim.launch_count()
+    with ClockSampler(local) as clk:
+        barrier()
+        e0.record(stream)
+        sim.step(K)
+        e1.record(stream)
+        barrier()
+    launches = sim.launch_count() - n0
+    ms = e0.elapsed_time(e1)
+
+    # ---- per-launch CUDA events over the same K steps (roofline of the dominant kernel) ----
+    sim.profile(True)
+    sim.step(K)
+    prof = sim.profile_read(reset=True)
+    sim.profile(False)
+    norm_after = sim.diagnostics()["norm"]
+
+    # ---- e2e: host buffers through the public API, copies inside the timed region ----
+    barrier()
+    t0 = time.perf_counter()
+    sim.set_state(host_in)
+    sim.step(K)
+    sim.get_state(host_out)
+    d = sim.diagnostics()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    sim.close()
+
+    # max over ranks
+    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms, e2e_ms = float(t[0]), float(t[1])
+
+    if rank == 0:
+        cells = cfg.cells
+        value = world * cells * K / (ms * 1e-3)
+        peak, peak_src = load_peaks()
+        tot = sum(v[0] for v in prof.values()) or 1.0
+        dom = max(prof, key=lambda k: prof[k][0])
+        dom_ms = prof[dom][0] / prof[dom][1]
+        hs_frac = (cfg.dims[0] // 2 + 1) / (cfg.dims[0] / 2)   # exact half-spectrum factor on the 4-byte terms
+        bpc = PASS_BYTES_PER_CELL[dom]
+        if dom == "H_NLKIN":
+            bpc = 16.0 + 4.0 * hs_frac
+        elif dom == "H_R2C":
+            bpc = 8.0 + 4.0 * hs_frac
+        elif dom in ("S_FFT", "X_POISSON"):
+            bpc = 8.0 * hs_frac
+        achieved = bpc * cells / (dom_ms * 1e-3) / 1e9
+        out = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
+            "config": {"workload": f"{cfg.name}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
+                                   f"B={cfg.B}, C={cfg.C}, D={cfg.D:.6g}, g={list(cfg.g)}, dtau={cfg.dtau}",
+                       "dims": list(cfg.dims), "parallelism": "replicas only" if world > 1 else "single GPU",
+                       "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
+                           cells, cells * 8 / 2 ** 20) if cells * 8 > 126e6 else
+                       "state fits L2: launch/L2-bound regime, HBM fraction is an effective figure only",
+                       "timed_call": f"one sn_step({K}) (merged half kinetics)"},
+            "gpu_launches": launches,
+            "clocks": clk.summary(),
+            "roofline": {
+                "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
+                "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot}
+                             for k, v in sorted(prof.items())},
+                "step": {"b_min_bytes_per_cell_update": B_MIN[nd],
+                         "achieved_GBps_over_b_min": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9,
+                         "frac_of_measured_peak": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBps_nominal": B_MIN[nd] * cells * K / (ms * 1e-3) / 8e12},
+            },
+            "e2e": {"value": world * cells * K / (e2e_ms * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": cells * 8 / K, "d2h_bytes_per_step": (cells * 8 + 40) / K,
+                    "call": f"sn_set_state(pinned host) + sn_step({K}) + sn_get_state(pinned host) + sn_diagnostics",
+                    "h2d_bytes_per_call": cells * 8, "d2h_bytes_per_call": cells * 8 + 40, "ms_per_call": e2e_ms},
+            "checks": {"norm_after_timed_steps": norm_after, "norm_after_e2e": d["norm"]},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            out["cpu_baseline"] = oracle_rate(args.workload, args.cpu_budget, inputs)[0]
+        print(json.dumps(out))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
