@@ -18,6 +18,7 @@ LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
          "-Xcompiler", "-fPIC", "-diag-suppress", "128"]
+FLAGS += os.environ.get("SN_NVCC_EXTRA", "").split()  # tuning experiments, e.g. -DSN_CPCAP=4096
 
 
 def _sources():
@@ -51,6 +52,8 @@ def build(force: bool = False) -> str:
         return LIB
     jobs = [(os.path.join(CSRC, "sn_kernels.cu"), os.path.join(OBJ, f"sn_kernels_{n}.o"), [f"-DSN_LEN={n}"])
             for n in LENGTHS]
+    jobs += [(os.path.join(CSRC, "sn_pipe.cu"), os.path.join(OBJ, f"sn_pipe_{n}.o"), [f"-DSN_LEN={n}"])
+             for n in LENGTHS]
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(_compile, jobs))

@@ -7,6 +7,7 @@
 #include "sn_launch.h"
 
 #include <cmath>
+#include <cstdlib>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -104,6 +105,11 @@ struct sn_ctx {
     const float4 *tw[3], *ph_full[3], *ph_half[3];
     const float *ksq[3], *kother;
     double *diag;
+    // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
+    bool use_pipe;
+    int sm_count;
+    CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row;
+    bool m_ok[2];
     // optional per-launch timing (sn_profile): event pairs around every launch, summed per pass kind
     bool profiling;
     std::vector<cudaEvent_t> *ev;       // pool, pairs (start, stop)
@@ -140,6 +146,67 @@ int profile_flush(sn_ctx *c)
     return SN_OK;
 }
 
+// ---- TMA tensor maps (driver entry point fetched through the runtime: no libcuda link) ----
+typedef CUresult (*encode_tiled_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                    const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                    CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+encode_tiled_fn get_encode_fn()
+{
+    static encode_tiled_fn fn = nullptr;
+    if (!fn) {
+        void *ptr = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &ptr, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<encode_tiled_fn>(ptr);
+    }
+    return fn;
+}
+
+// complex64 array [outer][rows][cols] seen as float32 [outer][rows][2*cols]; box = 16 complex x box_rows x 1
+int make_map(CUtensorMap *m, void *ptr, int64_t outer, int64_t rows, int64_t cols, int box_rows)
+{
+    encode_tiled_fn fn = get_encode_fn();
+    if (!fn) {
+        std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled entry point not available");
+        return SN_ERR_CUDA;
+    }
+    const cuuint64_t gdim[3] = {(cuuint64_t)(2 * cols), (cuuint64_t)rows, (cuuint64_t)outer};
+    const cuuint64_t gstr[2] = {(cuuint64_t)(cols * 8), (cuuint64_t)(rows * cols * 8)};
+    const cuuint32_t box[3] = {32u, (cuuint32_t)box_rows, 1u};
+    const cuuint32_t estr[3] = {1u, 1u, 1u};
+    const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+        return SN_ERR_CUDA;
+    }
+    return SN_OK;
+}
+
+int make_tensor_maps(sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    int rc;
+    c->m_ok[0] = c->m_ok[1] = false;
+    if (l.n[0] <= 512 && l.cols0 % 16 == 0) {
+        const int n0 = (int)l.n[0];
+        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, n0 < 256 ? n0 : 256))) return rc;
+        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, n0 / 2))) return rc;
+        if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1))) return rc;
+        c->m_ok[0] = true;
+    }
+    if (l.ndim == 3 && l.n[1] <= 512 && l.n[2] % 16 == 0) {
+        const int n1 = (int)l.n[1];
+        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
+        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
+        c->m_ok[1] = true;
+    }
+    return SN_OK;
+}
+
 int run_pass_raw(sn_ctx *c, int N, PassArgs &a);
 
 int run_pass(sn_ctx *c, int N, PassArgs &a)
@@ -166,6 +233,45 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
 {
     a.stream = c->stream;
     int rc;
+    if (c->use_pipe) {
+        const bool strided = a.kind == snk::P_S_FFT || a.kind == snk::P_S_KIN;
+        const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C;
+        const int axis = strided ? a.axis : 0;
+        const bool maps = (strided || haxis) ? c->m_ok[axis] : true;
+        if (maps && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
+            snk::PipeArgs pa;
+            std::memset(&pa, 0, sizeof(pa));
+            pa.a = a;
+            if (strided) {
+                pa.m_data = axis == 1 ? (a.data == c->hs ? c->m_hs1 : c->m_psi[1]) : c->m_psi[0];
+                pa.tiles_per_outer = a.ncols / (2 * (4096 / N));
+                pa.n_tiles = pa.tiles_per_outer * a.n_outer;
+            } else if (haxis) {
+                pa.m_data = c->m_psi[0];
+                pa.m_hs = c->m_hs0;
+                pa.m_hs_row = c->m_hs0_row;
+                pa.tiles_per_outer = a.ncols / (2 * (4096 / N));
+                pa.n_tiles = pa.tiles_per_outer;
+            } else {
+                const int lines = 2 * (4096 / N);
+                pa.n_tiles = (int)((a.nlines + lines - 1) / lines);
+            }
+            pa.grid = pa.n_tiles < c->sm_count ? pa.n_tiles : c->sm_count;
+            switch (N) {
+            case 64: rc = snk::launch_pipe<64>(pa); break;
+            case 128: rc = snk::launch_pipe<128>(pa); break;
+            case 256: rc = snk::launch_pipe<256>(pa); break;
+            case 512: rc = snk::launch_pipe<512>(pa); break;
+            case 1024: rc = snk::launch_pipe<1024>(pa); break;
+            case 2048: rc = snk::launch_pipe<2048>(pa); break;
+            case 4096: rc = snk::launch_pipe<4096>(pa); break;
+            default: return SN_ERR_DIMS;
+            }
+            if (rc != 0) return cuda_fail((cudaError_t)rc);
+            c->launches++;
+            return SN_OK;
+        }
+    }
     switch (N) {
     case 64: rc = snk::launch_pass<64>(a); break;
     case 128: rc = snk::launch_pass<128>(a); break;
@@ -211,14 +317,14 @@ int upload_static_tables(sn_ctx *c)
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
         const int N = (int)l.n[d];
-        // twiddles: for each stage (NS, R) with NS > 1: entry [kp][r-1] = exp(-2 pi i r kp/(NS R))
+        // twiddles: for each stage (NS, R) with NS > 1: entry [r-1][kp] = exp(-2 pi i r kp/(NS R))
         std::vector<f4> tw;
         tw.reserve(twiddle_entries(N));
         for (int ns = 1; ns < N;) {
             const int rem = N / ns, r = rem >= 8 ? 8 : rem;
             if (ns > 1)
-                for (int kp = 0; kp < ns; kp++)
-                    for (int q = 1; q < r; q++) {
+                for (int q = 1; q < r; q++)
+                    for (int kp = 0; kp < ns; kp++) {
                         const double th = -2.0 * M_PI * (double)((q * kp) % (ns * r)) / (double)(ns * r);
                         tw.push_back(split_hilo(std::cos(th), std::sin(th)));
                     }
@@ -271,6 +377,7 @@ PassArgs base_args(const sn_ctx *c)
 void set_axis_geometry(const sn_ctx *c, PassArgs &a, int axis, int64_t n0)
 {
     const Layout &l = c->lay;
+    a.axis = axis;
     if (axis == 0) {
         a.n_outer = 1; a.outer_stride = 0; a.ncols = (int)l.cols0; a.row_stride = l.cols0;
     } else { // axis 1 of a 3D array
@@ -397,6 +504,16 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
     c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
     int rc = upload_static_tables(c);
     if (rc == SN_OK) rc = upload_phase_tables(c);
+    if (rc == SN_OK) {
+        int dev = 0;
+        const char *np = std::getenv("SN_NO_PIPE"); // SN_NO_PIPE=1: first-path kernels only (A/B runs, tests)
+        c->use_pipe = !(np && np[0] == '1');
+        if (cudaGetDevice(&dev) != cudaSuccess ||
+            cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->sm_count < 1)
+            rc = cuda_fail(cudaGetLastError());
+        else if (c->use_pipe)
+            rc = make_tensor_maps(c);
+    }
     if (rc != SN_OK) {
         delete c;
         return rc;

@@ -135,31 +135,32 @@ constexpr int twiddle_entries(int N)
 
 // One Stockham stage on both lines: twiddle (if NS > 1) then radix-R butterflies.
 // Butterfly q of thread j is butterfly number bq = j + T*q of the stage; its inputs are the
-// thread's own points j + T*(q + r*NB) = bq + r*N/R; twiddle exp(-/+ 2 pi i r (bq % NS)/(NS R)).
-template <int N, int R, int NS, int DIR, bool HILO>
+// thread's own points j + T*(q + r*NB) = bq + r*N/R; twiddle exp(-/+ 2 pi i r (bq % NS)/(NS R)),
+// stored at tw[(r-1)*NS + (bq % NS)] so that lanes with consecutive j read consecutive entries.
+// ONE = true: only line a is transformed (b is never touched).
+template <int N, int R, int NS, int DIR, bool HILO, bool ONE>
 __device__ __forceinline__ void stage_compute(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw)
 {
     constexpr int T = N / 8, NB = 8 / R;
 #pragma unroll
     for (int q = 0; q < NB; q++) {
         if constexpr (NS > 1) {
-            const int kp = (j + T * q) & (NS - 1);
-            const float4 *w = tw + kp * (R - 1);
+            const float4 *w = tw + ((j + T * q) & (NS - 1));
 #pragma unroll
             for (int r = 1; r < R; r++) {
                 float4 ww;
                 if (HILO) {
-                    ww = __ldg(w + (r - 1));
+                    ww = __ldg(w + (r - 1) * NS);
                 } else {
-                    const float2 h = __ldg(reinterpret_cast<const float2 *>(w + (r - 1)));
+                    const float2 h = __ldg(reinterpret_cast<const float2 *>(w + (r - 1) * NS));
                     ww = make_float4(h.x, h.y, 0.f, 0.f);
                 }
                 a[q + r * NB] = twmul<DIR, HILO>(a[q + r * NB], ww);
-                b[q + r * NB] = twmul<DIR, HILO>(b[q + r * NB], ww);
+                if (!ONE) b[q + r * NB] = twmul<DIR, HILO>(b[q + r * NB], ww);
             }
         }
         butterfly<R, NB, DIR, HILO>(a, q);
-        butterfly<R, NB, DIR, HILO>(b, q);
+        if (!ONE) butterfly<R, NB, DIR, HILO>(b, q);
     }
 }
 
@@ -182,16 +183,16 @@ __device__ __forceinline__ void stage_exchange(float2 (&a)[8], float2 (&b)[8], i
     for (int m = 0; m < 8; m++) sm.ld(j + T * m, a[m], b[m]);
 }
 
-template <int N, int NS, int DIR, bool HILO, class SM>
+template <int N, int NS, int DIR, bool HILO, bool ONE, class SM>
 __device__ __forceinline__ void fft_stages(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw,
                                            SM &sm)
 {
     constexpr int REM = N / NS;
     constexpr int R = REM >= 8 ? 8 : REM;
-    stage_compute<N, R, NS, DIR, HILO>(a, b, j, tw);
+    stage_compute<N, R, NS, DIR, HILO, ONE>(a, b, j, tw);
     if constexpr (NS * R < N) {
         stage_exchange<N, R, NS, SM>(a, b, j, sm);
-        fft_stages<N, NS * R, DIR, HILO, SM>(a, b, j, tw + (NS > 1 ? NS * (R - 1) : 0), sm);
+        fft_stages<N, NS * R, DIR, HILO, ONE, SM>(a, b, j, tw + (NS > 1 ? NS * (R - 1) : 0), sm);
     }
 }
 
@@ -200,7 +201,15 @@ __device__ __forceinline__ void fft_stages(float2 (&a)[8], float2 (&b)[8], int j
 template <int N, int DIR, bool HILO, class SM>
 __device__ __forceinline__ void fft_pair(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw, SM &sm)
 {
-    fft_stages<N, 1, DIR, HILO, SM>(a, b, j, tw, sm);
+    fft_stages<N, 1, DIR, HILO, false, SM>(a, b, j, tw, sm);
+}
+
+// Same for ONE line (a); the accessor SM stores/loads only a.
+template <int N, int DIR, bool HILO, class SM>
+__device__ __forceinline__ void fft_single(float2 (&a)[8], int j, const float4 *__restrict__ tw, SM &sm)
+{
+    float2 dummy[8];
+    fft_stages<N, 1, DIR, HILO, true, SM>(a, dummy, j, tw, sm);
 }
 
 // ---- shared-memory accessors -------------------------------------------------------------

@@ -10,33 +10,13 @@
 //   along the contiguous axis of the half spectrum.
 #include "sn_fft_core.cuh"
 #include "sn_launch.h"
+#include "sn_pointwise.cuh"
 
 #ifndef SN_LEN
 #error "compile with -DSN_LEN=<line length>"
 #endif
 
 namespace snk {
-
-// ---------------------------------------------------------------------------- helpers
-
-__device__ __forceinline__ float2 lo2(float4 v) { return make_float2(v.x, v.y); }
-__device__ __forceinline__ float2 hi2(float4 v) { return make_float2(v.z, v.w); }
-__device__ __forceinline__ float4 pack4(float2 a, float2 b) { return make_float4(a.x, a.y, b.x, b.y); }
-__device__ __forceinline__ float abs2(float2 v) { return fmaf(v.x, v.x, v.y * v.y); }
-
-// psi *= exp(i theta), theta/2 = hb*phi + rho*poly(rho).  Written as psi + psi*(e^{i theta}-1)
-// with e^{i theta} - 1 = (-2 sin^2(theta/2), 2 sin(theta/2) cos(theta/2)), so the rounding
-// error of the update scales with |theta| and |e^{i theta}| carries no bias from cos ~ 1.
-__device__ __forceinline__ float2 nl_phase(float2 psi, float phi, const NLParams &nl)
-{
-    const float rho = abs2(psi);
-    const float poly = fmaf(rho, fmaf(rho, fmaf(rho, nl.hg[3], nl.hg[2]), nl.hg[1]), nl.hg[0]);
-    const float th = fmaf(nl.hb, phi, rho * poly);
-    float sh, ch;
-    sincosf(th, &sh, &ch);
-    const float cm1 = -2.f * sh * sh, s = 2.f * sh * ch;
-    return make_float2(psi.x + fmaf(psi.x, cm1, -psi.y * s), psi.y + fmaf(psi.y, cm1, psi.x * s));
-}
 
 // block-wide sum of up to 3 doubles, one atomicAdd per block and value
 template <int NV>
@@ -63,7 +43,10 @@ __device__ __forceinline__ void block_accumulate(double (&v)[NV], double *out)
     }
 }
 
-__host__ __device__ constexpr int cp_for(int N) { return N <= 512 ? 8 : (4096 / N); }
+// column pairs per CTA tile: 512-point lines run as two 256-thread CTAs per SM (measured 15-30 % faster
+// than one 512-thread CTA: the second CTA's loads overlap the first one's butterflies)
+__host__ __device__ constexpr int cp_for(int N) { return N <= 256 ? 8 : (N <= 1024 ? 4 : 4096 / N); }
+__host__ __device__ constexpr int sblocks(int N) { return cp_for(N) * N / 8 <= 256 ? 2 : 1; }
 
 // ---------------------------------------------------------------------------- strided axis
 // Tile: N rows (points of the line, `row_stride` elements apart) x 2*CP adjacent columns.
@@ -71,7 +54,7 @@ __host__ __device__ constexpr int cp_for(int N) { return N <= 512 ? 8 : (4096 / 
 // lanes read/write one 128-byte row segment.
 
 template <int N, int CP, int MODE, int DIR, bool HILO>
-__global__ void __launch_bounds__(CP *N / 8, 1) k_strided(const PassArgs p)
+__global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArgs p)
 {
     extern __shared__ float4 smem[];
     constexpr int T = N / 8;
@@ -154,7 +137,7 @@ __device__ __forceinline__ void c2r_potential(const PassArgs &p, const float4 *h
 }
 
 template <int N, int CP, int MODE>
-__global__ void __launch_bounds__(CP *N / 8, 1) k_haxis(const PassArgs p)
+__global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs p)
 {
     extern __shared__ float4 smem[];
     constexpr int T = N / 8;

@@ -1,6 +1,7 @@
 // sn_launch.h -- internal interface between the scheduler (sn_api.cu) and the per-length kernel
 // translation units (sn_kernels.cu compiled once per line length with -DSN_LEN=N).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 namespace snk {
@@ -37,6 +38,7 @@ struct PassArgs {
     long long outer_stride; // elements between outer blocks
     int ncols;              // contiguous columns per outer block
     int n_outer;
+    int axis;               // strided kinds: 0 or 1 (which view of the array the lines run along)
     int nlines;             // contiguous kinds: number of lines (even)
     const float4 *tw;       // DEVICE: twiddle table for this length
     const float4 *phase;    // DEVICE: kinetic phase table (hi/lo, includes 1/N)
@@ -54,5 +56,41 @@ struct PassArgs {
 // Returns cudaError_t as int.  Explicitly instantiated for N in {64,...,4096}.
 template <int N>
 int launch_pass(const PassArgs &a);
+
+// ---- pipelined (persistent, TMA-fed) variants of the hot passes: sn_pipe.cu ----
+// One 512-thread CTA per SM walks over 64 KB tiles; tiles are moved by the TMA unit between
+// HBM and a ring of shared-memory stages, so loads and stores of neighbouring tiles overlap the
+// butterflies of the current one.  Kinds served: P_S_FFT, P_S_KIN, P_H_NLKIN, P_H_R2C (N <= 512)
+// and P_X_KIN, P_X_POISSON (all N).  Tensor maps view an array as [outer][row][2*cols floats]
+// with 128-byte (16 complex) wide, 128B-swizzled boxes.
+struct PipeArgs {
+    CUtensorMap m_data;   // psi (or the half spectrum for P_S_FFT): box {32 floats, min(N,256) rows, 1}
+    CUtensorMap m_hs;     // P_H_*: half spectrum [N/2+1 rows][2*cols floats]: box {32, N/2 rows, 1}
+    CUtensorMap m_hs_row; // P_H_*: same tensor, box {32, 1, 1} (the row N/2)
+    PassArgs a;
+    int n_tiles;          // tiles of this pass
+    int tiles_per_outer;  // strided kinds: column blocks per outer index
+    int grid;             // CTAs to launch (<= number of SMs)
+};
+
+// true when launch_pipe<N> serves this kind/geometry (otherwise use launch_pass<N>)
+inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
+{
+    switch (kind) {
+    case P_S_FFT:
+    case P_S_KIN:
+    case P_H_NLKIN:
+    case P_H_R2C:
+        return N <= 512 && ncols % (2 * (4096 / N)) == 0; // a tile is 2 * 512/(N/8) columns wide
+    case P_X_KIN:
+    case P_X_POISSON:
+        return nlines % 2 == 0;
+    default:
+        return false;
+    }
+}
+
+template <int N>
+int launch_pipe(const PipeArgs &a);
 
 } // namespace snk

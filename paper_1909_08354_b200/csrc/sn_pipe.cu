@@ -1,0 +1,509 @@
+// sn_pipe.cu -- pipelined, persistent, TMA-fed versions of the hot pass kernels (sm_100a),
+// compiled once per line length (-DSN_LEN=N).
+//
+// Why: the first-path kernels (sn_kernels.cu) are "load tile -> FFT -> store" with the three
+// phases serialised inside a CTA whose 128 registers/thread allow one 512-thread CTA per SM:
+// ncu showed DRAM 20-58 % busy, issue slots 25-57 % busy, the dominant stall the global loads
+// (profiles/r01a_first_path_C5_512.md).  Here one 512-thread CTA per SM loops over tiles; the
+// TMA unit moves 64 KB tiles between HBM and a ring of shared-memory stages
+// (cp.async.bulk.tensor with 128-byte swizzle for strided lines, cp.async.bulk for contiguous
+// lines), completion is tracked with mbarriers, and the butterflies of tile k run while tile
+// k+1/k+2 are landing and tile k-1 is draining.  No register is spent on global addresses.
+//
+// Tile geometry (strided kinds): T = N/8 threads carry one PAIR of adjacent columns (a "line
+// pair", one float4 = 2 complex per row); G = 512/T groups per CTA; a tile is N rows x 2G
+// columns, stored as G/8 sub-tiles of [N rows][128 B].  In a sub-tile the TMA 128B swizzle puts
+// the 16-byte chunk c of row r at chunk c ^ (r & 7): the 8 lanes of a quarter-warp (consecutive
+// rows, same column pair) hit 8 different bank groups, so every 128-bit access is conflict-free.
+// A group only ever touches its own N slots (one per row), so the Stockham exchanges of its FFT
+// run IN PLACE in the tile, position pos living in the slot of row pos ^ ((pos >> 3) & 7).
+#include "sn_fft_core.cuh"
+#include "sn_launch.h"
+#include "sn_pointwise.cuh"
+#include "sn_tma.cuh"
+
+#ifndef SN_LEN
+#error "compile with -DSN_LEN=<line length>"
+#endif
+
+namespace snk {
+
+constexpr int PIPE_THREADS = 512;
+constexpr int PIPE_WARPS = PIPE_THREADS / 32;
+constexpr int TILE_BYTES = 65536; // N rows x 2G columns x 8 B, for every N <= 512
+
+template <int N>
+struct Geo {
+    static constexpr int T = N / 8;                       // threads per line pair
+    static constexpr int G = PIPE_THREADS / T;            // line pairs (groups) per tile
+    static constexpr int SUB = G / 8;                     // 128-byte wide sub-tiles
+    static constexpr int RB = N < 256 ? N : 256;          // rows per TMA box
+    static constexpr int NBOX = N / RB;
+    static constexpr int SUB_F4 = N * 8;                  // float4 slots of a psi sub-tile
+    static constexpr int HROWS = N / 2 + 1;               // rows of the half spectrum
+    static constexpr int HS_SUB_BYTES = (HROWS * 128 + 1023) / 1024 * 1024;
+    static constexpr int HS_SUB_F4 = HS_SUB_BYTES / 16;
+    static constexpr int HS_TX = SUB * HROWS * 128;       // bytes one hs tile load delivers
+};
+
+// slot (float4 index inside a sub-tile) of row r for column pair t: the TMA SWIZZLE_128B layout
+__device__ __forceinline__ int nat_slot(int r, int t) { return r * 8 + (t ^ (r & 7)); }
+
+// Exchange accessor for a line PAIR living in its own slots of a swizzled sub-tile.
+template <int T>
+struct SmemSub {
+    float4 *sub;
+    int t, bar_id;
+    __device__ __forceinline__ int idx(int pos) const { return nat_slot(pos ^ ((pos >> 3) & 7), t); }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const { sub[idx(pos)] = pack4(a, b); }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
+    {
+        const float4 v = sub[idx(pos)];
+        a = lo2(v);
+        b = hi2(v);
+    }
+    __device__ __forceinline__ void sync() const
+    {
+        if (T <= 32) __syncwarp();
+        else named_bar_sync(bar_id, T);
+    }
+};
+
+// Exchange accessor for ONE line (float2 per position) living in the first N/2 slots of a group's
+// column pair: position pos -> row q ^ ((q >> 2) & 7), q = pos >> 1, half (pos ^ (pos >> 6)) & 1.
+template <int T>
+struct SmemSubOne {
+    float2 *sub2; // the sub-tile as float2
+    int t, bar_id;
+    __device__ __forceinline__ int idx(int pos) const
+    {
+        const int q = pos >> 1, r = q ^ ((q >> 2) & 7);
+        return nat_slot(r, t) * 2 + ((pos ^ (pos >> 6)) & 1);
+    }
+    __device__ __forceinline__ void st(int pos, float2 a, float2) const { sub2[idx(pos)] = a; }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &) const { a = sub2[idx(pos)]; }
+    __device__ __forceinline__ void sync() const
+    {
+        if (T <= 32) __syncwarp();
+        else named_bar_sync(bar_id, T);
+    }
+};
+
+__device__ __forceinline__ uint8_t *align_1024(uint8_t *p)
+{
+    return p + ((1024u - (smem_u32(p) & 1023u)) & 1023u);
+}
+
+// all warps: "this warp is done with the stage" (generic writes fenced for the TMA store)
+__device__ __forceinline__ void warp_arrive_done(uint64_t *bar)
+{
+    fence_proxy_async();
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) mbar_arrive(bar);
+}
+
+// kinetic phase on a line pair: a, b *= phase[j + T m]   (S2 of SURVEY.md 8(a), separable per axis)
+template <int T>
+__device__ __forceinline__ void apply_phase(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ phase)
+{
+#pragma unroll
+    for (int m = 0; m < 8; m++) {
+        const float4 ph = __ldg(phase + j + T * m);
+        a[m] = twmul<+1, true>(a[m], ph);
+        b[m] = twmul<+1, true>(b[m], ph);
+    }
+}
+
+// ---------------------------------------------------------------------------- strided axis
+// P_S_KIN: forward -> kinetic phase -> inverse along a strided axis; P_S_FFT: plain transform.
+// 3-stage ring.  Thread 0 is the issuer: at the end of tile k it waits until every warp has
+// released the stage, stores it, and reloads the stage that tile k-1 was stored from with tile k+2.
+
+template <int N, int MODE, int DIR, bool HILO>
+__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_constant__ PipeArgs p)
+{
+    using g_ = Geo<N>;
+    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 3;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = align_1024(smem_raw);
+    uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * TILE_BYTES), *done = full + NST;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+
+    if (tid == 0) {
+        for (int i = 0; i < NST; i++) {
+            mbar_init(full + i, 1);
+            mbar_init(done + i, PIPE_WARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto tile_coords = [&](int k, int &outer, int &col0) {
+        const int tile = blockIdx.x + k * gridDim.x;
+        outer = tile / p.tiles_per_outer;
+        col0 = (tile % p.tiles_per_outer) * 2 * G;
+    };
+    auto issue_load = [&](int k) {
+        int outer, col0;
+        tile_coords(k, outer, col0);
+        const int b = k % NST;
+        mbar_arrive_expect_tx(full + b, TILE_BYTES);
+#pragma unroll
+        for (int ss = 0; ss < SUB; ss++)
+#pragma unroll
+            for (int bx = 0; bx < NBOX; bx++)
+                tma_load_3d(base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, &p.m_data, full + b,
+                            2 * (col0 + 16 * ss), bx * RB, outer);
+    };
+    if (tid == 0) {
+        if (nk > 0) issue_load(0);
+        if (nk > 1) issue_load(1);
+    }
+
+    for (int k = 0; k < nk; k++) {
+        const int b = k % NST;
+        const uint32_t par = (k / NST) & 1;
+        float4 *sub = reinterpret_cast<float4 *>(base + b * TILE_BYTES) + s * g_::SUB_F4;
+        SmemSub<T> sm{sub, t, 1 + g};
+        mbar_wait(full + b, par);
+
+        float2 a[8], c[8];
+#pragma unroll
+        for (int m = 0; m < 8; m++) {
+            const float4 v = sub[nat_slot(j + T * m, t)];
+            a[m] = lo2(v);
+            c[m] = hi2(v);
+        }
+        if (MODE == P_S_FFT) {
+            fft_pair<N, DIR, HILO>(a, c, j, p.a.tw, sm);
+            if (DIR < 0) {
+                const float sc = p.a.scale;
+#pragma unroll
+                for (int m = 0; m < 8; m++) {
+                    a[m].x *= sc; a[m].y *= sc; c[m].x *= sc; c[m].y *= sc;
+                }
+            }
+        } else { // P_S_KIN
+            fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
+            apply_phase<T>(a, c, j, p.a.phase);
+            fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+        }
+        // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
+        __syncwarp();
+#pragma unroll
+        for (int m = 0; m < 8; m++) sub[nat_slot(j + T * m, t)] = pack4(a[m], c[m]);
+        warp_arrive_done(done + b);
+
+        if (tid == 0) {
+            mbar_wait(done + b, par);
+            int outer, col0;
+            tile_coords(k, outer, col0);
+#pragma unroll
+            for (int ss = 0; ss < SUB; ss++)
+#pragma unroll
+                for (int bx = 0; bx < NBOX; bx++)
+                    tma_store_3d(&p.m_data, base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss),
+                                 bx * RB, outer);
+            bulk_commit();
+            if (k + 2 < nk) {
+                bulk_wait_read<1>(); // the store of tile k-1 has left its stage
+                issue_load(k + 2);
+            }
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// ---------------------------------------------------------------------------- axis 0 ("h") kernels
+// P_H_NLKIN (S7, S8, S1-S3 of SURVEY.md 8(a)): c2r of phi^ along axis 0 -> nonlinear phase on psi ->
+// forward -> kinetic phase -> inverse along axis 0.  P_H_R2C (S4, S5): rho = |psi|^2 -> packed r2c.
+// A group's two psi columns 2t, 2t+1 carry two REAL columns of rho / phi as ONE complex line
+// z = x + i y (two-for-one trick):
+//   X[k] = (Z[k] + conj Z[N-k])/2,  Y[k] = (Z[k] - conj Z[N-k])/(2i),  k = 0..N/2;
+//   inverse: Z[k] = X[k] + i Y[k] (k <= N/2), Z[N-k] = conj X[k] + i conj Y[k];
+// the factor 1/2 is folded into the Poisson multiplier (PassArgs::pscale).
+// Stage = psi tile (64 KB) + half-spectrum tile ((N/2+1) rows, <= 33 KB); 2-stage ring.  The stage
+// that tile k was stored from is reloaded with tile k+2 from a point INSIDE tile k+1's compute, so
+// the issuer never waits for its own store to drain.
+
+template <int N, int MODE>
+__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_constant__ PipeArgs p)
+{
+    using g_ = Geo<N>;
+    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int STAGE_BYTES = TILE_BYTES + SUB * g_::HS_SUB_BYTES;
+    constexpr bool LOAD_HS = MODE == P_H_NLKIN;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = align_1024(smem_raw);
+    uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+
+    if (tid == 0) {
+        for (int i = 0; i < NST; i++) {
+            mbar_init(full + i, 1);
+            mbar_init(done + i, PIPE_WARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto issue_load = [&](int k) {
+        const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
+        const int b = k % NST;
+        uint8_t *st = base + b * STAGE_BYTES;
+        mbar_arrive_expect_tx(full + b, TILE_BYTES + (LOAD_HS ? g_::HS_TX : 0));
+#pragma unroll
+        for (int ss = 0; ss < SUB; ss++) {
+#pragma unroll
+            for (int bx = 0; bx < NBOX; bx++)
+                tma_load_3d(st + ss * N * 128 + bx * RB * 128, &p.m_data, full + b, 2 * (col0 + 16 * ss), bx * RB, 0);
+            if (LOAD_HS) {
+                uint8_t *hs = st + TILE_BYTES + ss * g_::HS_SUB_BYTES;
+                tma_load_3d(hs, &p.m_hs, full + b, 2 * (col0 + 16 * ss), 0, 0);
+                tma_load_3d(hs + (N / 2) * 128, &p.m_hs_row, full + b, 2 * (col0 + 16 * ss), N / 2, 0);
+            }
+        }
+    };
+    if (tid == 0) {
+        if (nk > 0) issue_load(0);
+        if (nk > 1) issue_load(1);
+    }
+
+    for (int k = 0; k < nk; k++) {
+        const int b = k % NST;
+        const uint32_t par = (k / NST) & 1;
+        uint8_t *st = base + b * STAGE_BYTES;
+        float4 *sub = reinterpret_cast<float4 *>(st) + s * g_::SUB_F4;
+        float4 *hsub = reinterpret_cast<float4 *>(st + TILE_BYTES) + s * g_::HS_SUB_F4;
+        SmemSub<T> sm{sub, t, 1 + g};
+        mbar_wait(full + b, par);
+
+        if (MODE == P_H_NLKIN) {
+            float2 z[8];
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                const int km = j + T * m;
+                const float4 u = hsub[nat_slot(m < 4 ? km : N - km, t)];
+                z[m] = m < 4 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
+            }
+            SmemSubOne<T> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
+            fft_single<N, -1, false>(z, j, p.a.tw, sm1);
+            // z[m] = (phi[col 2t], phi[col 2t+1]) at row j + T m.  The previous tile's store has had the
+            // whole c2r to leave its stage: reload it now.
+            if (tid == 0 && k >= 1 && k + 1 < nk) {
+                bulk_wait_read<0>();
+                issue_load(k + 1);
+            }
+            float2 a[8], c[8];
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                const float4 v = sub[nat_slot(j + T * m, t)];
+                a[m] = nl_phase(lo2(v), z[m].x, p.a.nl);
+                c[m] = nl_phase(hi2(v), z[m].y, p.a.nl);
+            }
+            fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
+            apply_phase<T>(a, c, j, p.a.phase);
+            fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+            __syncwarp();
+#pragma unroll
+            for (int m = 0; m < 8; m++) sub[nat_slot(j + T * m, t)] = pack4(a[m], c[m]);
+        } else { // P_H_R2C
+            float2 z[8];
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                const float4 v = sub[nat_slot(j + T * m, t)];
+                z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+            }
+            // every psi value of the stage is in registers once all warps pass this point, but only the
+            // hs half of the stage is stored, so the reload still waits for the previous store (below)
+            SmemSubOne<T> sm1{reinterpret_cast<float2 *>(sub), t, 1 + g};
+            fft_single<N, +1, false>(z, j, p.a.tw, sm1);
+            if (tid == 0 && k >= 1 && k + 1 < nk) {
+                bulk_wait_read<0>();
+                issue_load(k + 1);
+            }
+            sm1.sync();
+            float2 dummy = make_float2(0.f, 0.f);
+#pragma unroll
+            for (int m = 0; m < 8; m++) sm1.st(j + T * m, z[m], dummy);
+            sm1.sync();
+#pragma unroll
+            for (int m = 0; m < 5; m++) {
+                if (m < 4 || j == 0) {
+                    const int kk = j + T * m;
+                    float2 y;
+                    sm1.ld((N - kk) & (N - 1), y, dummy);
+                    hsub[nat_slot(kk, t)] = make_float4(z[m].x + y.x, z[m].y - y.y, z[m].y + y.y, y.x - z[m].x);
+                }
+            }
+        }
+        warp_arrive_done(done + b);
+
+        if (tid == 0) {
+            mbar_wait(done + b, par);
+            const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
+#pragma unroll
+            for (int ss = 0; ss < SUB; ss++) {
+                if (MODE == P_H_NLKIN) {
+#pragma unroll
+                    for (int bx = 0; bx < NBOX; bx++)
+                        tma_store_3d(&p.m_data, st + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss), bx * RB, 0);
+                } else {
+                    const uint8_t *hs = st + TILE_BYTES + ss * g_::HS_SUB_BYTES;
+                    tma_store_3d(&p.m_hs, hs, 2 * (col0 + 16 * ss), 0, 0);
+                    tma_store_3d(&p.m_hs_row, hs + (N / 2) * 128, 2 * (col0 + 16 * ss), N / 2, 0);
+                }
+            }
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// ---------------------------------------------------------------------------- contiguous axis
+// P_X_KIN: forward -> kinetic phase -> inverse along the contiguous axis of psi; P_X_POISSON (S5-S7,
+// eq. (2)): forward -> D/(C - k^2) -> inverse along the contiguous axis of the half
+// spectrum.  A tile is 2G consecutive lines = one contiguous 64 KB run, moved with 1D bulk copies;
+// a group owns two adjacent lines and exchanges inside its own 16*N bytes.  3-stage ring as above.
+
+template <int N>
+struct GeoX {
+    static constexpr int T = N / 8;
+    static constexpr int G = PIPE_THREADS / T;
+    static constexpr int LINES = 2 * G;
+    static_assert(LINES * N * 8 == TILE_BYTES, "tile size");
+};
+
+template <int N, int MODE>
+__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_constant__ PipeArgs p)
+{
+    constexpr int T = GeoX<N>::T, LINES = GeoX<N>::LINES, NST = 3;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = align_1024(smem_raw);
+    uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * TILE_BYTES), *done = full + NST;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T;
+
+    if (tid == 0) {
+        for (int i = 0; i < NST; i++) {
+            mbar_init(full + i, 1);
+            mbar_init(done + i, PIPE_WARPS);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto tile_lines = [&](int k, long long &line0) {
+        line0 = (long long)(blockIdx.x + k * gridDim.x) * LINES;
+        const long long left = p.a.nlines - line0;
+        return (int)(left < LINES ? left : LINES);
+    };
+    auto issue_load = [&](int k) {
+        long long line0;
+        const uint32_t bytes = (uint32_t)tile_lines(k, line0) * N * 8;
+        const int b = k % NST;
+        mbar_arrive_expect_tx(full + b, bytes);
+        bulk_load_1d(base + b * TILE_BYTES, p.a.data + line0 * N, bytes, full + b);
+    };
+    if (tid == 0) {
+        if (nk > 0) issue_load(0);
+        if (nk > 1) issue_load(1);
+    }
+
+    for (int k = 0; k < nk; k++) {
+        const int b = k % NST;
+        const uint32_t par = (k / NST) & 1;
+        long long line0;
+        const int nl = tile_lines(k, line0);
+        float4 *grp = reinterpret_cast<float4 *>(base + b * TILE_BYTES) + g * N; // two lines = N float4
+        float2 *la = reinterpret_cast<float2 *>(grp), *lb = la + N;
+        SmemLine<T> sm{grp, 1 + g, T == PIPE_THREADS};
+        mbar_wait(full + b, par);
+
+        if (2 * g < nl) {
+            float2 a[8], c[8];
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                a[m] = la[j + T * m];
+                c[m] = lb[j + T * m];
+            }
+            if (MODE == P_X_KIN) {
+                fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
+                apply_phase<T>(a, c, j, p.a.phase);
+                fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+            } else { // P_X_POISSON
+                fft_pair<N, +1, false>(a, c, j, p.a.tw, sm);
+                const float ka = __ldg(p.a.kother2 + line0 + 2 * g), kb = __ldg(p.a.kother2 + line0 + 2 * g + 1);
+#pragma unroll
+                for (int m = 0; m < 8; m++) {
+                    const float kx2 = __ldg(p.a.ksq + j + T * m);
+                    const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
+                    const float ga = da == 0.f ? 0.f : p.a.pscale / da;
+                    const float gb = db == 0.f ? 0.f : p.a.pscale / db;
+                    a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
+                }
+                fft_pair<N, -1, false>(a, c, j, p.a.tw, sm);
+            }
+            sm.sync(); // exchange layout (float4 per position) != line layout: whole group must be done reading
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                la[j + T * m] = a[m];
+                lb[j + T * m] = c[m];
+            }
+        }
+        warp_arrive_done(done + b);
+
+        if (tid == 0) {
+            mbar_wait(done + b, par);
+            bulk_store_1d(p.a.data + line0 * N, base + b * TILE_BYTES, (uint32_t)nl * N * 8);
+            bulk_commit();
+            if (k + 2 < nk) {
+                bulk_wait_read<1>();
+                issue_load(k + 2);
+            }
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// ---------------------------------------------------------------------------- launchers
+
+template <class K>
+static int launch_pipe_kernel(K kern, size_t smem_bytes, const PipeArgs &a)
+{
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+    if (e != cudaSuccess) return (int)e;
+    kern<<<a.grid, PIPE_THREADS, smem_bytes, a.a.stream>>>(a);
+    return (int)cudaGetLastError();
+}
+
+template <int N>
+int launch_pipe(const PipeArgs &a)
+{
+    constexpr size_t SLACK = 1024 + 64; // alignment of the ring + the mbarriers
+    constexpr size_t S3 = 3 * (size_t)TILE_BYTES + SLACK;
+    if (a.a.kind == P_X_KIN) return launch_pipe_kernel(k_pipe_contig<N, P_X_KIN>, S3, a);
+    if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON>, S3, a);
+    if constexpr (N <= 512) {
+        constexpr size_t S2H = 2 * ((size_t)TILE_BYTES + Geo<N>::SUB * Geo<N>::HS_SUB_BYTES) + SLACK;
+        switch (a.a.kind) {
+        case P_S_KIN: return launch_pipe_kernel(k_pipe_strided<N, P_S_KIN, +1, true>, S3, a);
+        case P_S_FFT:
+            if (a.a.dir > 0)
+                return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, true>, S3, a)
+                                : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, false>, S3, a);
+            return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, true>, S3, a)
+                            : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, false>, S3, a);
+        case P_H_NLKIN: return launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN>, S2H, a);
+        case P_H_R2C: return launch_pipe_kernel(k_pipe_haxis<N, P_H_R2C>, S2H, a);
+        default: break;
+        }
+    }
+    return (int)cudaErrorInvalidValue;
+}
+
+template int launch_pipe<SN_LEN>(const PipeArgs &a);
+
+} // namespace snk
