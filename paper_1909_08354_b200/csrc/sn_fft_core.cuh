@@ -164,23 +164,50 @@ __device__ __forceinline__ void stage_compute(float2 (&a)[8], float2 (&b)[8], in
     }
 }
 
+// ---- XOR-linear shared-memory addressing --------------------------------------------------
+// Every exchange layout below is a GF(2)-linear map of the position bits (shifts, masks, XOR
+// swizzles) XORed with a per-group constant.  An exchange position is (thread part) ^ (compile-
+// time part) with disjoint bits, so   idx(pos) = idx(thread part) ^ lin(compile-time part):
+// ONE runtime index per stage and thread, and per access an XOR with an immediate (bits that the
+// thread part can also set) plus an immediate offset (bits it cannot).  Without this the compiler
+// precomputes ~20 addresses per thread, keeps them across tiles and spills them.
+template <class SM>
+__host__ __device__ constexpr int lin_mask(int posmask)
+{
+    int m = 0;
+    for (int bit = 0; bit < 16; bit++)
+        if (posmask >> bit & 1) m |= SM::lin(1 << bit);
+    return m;
+}
+// index of position (thread part ^ K) given tb = idx(thread part); PM = bits the thread part may set
+template <class SM>
+__device__ __forceinline__ int comb(int tb, int K, int PM)
+{
+    const int TM = lin_mask<SM>(PM) | SM::TMASK;
+    const int L = SM::lin(K);
+    const int X = L & TM, A = L & ~TM;
+    return (tb ^ X) + A;
+}
+
 // Stockham exchange after a stage (NS, R): output r of butterfly bq goes to position
 // (bq / NS) * NS * R + (bq % NS) + r * NS; afterwards thread j re-reads points j + T*m.
 template <int N, int R, int NS, class SM>
 __device__ __forceinline__ void stage_exchange(float2 (&a)[8], float2 (&b)[8], int j, SM &sm)
 {
     constexpr int T = N / 8, NB = 8 / R;
+    constexpr int WPM = ((T - 1) & ~(NS - 1)) * R | ((T - 1) & (NS - 1)); // position bits of butterfly j's base
     sm.sync(); // previous readers of the buffer are done
+    const int tbw = sm.idx((j & ~(NS - 1)) * R + (j & (NS - 1)));
 #pragma unroll
     for (int q = 0; q < NB; q++) {
-        const int bq = j + T * q;
-        const int base = (bq & ~(NS - 1)) * R + (bq & (NS - 1));
+        const int kq = ((T * q) & ~(NS - 1)) * R + ((T * q) & (NS - 1)); // base of butterfly T*q (compile time)
 #pragma unroll
-        for (int r = 0; r < R; r++) sm.st(base + r * NS, a[q + r * NB], b[q + r * NB]);
+        for (int r = 0; r < R; r++) sm.st_i(comb<SM>(tbw, kq + r * NS, WPM), a[q + r * NB], b[q + r * NB]);
     }
     sm.sync();
+    const int tbr = sm.idx(j);
 #pragma unroll
-    for (int m = 0; m < 8; m++) sm.ld(j + T * m, a[m], b[m]);
+    for (int m = 0; m < 8; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), a[m], b[m]);
 }
 
 template <int N, int NS, int DIR, bool HILO, bool ONE, class SM>
@@ -213,7 +240,9 @@ __device__ __forceinline__ void fft_single(float2 (&a)[8], int j, const float4 *
 }
 
 // ---- shared-memory accessors -------------------------------------------------------------
-// One float4 per point position: (a.re, a.im, b.re, b.im).
+// One float4 per point position: (a.re, a.im, b.re, b.im).  Interface: lin(pos) = linear index of a
+// position (group constant excluded), TMASK = index bits the group constant occupies,
+// idx(pos) = lin(pos) ^ group constant, st_i / ld_i = access by index.
 
 // Tile of CP column pairs per row (strided-axis kernels); thread t owns column pair t.  With
 // CP = 8 a row is 128 B = all 32 banks and 8 adjacent lanes cover it, so every 128-bit access
@@ -223,23 +252,24 @@ template <int CP>
 struct SmemTile {
     float4 *base;
     int t;
-    __device__ __forceinline__ int idx(int pos) const
+    static constexpr int TMASK = CP - 1;
+    __host__ __device__ static constexpr int lin(int pos)
     {
-        if (CP == 8) return pos * 8 + t;
-        if (CP == 4) return (pos * 4 + t) ^ (((pos >> 3) & 1) << 2);
-        if (CP == 2) return (pos * 2 + t) ^ (((pos >> 3) & 3) << 1);
+        if (CP == 8) return pos * 8;
+        if (CP == 4) return (pos * 4) ^ (((pos >> 3) & 1) << 2);
+        if (CP == 2) return (pos * 2) ^ (((pos >> 3) & 3) << 1);
         return pos ^ ((pos >> 3) & 7);
     }
-    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const
+    __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ t; }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { base[i] = make_float4(a.x, a.y, b.x, b.y); }
+    __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
-        base[idx(pos)] = make_float4(a.x, a.y, b.x, b.y);
-    }
-    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
-    {
-        const float4 v = base[idx(pos)];
+        const float4 v = base[i];
         a = make_float2(v.x, v.y);
         b = make_float2(v.z, v.w);
     }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const { st_i(idx(pos), a, b); }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const { ld_i(idx(pos), a, b); }
     __device__ __forceinline__ void sync() const { __syncthreads(); }
 };
 
@@ -251,17 +281,18 @@ struct SmemLine {
     float4 *base;
     int bar_id; // named barrier for this group when T > 32 and the CTA holds several groups
     bool whole_cta;
-    __device__ __forceinline__ static int sw(int pos) { return pos ^ ((pos >> 3) & 7); }
-    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const
+    static constexpr int TMASK = 0;
+    __host__ __device__ static constexpr int lin(int pos) { return pos ^ ((pos >> 3) & 7); }
+    __device__ __forceinline__ int idx(int pos) const { return lin(pos); }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { base[i] = make_float4(a.x, a.y, b.x, b.y); }
+    __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
-        base[sw(pos)] = make_float4(a.x, a.y, b.x, b.y);
-    }
-    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
-    {
-        const float4 v = base[sw(pos)];
+        const float4 v = base[i];
         a = make_float2(v.x, v.y);
         b = make_float2(v.z, v.w);
     }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const { st_i(idx(pos), a, b); }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const { ld_i(idx(pos), a, b); }
     __device__ __forceinline__ void sync() const
     {
         if (T <= 32) {

@@ -49,16 +49,23 @@ struct Geo {
 // slot (float4 index inside a sub-tile) of row r for column pair t: the TMA SWIZZLE_128B layout
 __device__ __forceinline__ int nat_slot(int r, int t) { return r * 8 + (t ^ (r & 7)); }
 
-// Exchange accessor for a line PAIR living in its own slots of a swizzled sub-tile.
+// Exchange accessor for a line PAIR living in its own slots of a swizzled sub-tile: position pos
+// lives in the slot of row pos ^ ((pos >> 3) & 7).
 template <int T>
 struct SmemSub {
     float4 *sub;
     int t, bar_id;
-    __device__ __forceinline__ int idx(int pos) const { return nat_slot(pos ^ ((pos >> 3) & 7), t); }
-    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const { sub[idx(pos)] = pack4(a, b); }
-    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const
+    static constexpr int TMASK = 7;
+    __host__ __device__ static constexpr int lin(int pos)
     {
-        const float4 v = sub[idx(pos)];
+        const int r = pos ^ ((pos >> 3) & 7);
+        return (r << 3) | (r & 7);
+    }
+    __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ t; }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { sub[i] = pack4(a, b); }
+    __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
+    {
+        const float4 v = sub[i];
         a = lo2(v);
         b = hi2(v);
     }
@@ -75,19 +82,31 @@ template <int T>
 struct SmemSubOne {
     float2 *sub2; // the sub-tile as float2
     int t, bar_id;
-    __device__ __forceinline__ int idx(int pos) const
+    static constexpr int TMASK = 7 << 1;
+    __host__ __device__ static constexpr int lin(int pos)
     {
         const int q = pos >> 1, r = q ^ ((q >> 2) & 7);
-        return nat_slot(r, t) * 2 + ((pos ^ (pos >> 6)) & 1);
+        return (((r << 3) | (r & 7)) << 1) | ((pos ^ (pos >> 6)) & 1);
     }
-    __device__ __forceinline__ void st(int pos, float2 a, float2) const { sub2[idx(pos)] = a; }
-    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &) const { a = sub2[idx(pos)]; }
+    __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ (t << 1); }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2) const { sub2[i] = a; }
+    __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &) const { a = sub2[i]; }
+    __device__ __forceinline__ void st(int pos, float2 a, float2 b) const { st_i(idx(pos), a, b); }
+    __device__ __forceinline__ void ld(int pos, float2 &a, float2 &b) const { ld_i(idx(pos), a, b); }
     __device__ __forceinline__ void sync() const
     {
         if (T <= 32) __syncwarp();
         else named_bar_sync(bar_id, T);
     }
 };
+
+// a value the compiler cannot hoist out of the tile loop or merge with another copy (keeps it from
+// precomputing per-thread address tables / re-using twiddles across transforms through local memory)
+__device__ __forceinline__ int opaque(int v)
+{
+    asm volatile("" : "+r"(v));
+    return v;
+}
 
 __device__ __forceinline__ uint8_t *align_1024(uint8_t *p)
 {
@@ -168,15 +187,17 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
         SmemSub<T> sm{sub, t, 1 + g};
         mbar_wait(full + b, par);
 
+        const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
+        float4 *mine = sub + nat_slot(jf, t);     // row jf; rows jf + T m are 8 T m slots further (T % 8 == 0)
         float2 a[8], c[8];
 #pragma unroll
         for (int m = 0; m < 8; m++) {
-            const float4 v = sub[nat_slot(j + T * m, t)];
+            const float4 v = mine[8 * T * m];
             a[m] = lo2(v);
             c[m] = hi2(v);
         }
         if (MODE == P_S_FFT) {
-            fft_pair<N, DIR, HILO>(a, c, j, p.a.tw, sm);
+            fft_pair<N, DIR, HILO>(a, c, jf, p.a.tw, sm);
             if (DIR < 0) {
                 const float sc = p.a.scale;
 #pragma unroll
@@ -185,14 +206,14 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
                 }
             }
         } else { // P_S_KIN
-            fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
-            apply_phase<T>(a, c, j, p.a.phase);
-            fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+            fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+            apply_phase<T>(a, c, jf, p.a.phase);
+            fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
         }
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
         __syncwarp();
 #pragma unroll
-        for (int m = 0; m < 8; m++) sub[nat_slot(j + T * m, t)] = pack4(a[m], c[m]);
+        for (int m = 0; m < 8; m++) mine[8 * T * m] = pack4(a[m], c[m]);
         warp_arrive_done(done + b);
 
         if (tid == 0) {
@@ -280,16 +301,19 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
         SmemSub<T> sm{sub, t, 1 + g};
         mbar_wait(full + b, par);
 
+        const int jf = opaque(j), ji = opaque(j), jz = opaque(j); // per-tile copies: see opaque()
+        float4 *mine = sub + nat_slot(jf, t);
         if (MODE == P_H_NLKIN) {
             float2 z[8];
+            // rows jz + T m (m < 4) and N - jz - T m (m >= 4): the mirrored rows step DOWN by 8 T slots
+            const float4 *hup = hsub + nat_slot(jz, t), *hdn = hsub + nat_slot(N / 2 - jz, t);
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const int km = j + T * m;
-                const float4 u = hsub[nat_slot(m < 4 ? km : N - km, t)];
+                const float4 u = m < 4 ? hup[8 * T * m] : hdn[-8 * T * (m - 4)];
                 z[m] = m < 4 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
             }
             SmemSubOne<T> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
-            fft_single<N, -1, false>(z, j, p.a.tw, sm1);
+            fft_single<N, -1, false>(z, jz, p.a.tw, sm1);
             // z[m] = (phi[col 2t], phi[col 2t+1]) at row j + T m.  The previous tile's store has had the
             // whole c2r to leave its stage: reload it now.
             if (tid == 0 && k >= 1 && k + 1 < nk) {
@@ -299,27 +323,27 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             float2 a[8], c[8];
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const float4 v = sub[nat_slot(j + T * m, t)];
+                const float4 v = mine[8 * T * m];
                 a[m] = nl_phase(lo2(v), z[m].x, p.a.nl);
                 c[m] = nl_phase(hi2(v), z[m].y, p.a.nl);
             }
-            fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
-            apply_phase<T>(a, c, j, p.a.phase);
-            fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+            fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+            apply_phase<T>(a, c, jf, p.a.phase);
+            fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
             __syncwarp();
 #pragma unroll
-            for (int m = 0; m < 8; m++) sub[nat_slot(j + T * m, t)] = pack4(a[m], c[m]);
+            for (int m = 0; m < 8; m++) mine[8 * T * m] = pack4(a[m], c[m]);
         } else { // P_H_R2C
             float2 z[8];
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const float4 v = sub[nat_slot(j + T * m, t)];
+                const float4 v = mine[8 * T * m];
                 z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
             }
             // every psi value of the stage is in registers once all warps pass this point, but only the
             // hs half of the stage is stored, so the reload still waits for the previous store (below)
             SmemSubOne<T> sm1{reinterpret_cast<float2 *>(sub), t, 1 + g};
-            fft_single<N, +1, false>(z, j, p.a.tw, sm1);
+            fft_single<N, +1, false>(z, jf, p.a.tw, sm1);
             if (tid == 0 && k >= 1 && k + 1 < nk) {
                 bulk_wait_read<0>();
                 issue_load(k + 1);
@@ -423,34 +447,35 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
         mbar_wait(full + b, par);
 
         if (2 * g < nl) {
+            const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
             float2 a[8], c[8];
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                a[m] = la[j + T * m];
-                c[m] = lb[j + T * m];
+                a[m] = la[jf + T * m];
+                c[m] = lb[jf + T * m];
             }
             if (MODE == P_X_KIN) {
-                fft_pair<N, +1, true>(a, c, j, p.a.tw, sm);
-                apply_phase<T>(a, c, j, p.a.phase);
-                fft_pair<N, -1, true>(a, c, j, p.a.tw, sm);
+                fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+                apply_phase<T>(a, c, jf, p.a.phase);
+                fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
             } else { // P_X_POISSON
-                fft_pair<N, +1, false>(a, c, j, p.a.tw, sm);
+                fft_pair<N, +1, false>(a, c, jf, p.a.tw, sm);
                 const float ka = __ldg(p.a.kother2 + line0 + 2 * g), kb = __ldg(p.a.kother2 + line0 + 2 * g + 1);
 #pragma unroll
                 for (int m = 0; m < 8; m++) {
-                    const float kx2 = __ldg(p.a.ksq + j + T * m);
+                    const float kx2 = __ldg(p.a.ksq + jf + T * m);
                     const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
                     const float ga = da == 0.f ? 0.f : p.a.pscale / da;
                     const float gb = db == 0.f ? 0.f : p.a.pscale / db;
                     a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
                 }
-                fft_pair<N, -1, false>(a, c, j, p.a.tw, sm);
+                fft_pair<N, -1, false>(a, c, ji, p.a.tw, sm);
             }
             sm.sync(); // exchange layout (float4 per position) != line layout: whole group must be done reading
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                la[j + T * m] = a[m];
-                lb[j + T * m] = c[m];
+                la[ji + T * m] = a[m];
+                lb[ji + T * m] = c[m];
             }
         }
         warp_arrive_done(done + b);
