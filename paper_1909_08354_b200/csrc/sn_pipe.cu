@@ -254,7 +254,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
     using g_ = Geo<N>;
     constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int STAGE_BYTES = TILE_BYTES + SUB * g_::HS_SUB_BYTES;
-    constexpr bool LOAD_HS = MODE == P_H_NLKIN;
+    constexpr bool LOAD_HS = true;
+    static_assert(MODE == P_H_NLKIN, "k_pipe_haxis serves P_H_NLKIN");
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
 
         const int jf = opaque(j), ji = opaque(j), jz = opaque(j); // per-tile copies: see opaque()
         float4 *mine = sub + nat_slot(jf, t);
-        if (MODE == P_H_NLKIN) {
+        {
             float2 z[8];
             // rows jz + T m (m < 4) and N - jz - T m (m >= 4): the mirrored rows step DOWN by 8 T slots
             const float4 *hup = hsub + nat_slot(jz, t), *hdn = hsub + nat_slot(N / 2 - jz, t);
@@ -333,35 +334,6 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             __syncwarp();
 #pragma unroll
             for (int m = 0; m < 8; m++) mine[8 * T * m] = pack4(a[m], c[m]);
-        } else { // P_H_R2C
-            float2 z[8];
-#pragma unroll
-            for (int m = 0; m < 8; m++) {
-                const float4 v = mine[8 * T * m];
-                z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
-            }
-            // every psi value of the stage is in registers once all warps pass this point, but only the
-            // hs half of the stage is stored, so the reload still waits for the previous store (below)
-            SmemSubOne<T> sm1{reinterpret_cast<float2 *>(sub), t, 1 + g};
-            fft_single<N, +1, false>(z, jf, p.a.tw, sm1);
-            if (tid == 0 && k >= 1 && k + 1 < nk) {
-                bulk_wait_read<0>();
-                issue_load(k + 1);
-            }
-            sm1.sync();
-            float2 dummy = make_float2(0.f, 0.f);
-#pragma unroll
-            for (int m = 0; m < 8; m++) sm1.st(j + T * m, z[m], dummy);
-            sm1.sync();
-#pragma unroll
-            for (int m = 0; m < 5; m++) {
-                if (m < 4 || j == 0) {
-                    const int kk = j + T * m;
-                    float2 y;
-                    sm1.ld((N - kk) & (N - 1), y, dummy);
-                    hsub[nat_slot(kk, t)] = make_float4(z[m].x + y.x, z[m].y - y.y, z[m].y + y.y, y.x - z[m].x);
-                }
-            }
         }
         warp_arrive_done(done + b);
 
@@ -369,18 +341,118 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             mbar_wait(done + b, par);
             const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
 #pragma unroll
-            for (int ss = 0; ss < SUB; ss++) {
-                if (MODE == P_H_NLKIN) {
+            for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
-                    for (int bx = 0; bx < NBOX; bx++)
-                        tma_store_3d(&p.m_data, st + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss), bx * RB, 0);
-                } else {
-                    const uint8_t *hs = st + TILE_BYTES + ss * g_::HS_SUB_BYTES;
-                    tma_store_3d(&p.m_hs, hs, 2 * (col0 + 16 * ss), 0, 0);
-                    tma_store_3d(&p.m_hs_row, hs + (N / 2) * 128, 2 * (col0 + 16 * ss), N / 2, 0);
-                }
+                for (int bx = 0; bx < NBOX; bx++)
+                    tma_store_3d(&p.m_data, st + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss), bx * RB, 0);
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
+// P_H_R2C (S4, S5): rho = |psi|^2 -> packed real-to-complex transform along axis 0 -> half spectrum.
+// Memory-bound (12 B/cell, one single-line FFT per column pair), so the two rings are decoupled:
+// a psi stage is reloaded as soon as every warp has pulled its values into registers, and the
+// transform runs in the OUTPUT buffer (a group's N/2+1 output slots hold its N float2 positions).
+template <int N>
+__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_constant__ PipeArgs p)
+{
+    using g_ = Geo<N>;
+    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int OUT_BYTES = SUB * g_::HS_SUB_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = align_1024(smem_raw);
+    uint8_t *outb = base + NST * TILE_BYTES;
+    uint64_t *full = reinterpret_cast<uint64_t *>(outb + NST * OUT_BYTES), *consumed = full + NST, *done = full + 2 * NST,
+             *freeb = full + 3 * NST;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+
+    if (tid == 0) {
+        for (int i = 0; i < NST; i++) {
+            mbar_init(full + i, 1);
+            mbar_init(consumed + i, PIPE_WARPS);
+            mbar_init(done + i, PIPE_WARPS);
+            mbar_init(freeb + i, 1);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto issue_load = [&](int k) {
+        const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
+        const int b = k % NST;
+        mbar_arrive_expect_tx(full + b, TILE_BYTES);
+#pragma unroll
+        for (int ss = 0; ss < SUB; ss++)
+#pragma unroll
+            for (int bx = 0; bx < NBOX; bx++)
+                tma_load_3d(base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, &p.m_data, full + b,
+                            2 * (col0 + 16 * ss), bx * RB, 0);
+    };
+    if (tid == 0) {
+        if (nk > 0) issue_load(0);
+        if (nk > 1) issue_load(1);
+    }
+
+    for (int k = 0; k < nk; k++) {
+        const int b = k % NST;
+        const uint32_t par = (k / NST) & 1;
+        const float4 *sub = reinterpret_cast<const float4 *>(base + b * TILE_BYTES) + s * g_::SUB_F4;
+        float4 *hsub = reinterpret_cast<float4 *>(outb + b * OUT_BYTES) + s * g_::HS_SUB_F4;
+        const int jf = opaque(j);
+        mbar_wait(full + b, par);
+        float2 z[8];
+        {
+            const float4 *mine = sub + nat_slot(jf, t);
+#pragma unroll
+            for (int m = 0; m < 8; m++) {
+                const float4 v = mine[8 * T * m];
+                z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+            }
+        }
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(consumed + b);
+        if (k >= NST) mbar_wait(freeb + b, ((k / NST) - 1) & 1); // the store of tile k-2 has left this output buffer
+
+        SmemSubOne<T> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
+        fft_single<N, +1, false>(z, jf, p.a.tw, sm1);
+        if (tid == 0 && k + NST < nk) {
+            mbar_wait(consumed + b, par);
+            issue_load(k + NST);
+        }
+        // X[k] and Y[k] from Z[k] and Z[N-k]: pass Z through the buffer once more
+        float2 dummy = make_float2(0.f, 0.f), y[5];
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m < 8; m++) sm1.st(jf + T * m, z[m], dummy);
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m < 5; m++)
+            if (m < 4 || j == 0) sm1.ld((N - (jf + T * m)) & (N - 1), y[m], dummy);
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m < 5; m++)
+            if (m < 4 || j == 0)
+                hsub[nat_slot(jf + T * m, t)] =
+                    make_float4(z[m].x + y[m].x, z[m].y - y[m].y, z[m].y + y[m].y, y[m].x - z[m].x);
+        warp_arrive_done(done + b);
+
+        if (tid == 0) {
+            mbar_wait(done + b, par);
+            const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
+#pragma unroll
+            for (int ss = 0; ss < SUB; ss++) {
+                const uint8_t *hs = outb + b * OUT_BYTES + ss * g_::HS_SUB_BYTES;
+                tma_store_3d(&p.m_hs, hs, 2 * (col0 + 16 * ss), 0, 0);
+                tma_store_3d(&p.m_hs_row, hs + (N / 2) * 128, 2 * (col0 + 16 * ss), N / 2, 0);
             }
             bulk_commit();
+            if (k >= 1) {
+                bulk_wait_read<1>(); // the store of tile k-1 has drained: its buffer is free for tile k+1
+                mbar_arrive(freeb + ((k + 1) % NST));
+            }
         }
     }
     if (tid == 0) bulk_wait<0>();
@@ -522,7 +594,7 @@ int launch_pipe(const PipeArgs &a)
             return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, true>, S3, a)
                             : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, false>, S3, a);
         case P_H_NLKIN: return launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN>, S2H, a);
-        case P_H_R2C: return launch_pipe_kernel(k_pipe_haxis<N, P_H_R2C>, S2H, a);
+        case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, S2H, a);
         default: break;
         }
     }
