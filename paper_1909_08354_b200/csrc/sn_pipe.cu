@@ -537,8 +537,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
                 for (int m = 0; m < 8; m++) {
                     const float kx2 = __ldg(p.a.ksq + jf + T * m);
                     const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
-                    const float ga = da == 0.f ? 0.f : p.a.pscale / da;
-                    const float gb = db == 0.f ? 0.f : p.a.pscale / db;
+                    const float ga = da == 0.f ? 0.f : __fdividef(p.a.pscale, da);
+                    const float gb = db == 0.f ? 0.f : __fdividef(p.a.pscale, db);
                     a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
                 }
                 fft_pair<N, -1, false>(a, c, ji, p.a.tw, sm);
