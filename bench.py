@@ -48,6 +48,10 @@ PASS_BYTES_PER_CELL = {
     "X_POISSON": 8.0,
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
+B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update
+# ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, C5_512, from profiles/r01b_ncu_full_C5_512.md
+NCU_TRAFFIC_C5_512 = {"H_NLKIN": 2.633e9, "S_KIN": 2.089e9, "X_KIN": 2.088e9, "H_R2C": 1.577e9, "S_FFT": 1.019e9,
+                      "X_POISSON": 1.019e9}
 
 
 def load_peaks():
@@ -280,14 +284,20 @@ def main():
             "clocks": clk.summary(),
             "roofline": {
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak,
+                "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" else None,
+                "traffic_source": "ncu --set full dram bytes per launch, profiles/r01b_ncu_full_C5_512.md",
+                "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
                 "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot}
                              for k, v in sorted(prof.items())},
                 "step": {"b_min_bytes_per_cell_update": B_MIN[nd],
                          "achieved_GBps_over_b_min": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9,
                          "frac_of_measured_peak": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak,
-                         "frac_of_8TBps_nominal": B_MIN[nd] * cells * K / (ms * 1e-3) / 8e12},
+                         "frac_of_8TBps_nominal": B_MIN[nd] * cells * K / (ms * 1e-3) / 8e12,
+                         "own_bytes_per_cell_update": B_OWN[nd],
+                         "achieved_GBps_over_own_bytes": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9,
+                         "own_frac_of_measured_peak": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak},
             },
             "e2e": {"value": world * cells * K / (e2e_ms * 1e-3), "unit": UNIT,
                     "h2d_bytes_per_step": cells * 8 / K, "d2h_bytes_per_step": (cells * 8 + 40) / K,
