@@ -186,7 +186,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1909_08354_b200 import sn
+    from paper_1909_08354_b200 import replicas, sn
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -248,14 +248,11 @@ def main():
     sim.close()
 
     # max over ranks
-    t = torch.tensor([ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms, e2e_ms = float(t[0]), float(t[1])
+    ms, e2e_ms = replicas.max_over_ranks([ms, e2e_s * 1e3], device=dev)
 
     if rank == 0:
         cells = cfg.cells
-        value = world * cells * K / (ms * 1e-3)
+        value = replicas.whole_job_rate(cells, K, world, ms)
         peak, peak_src = load_peaks()
         tot = sum(v[0] for v in prof.values()) or 1.0
         dom = max(prof, key=lambda k: prof[k][0])
@@ -299,7 +296,7 @@ def main():
                          "achieved_GBps_over_own_bytes": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9,
                          "own_frac_of_measured_peak": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak},
             },
-            "e2e": {"value": world * cells * K / (e2e_ms * 1e-3), "unit": UNIT,
+            "e2e": {"value": replicas.whole_job_rate(cells, K, world, e2e_ms), "unit": UNIT,
                     "h2d_bytes_per_step": cells * 8 / K, "d2h_bytes_per_step": (cells * 8 + 40) / K,
                     "call": f"sn_set_state(pinned host) + sn_step({K}) + sn_get_state(pinned host) + sn_diagnostics",
                     "h2d_bytes_per_call": cells * 8, "d2h_bytes_per_call": cells * 8 + 40, "ms_per_call": e2e_ms},
