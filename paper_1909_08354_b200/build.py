@@ -14,7 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsn.so")
-LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)
+LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)   # pipelined + first-path kernels
+LENGTHS3 = (96, 384, 1536)                         # 6*4^a: first-path kernels only
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
          "-Xcompiler", "-fPIC", "-diag-suppress", "128"]
@@ -51,7 +52,7 @@ def build(force: bool = False) -> str:
     if not _stale(LIB):
         return LIB
     jobs = [(os.path.join(CSRC, "sn_kernels.cu"), os.path.join(OBJ, f"sn_kernels_{n}.o"), [f"-DSN_LEN={n}"])
-            for n in LENGTHS]
+            for n in LENGTHS + LENGTHS3]
     jobs += [(os.path.join(CSRC, "sn_pipe.cu"), os.path.join(OBJ, f"sn_pipe_{n}.o"), [f"-DSN_LEN={n}"])
              for n in LENGTHS]
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))

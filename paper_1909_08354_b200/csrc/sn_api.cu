@@ -19,14 +19,27 @@ using snk::PassArgs;
 
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
-inline bool len_ok(int64_t n) { return n >= 64 && n <= 4096 && (n & (n - 1)) == 0; }
+// supported line lengths: 2^n in [64, 4096] and 6*4^a (96, 384, 1536); keep in step with build.py LENGTHS
+inline bool len_ok(int64_t n)
+{
+    if (n >= 64 && n <= 4096 && (n & (n - 1)) == 0) return true;
+    return n == 96 || n == 384 || n == 1536;
+}
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// stage radices of the line-FFT engine (the same rule as snk::radix_for in sn_fft_core.cuh)
+int radix_for(int N, int ns)
+{
+    const int rem = N / ns;
+    if (N % 3 == 0) return rem == 6 ? 6 : 4;
+    return rem >= 8 ? 8 : rem;
+}
 
 int twiddle_entries(int N)
 {
     int total = 0, ns = 1;
     while (ns < N) {
-        const int rem = N / ns, r = rem >= 8 ? 8 : rem;
+        const int r = radix_for(N, ns);
         if (ns > 1) total += ns * (r - 1);
         ns *= r;
     }
@@ -191,14 +204,15 @@ int make_tensor_maps(sn_ctx *c)
     const Layout &l = c->lay;
     int rc;
     c->m_ok[0] = c->m_ok[1] = false;
-    if (l.n[0] <= 512 && l.cols0 % 16 == 0) {
+    auto pow2 = [](int64_t n) { return (n & (n - 1)) == 0; };
+    if (l.n[0] <= 512 && pow2(l.n[0]) && l.cols0 % 16 == 0) {
         const int n0 = (int)l.n[0];
         if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, n0 < 256 ? n0 : 256))) return rc;
         if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, n0 / 2))) return rc;
         if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1))) return rc;
         c->m_ok[0] = true;
     }
-    if (l.ndim == 3 && l.n[1] <= 512 && l.n[2] % 16 == 0) {
+    if (l.ndim == 3 && l.n[1] <= 512 && pow2(l.n[1]) && l.n[2] % 16 == 0) {
         const int n1 = (int)l.n[1];
         if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
         if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
@@ -238,7 +252,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C;
         const int axis = strided ? a.axis : 0;
         const bool maps = (strided || haxis) ? c->m_ok[axis] : true;
-        if (maps && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
+        if (maps && (N & (N - 1)) == 0 && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
             pa.a = a;
@@ -273,6 +287,9 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         }
     }
     switch (N) {
+    case 96: rc = snk::launch_pass<96>(a); break;
+    case 384: rc = snk::launch_pass<384>(a); break;
+    case 1536: rc = snk::launch_pass<1536>(a); break;
     case 64: rc = snk::launch_pass<64>(a); break;
     case 128: rc = snk::launch_pass<128>(a); break;
     case 256: rc = snk::launch_pass<256>(a); break;
@@ -321,7 +338,7 @@ int upload_static_tables(sn_ctx *c)
         std::vector<f4> tw;
         tw.reserve(twiddle_entries(N));
         for (int ns = 1; ns < N;) {
-            const int rem = N / ns, r = rem >= 8 ? 8 : rem;
+            const int r = radix_for(N, ns);
             if (ns > 1)
                 for (int q = 1; q < r; q++)
                     for (int kp = 0; kp < ns; kp++) {
@@ -705,7 +722,7 @@ const char *sn_strerror(int code)
     switch (code) {
     case SN_OK: return "ok";
     case SN_ERR_NULL: return "null pointer argument";
-    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths powers of two in [64, 4096])";
+    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths 2^n in [64, 4096] or 96, 384, 1536)";
     case SN_ERR_PARAM: return "invalid parameter";
     case SN_ERR_SINGULAR: return "C > 0 coincides with k^2 of a grid mode: eq. (2) is singular";
     case SN_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";

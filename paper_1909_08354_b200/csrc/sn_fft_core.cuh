@@ -1,7 +1,9 @@
 // sn_fft_core.cuh -- register/shared-memory Stockham line FFT engine (sm_100a).
 //
 // The "Fourier methods" of PAPER.md:113 (section III) are hand-written here: one line of
-// N = 2^n complex64 points is held by T = N/8 threads, 8 points per thread in registers.
+// N = 2^n complex64 points is held by T = N/8 threads, 8 points per thread in registers
+// (N = 6*4^a: T = N/12 threads, 12 points per thread, radix-4 stages and a final radix-6 stage
+// done as 2 x 3 with prime-factor index maps).
 // Every thread carries TWO independent lines (a[], b[]) so that each twiddle load, each
 // shared-memory instruction (128-bit: one point of each line) and each index computation is
 // amortised over two transforms.  Stages are radix-8 (a trailing radix-2/4 stage when n is
@@ -25,6 +27,9 @@ namespace snk {
 constexpr double SQRT_HALF_D = 0.70710678118654752440084436210485;
 constexpr float C8_HI = (float)SQRT_HALF_D;
 constexpr float C8_LO = (float)(SQRT_HALF_D - (double)C8_HI);
+constexpr double SIN60_D = 0.86602540378443864676372317075294;
+constexpr float S3_HI = (float)SIN60_D;
+constexpr float S3_LO = (float)(SIN60_D - (double)S3_HI);
 
 __device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
@@ -107,12 +112,43 @@ __device__ __forceinline__ void bf8(float2 &x0, float2 &x1, float2 &x2, float2 &
     x0 = a0; x1 = b0; x2 = a1; x3 = b1; x4 = a2; x5 = b2; x6 = a3; x7 = b3;
 }
 
+// 3-point DFT in place; W3 = -1/2 -+ i sqrt(3)/2 (sqrt(3)/2 as hi/lo like the twiddles)
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf3(float2 &x0, float2 &x1, float2 &x2)
+{
+    const float2 t = cadd(x1, x2), u = csub(x1, x2);
+    const float2 m = make_float2(fmaf(-0.5f, t.x, x0.x), fmaf(-0.5f, t.y, x0.y));
+    const float vx = HILO ? fmaf(u.x, S3_HI, u.x * S3_LO) : u.x * S3_HI;
+    const float vy = HILO ? fmaf(u.y, S3_HI, u.y * S3_LO) : u.y * S3_HI;
+    // forward: X1 = m - i v, X2 = m + i v; inverse: swapped
+    const float2 iv = DIR > 0 ? make_float2(vy, -vx) : make_float2(-vy, vx);
+    x0 = cadd(x0, t);
+    x1 = cadd(m, iv);
+    x2 = csub(m, iv);
+}
+
+// 6-point DFT, natural order in and out, as 2 x 3 with the prime-factor index maps
+// n = (3 n1 + 2 n2) mod 6, k = (3 k1 + 4 k2) mod 6 (no twiddles between the factors).
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf6(float2 &x0, float2 &x1, float2 &x2, float2 &x3, float2 &x4, float2 &x5)
+{
+    float2 s0 = cadd(x0, x3), d0 = csub(x0, x3); // n2 = 0: x[0], x[3]
+    float2 s1 = cadd(x2, x5), d1 = csub(x2, x5); // n2 = 1: x[2], x[5]
+    float2 s2 = cadd(x4, x1), d2 = csub(x4, x1); // n2 = 2: x[4], x[1]
+    bf3<DIR, HILO>(s0, s1, s2);                  // k1 = 0: X[0], X[4], X[2]
+    bf3<DIR, HILO>(d0, d1, d2);                  // k1 = 1: X[3], X[1], X[5]
+    x0 = s0; x4 = s1; x2 = s2; x3 = d0; x1 = d1; x5 = d2;
+}
+
 // radix-R butterfly on x[q + r*NB], r = 0..R-1
-template <int R, int NB, int DIR, bool HILO>
-__device__ __forceinline__ void butterfly(float2 (&x)[8], int q)
+template <int R, int NB, int DIR, bool HILO, int P>
+__device__ __forceinline__ void butterfly(float2 (&x)[P], int q)
 {
     if constexpr (R == 8) {
-        bf8<DIR, HILO>(x[0], x[1], x[2], x[3], x[4], x[5], x[6], x[7]);
+        bf8<DIR, HILO>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB], x[q + 4 * NB], x[q + 5 * NB], x[q + 6 * NB],
+                       x[q + 7 * NB]);
+    } else if constexpr (R == 6) {
+        bf6<DIR, HILO>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB], x[q + 4 * NB], x[q + 5 * NB]);
     } else if constexpr (R == 4) {
         bf4<DIR>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB]);
     } else {
@@ -120,13 +156,22 @@ __device__ __forceinline__ void butterfly(float2 (&x)[8], int q)
     }
 }
 
+// Engine shape per length.  N = 2^n: 8 points per thread and line, radix-8 stages with a trailing
+// radix-4/2.  N = 6 * 4^a (96, 384, 1536): 12 points per thread, radix-4 stages and a final radix-6.
+__host__ __device__ constexpr int ppt_for(int N) { return N % 3 == 0 ? 12 : 8; }
+__host__ __device__ constexpr int radix_for(int N, int NS)
+{
+    const int rem = N / NS;
+    if (N % 3 == 0) return rem == 6 ? 6 : 4;
+    return rem >= 8 ? 8 : rem;
+}
+
 // Number of float4 twiddle entries of the table for length N (all stages with NS > 1).
-constexpr int twiddle_entries(int N)
+__host__ __device__ constexpr int twiddle_entries(int N)
 {
     int total = 0, ns = 1;
     while (ns < N) {
-        const int rem = N / ns;
-        const int r = rem >= 8 ? 8 : rem;
+        const int r = radix_for(N, ns);
         if (ns > 1) total += ns * (r - 1);
         ns *= r;
     }
@@ -138,10 +183,10 @@ constexpr int twiddle_entries(int N)
 // thread's own points j + T*(q + r*NB) = bq + r*N/R; twiddle exp(-/+ 2 pi i r (bq % NS)/(NS R)),
 // stored at tw[(r-1)*NS + (bq % NS)] so that lanes with consecutive j read consecutive entries.
 // ONE = true: only line a is transformed (b is never touched).
-template <int N, int R, int NS, int DIR, bool HILO, bool ONE>
-__device__ __forceinline__ void stage_compute(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw)
+template <int N, int R, int NS, int DIR, bool HILO, bool ONE, int P>
+__device__ __forceinline__ void stage_compute(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw)
 {
-    constexpr int T = N / 8, NB = 8 / R;
+    constexpr int T = N / P, NB = P / R;
 #pragma unroll
     for (int q = 0; q < NB; q++) {
         if constexpr (NS > 1) {
@@ -191,10 +236,10 @@ __device__ __forceinline__ int comb(int tb, int K, int PM)
 
 // Stockham exchange after a stage (NS, R): output r of butterfly bq goes to position
 // (bq / NS) * NS * R + (bq % NS) + r * NS; afterwards thread j re-reads points j + T*m.
-template <int N, int R, int NS, class SM>
-__device__ __forceinline__ void stage_exchange(float2 (&a)[8], float2 (&b)[8], int j, SM &sm)
+template <int N, int R, int NS, class SM, int P>
+__device__ __forceinline__ void stage_exchange(float2 (&a)[P], float2 (&b)[P], int j, SM &sm)
 {
-    constexpr int T = N / 8, NB = 8 / R;
+    constexpr int T = N / P, NB = P / R;
     constexpr int WPM = ((T - 1) & ~(NS - 1)) * R | ((T - 1) & (NS - 1)); // position bits of butterfly j's base
     sm.sync(); // previous readers of the buffer are done
     const int tbw = sm.idx((j & ~(NS - 1)) * R + (j & (NS - 1)));
@@ -207,15 +252,15 @@ __device__ __forceinline__ void stage_exchange(float2 (&a)[8], float2 (&b)[8], i
     sm.sync();
     const int tbr = sm.idx(j);
 #pragma unroll
-    for (int m = 0; m < 8; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), a[m], b[m]);
+    for (int m = 0; m < P; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), a[m], b[m]);
 }
 
-template <int N, int NS, int DIR, bool HILO, bool ONE, class SM>
-__device__ __forceinline__ void fft_stages(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw,
+template <int N, int NS, int DIR, bool HILO, bool ONE, class SM, int P>
+__device__ __forceinline__ void fft_stages(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw,
                                            SM &sm)
 {
-    constexpr int REM = N / NS;
-    constexpr int R = REM >= 8 ? 8 : REM;
+    static_assert(P == ppt_for(N), "points per thread");
+    constexpr int R = radix_for(N, NS);
     stage_compute<N, R, NS, DIR, HILO, ONE>(a, b, j, tw);
     if constexpr (NS * R < N) {
         stage_exchange<N, R, NS, SM>(a, b, j, sm);
@@ -223,19 +268,19 @@ __device__ __forceinline__ void fft_stages(float2 (&a)[8], float2 (&b)[8], int j
     }
 }
 
-// Unscaled DFT of two lines.  In: thread j holds points j + T*m of each line (T = N/8).
+// Unscaled DFT of two lines.  In: thread j holds points j + T*m of each line (T = N/P, P = ppt_for(N)).
 // Out: thread j holds outputs j + T*m.  DIR = +1: sum x e^{-2 pi i jk/N}; DIR = -1: e^{+...}.
-template <int N, int DIR, bool HILO, class SM>
-__device__ __forceinline__ void fft_pair(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ tw, SM &sm)
+template <int N, int DIR, bool HILO, class SM, int P>
+__device__ __forceinline__ void fft_pair(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
     fft_stages<N, 1, DIR, HILO, false, SM>(a, b, j, tw, sm);
 }
 
 // Same for ONE line (a); the accessor SM stores/loads only a.
-template <int N, int DIR, bool HILO, class SM>
-__device__ __forceinline__ void fft_single(float2 (&a)[8], int j, const float4 *__restrict__ tw, SM &sm)
+template <int N, int DIR, bool HILO, class SM, int P>
+__device__ __forceinline__ void fft_single(float2 (&a)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
-    float2 dummy[8];
+    float2 dummy[P];
     fft_stages<N, 1, DIR, HILO, true, SM>(a, dummy, j, tw, sm);
 }
 

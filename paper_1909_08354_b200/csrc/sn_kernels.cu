@@ -45,8 +45,9 @@ __device__ __forceinline__ void block_accumulate(double (&v)[NV], double *out)
 
 // column pairs per CTA tile: 512-point lines run as two 256-thread CTAs per SM (measured 15-30 % faster
 // than one 512-thread CTA: the second CTA's loads overlap the first one's butterflies)
-__host__ __device__ constexpr int cp_for(int N) { return N <= 256 ? 8 : (N <= 1024 ? 4 : 4096 / N); }
-__host__ __device__ constexpr int sblocks(int N) { return cp_for(N) * N / 8 <= 256 ? 2 : 1; }
+__host__ __device__ constexpr int cp_for(int N) { return N <= 256 ? 8 : (N <= 1024 ? 4 : (N <= 2048 ? 2 : 1)); }
+__host__ __device__ constexpr int sthreads(int N) { return cp_for(N) * (N / ppt_for(N)); }
+__host__ __device__ constexpr int sblocks(int N) { return sthreads(N) <= 256 ? 2 : 1; }
 
 // ---------------------------------------------------------------------------- strided axis
 // Tile: N rows (points of the line, `row_stride` elements apart) x 2*CP adjacent columns.
@@ -54,10 +55,10 @@ __host__ __device__ constexpr int sblocks(int N) { return cp_for(N) * N / 8 <= 2
 // lanes read/write one 128-byte row segment.
 
 template <int N, int CP, int MODE, int DIR, bool HILO>
-__global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArgs p)
+__global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_strided(const PassArgs p)
 {
     extern __shared__ float4 smem[];
-    constexpr int T = N / 8;
+    constexpr int P = ppt_for(N), T = N / P;
     const int t = threadIdx.x % CP, j = threadIdx.x / CP;
     const int tiles_per_outer = p.ncols / (2 * CP);
     const int outer = blockIdx.x / tiles_per_outer, tile = blockIdx.x % tiles_per_outer;
@@ -65,9 +66,9 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArg
     const long long rs4 = p.row_stride / 2;
     SmemTile<CP> sm{smem, t};
 
-    float2 a[8], b[8];
+    float2 a[P], b[P];
 #pragma unroll
-    for (int m = 0; m < 8; m++) {
+    for (int m = 0; m < P; m++) {
         const float4 v = g4[(long long)(j + T * m) * rs4];
         a[m] = lo2(v);
         b[m] = hi2(v);
@@ -76,7 +77,7 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArg
         fft_pair<N, DIR, HILO>(a, b, j, p.tw, sm);
         const float s = p.scale;
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             if (DIR < 0) {
                 a[m].x *= s; a[m].y *= s; b[m].x *= s; b[m].y *= s;
             }
@@ -85,19 +86,19 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArg
     } else if (MODE == P_S_KIN) {
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 ph = __ldg(p.phase + j + T * m);
             a[m] = twmul<+1, true>(a[m], ph);
             b[m] = twmul<+1, true>(b[m], ph);
         }
         fft_pair<N, -1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
+        for (int m = 0; m < P; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
     } else { // P_S_KDIAG
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
         float acc = 0.f;
 #pragma unroll
-        for (int m = 0; m < 8; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
+        for (int m = 0; m < P; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
         double v[1] = {(double)acc};
         block_accumulate<1>(v, p.diag);
     }
@@ -115,16 +116,16 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_strided(const PassArg
 
 template <int N, int CP, class SM>
 __device__ __forceinline__ void c2r_potential(const PassArgs &p, const float4 *hs4, long long rs4, int t, int j,
-                                              float2 (&fa)[8], float2 (&fb)[8], SM &sm)
+                                              float2 (&fa)[ppt_for(N)], float2 (&fb)[ppt_for(N)], SM &sm)
 {
-    constexpr int T = N / 8;
+    constexpr int P = ppt_for(N), T = N / P;
 #pragma unroll
-    for (int m = 0; m < 8; m++) {
+    for (int m = 0; m < P; m++) {
         const int km = j + T * m;
-        const int src = m < 4 ? km : N - km; // m >= 4: km >= N/2, mirrored row in [0, N/2]
+        const int src = m < P / 2 ? km : N - km; // m >= P/2: km >= N/2, mirrored row in [0, N/2]
         const float4 u = hs4[(long long)src * rs4 + t];
         const float4 v = hs4[(long long)src * rs4 + CP + t];
-        if (m < 4) {
+        if (m < P / 2) {
             fa[m] = make_float2(u.x - u.w, u.y + u.z);
             fb[m] = make_float2(v.x - v.w, v.y + v.z);
         } else {
@@ -137,10 +138,10 @@ __device__ __forceinline__ void c2r_potential(const PassArgs &p, const float4 *h
 }
 
 template <int N, int CP, int MODE>
-__global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs p)
+__global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArgs p)
 {
     extern __shared__ float4 smem[];
-    constexpr int T = N / 8;
+    constexpr int P = ppt_for(N), T = N / P;
     const int t = threadIdx.x % CP, j = threadIdx.x / CP;
     const long long rs4 = p.row_stride / 2;
     const long long col4 = (long long)blockIdx.x * 2 * CP; // first column pair of the tile
@@ -149,9 +150,9 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
     SmemTile<CP> sm{smem, t};
 
     if (MODE == P_H_R2C) {
-        float2 a[8], b[8];
+        float2 a[P], b[P];
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
             const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
             a[m] = make_float2(abs2(lo2(u)), abs2(hi2(u)));
@@ -160,14 +161,14 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
         fft_pair<N, +1, false>(a, b, j, p.tw, sm);
         sm.sync();
 #pragma unroll
-        for (int m = 0; m < 8; m++) sm.st(j + T * m, a[m], b[m]);
+        for (int m = 0; m < P; m++) sm.st(j + T * m, a[m], b[m]);
         sm.sync();
 #pragma unroll
-        for (int m = 0; m < 5; m++) {
-            if (m < 4 || j == 0) {
+        for (int m = 0; m <= P / 2; m++) {
+            if (m < P / 2 || j == 0) {
                 const int k = j + T * m;
                 float2 ya, yb;
-                sm.ld((N - k) & (N - 1), ya, yb);
+                sm.ld((N - k) % N, ya, yb);
                 hs4[(long long)k * rs4 + t] = make_float4(a[m].x + ya.x, a[m].y - ya.y, a[m].y + ya.y, ya.x - a[m].x);
                 hs4[(long long)k * rs4 + CP + t] =
                     make_float4(b[m].x + yb.x, b[m].y - yb.y, b[m].y + yb.y, yb.x - b[m].x);
@@ -176,13 +177,13 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
         return;
     }
 
-    float2 fa[8], fb[8];
+    float2 fa[P], fb[P];
     c2r_potential<N, CP>(p, hs4, rs4, t, j, fa, fb, sm);
 
     if (MODE == P_H_POT) {
         float2 *out = reinterpret_cast<float2 *>(p.phi_out) + col4;
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             out[(long long)(j + T * m) * rs4 + t] = fa[m];
             out[(long long)(j + T * m) * rs4 + CP + t] = fb[m];
         }
@@ -191,7 +192,7 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
     if (MODE == P_H_DIAG) {
         float s_rho = 0.f, s_pr = 0.f, s_f = 0.f;
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
             const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
             const float r[4] = {abs2(lo2(u)), abs2(hi2(u)), abs2(lo2(v)), abs2(hi2(v))};
@@ -213,9 +214,9 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
 #pragma unroll
     for (int half = 0; half < 2; half++) {
         float4 *g4 = psi4 + half * CP + t;
-        float2 a[8], b[8];
+        float2 a[P], b[P];
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 v = g4[(long long)(j + T * m) * rs4];
             const float2 ph = half == 0 ? fa[m] : fb[m];
             a[m] = nl_phase(lo2(v), ph.x, p.nl);
@@ -223,14 +224,14 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
         }
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 ph = __ldg(p.phase + j + T * m);
             a[m] = twmul<+1, true>(a[m], ph);
             b[m] = twmul<+1, true>(b[m], ph);
         }
         fft_pair<N, -1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
+        for (int m = 0; m < P; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
     }
 }
 
@@ -238,13 +239,13 @@ __global__ void __launch_bounds__(CP *N / 8, sblocks(N)) k_haxis(const PassArgs 
 // A group of T = N/8 threads owns two adjacent lines; lanes are consecutive j, so every global
 // access of a warp is one contiguous 256-byte run of a line.
 
-__host__ __device__ constexpr int xthreads(int N) { return N / 8 >= 256 ? N / 8 : 256; }
+__host__ __device__ constexpr int xthreads(int N) { return N / ppt_for(N) >= 256 ? N / ppt_for(N) : 256; }
 
 template <int N, int MODE, int DIR, bool HILO>
 __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_contig(const PassArgs p)
 {
     extern __shared__ float4 smem[];
-    constexpr int T = N / 8, G = xthreads(N) / T;
+    constexpr int P = ppt_for(N), T = N / P, G = xthreads(N) / T;
     const int j = threadIdx.x % T, grp = threadIdx.x / T;
     const long long pair = (long long)blockIdx.x * G + grp;
     const bool active = 2 * pair < p.nlines;
@@ -253,9 +254,9 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
     float2 *lb = la + N;
     SmemLine<T> sm{smem + grp * N, 1 + grp, G == 1};
 
-    float2 a[8], b[8];
+    float2 a[P], b[P];
 #pragma unroll
-    for (int m = 0; m < 8; m++) {
+    for (int m = 0; m < P; m++) {
         a[m] = la[j + T * m];
         b[m] = lb[j + T * m];
     }
@@ -263,7 +264,7 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         fft_pair<N, DIR, HILO>(a, b, j, p.tw, sm);
         const float s = p.scale;
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             if (DIR < 0) {
                 a[m].x *= s; a[m].y *= s; b[m].x *= s; b[m].y *= s;
             }
@@ -273,14 +274,14 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
     } else if (MODE == P_X_KIN) {
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 ph = __ldg(p.phase + j + T * m);
             a[m] = twmul<+1, true>(a[m], ph);
             b[m] = twmul<+1, true>(b[m], ph);
         }
         fft_pair<N, -1, true>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             la[j + T * m] = a[m];
             lb[j + T * m] = b[m];
         }
@@ -289,7 +290,7 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         fft_pair<N, +1, false>(a, b, j, p.tw, sm);
         const float ka = __ldg(p.kother2 + 2 * pair), kb = __ldg(p.kother2 + 2 * pair + 1);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float kx2 = __ldg(p.ksq + j + T * m);
             const float da = p.C - kx2 - ka, db = p.C - kx2 - kb;
             const float ga = da == 0.f ? 0.f : p.pscale / da;
@@ -298,7 +299,7 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         }
         fft_pair<N, -1, false>(a, b, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             la[j + T * m] = a[m];
             lb[j + T * m] = b[m];
         }
@@ -306,7 +307,7 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
         float acc = 0.f;
 #pragma unroll
-        for (int m = 0; m < 8; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
+        for (int m = 0; m < P; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
         double v[1] = {active ? (double)acc : 0.0};
         block_accumulate<1>(v, p.diag);
     }
@@ -328,7 +329,7 @@ static int launch_kernel(K kern, unsigned grid, int threads, size_t smem_bytes, 
 template <int N>
 int launch_pass(const PassArgs &a)
 {
-    constexpr int CP = cp_for(N), T = N / 8;
+    constexpr int CP = cp_for(N), T = N / ppt_for(N);
     constexpr int ST = CP * T;                       // threads of a strided-axis CTA
     constexpr size_t SSMEM = (size_t)N * CP * 16;    // one float4 per point and column pair
     constexpr int XT = xthreads(N), G = XT / T;

@@ -58,7 +58,8 @@ def run_pair(mods, cfg, steps, split=None):
 # ------------------------------------------------------------------ transforms
 
 FFT_DIMS = [(64, 64), (128, 256), (512, 64), (64, 1024), (2048, 64), (64, 4096), (4096, 128),
-            (64, 64, 64), (128, 64, 256), (64, 512, 128)]
+            (64, 64, 64), (128, 64, 256), (64, 512, 128),
+            (96, 96), (384, 64), (64, 384), (1536, 64), (64, 1536), (96, 384, 64)]   # 6*4^a lengths (radix-6 stage)
 
 
 @pytest.mark.parametrize("dims", FFT_DIMS)
@@ -90,7 +91,8 @@ def test_round_trip_on_config_states(mods, name):
 
 # ------------------------------------------------------------------ eq. (2): potential
 
-@pytest.mark.parametrize("dims,C", [((64, 128), 0.0), ((128, 64), -1.0), ((64, 64, 128), 0.0), ((64, 128, 64), -0.7)])
+@pytest.mark.parametrize("dims,C", [((64, 128), 0.0), ((128, 64), -1.0), ((64, 64, 128), 0.0), ((64, 128, 64), -0.7),
+                                    ((384, 96), 0.0), ((96, 64, 384), -0.7)])
 def test_potential_matches_oracle(mods, dims, C):
     snref, Oracle, inputs, sn = mods
     cfg = inputs.scaled(inputs.CONFIGS["C2" if len(dims) == 2 else "C4"], dims, L=16.0)
@@ -146,6 +148,10 @@ STEP_CASES = [
     ("C5_128", (128, 128, 128), 128.0, 10),
     ("C4", (64, 128, 256), 32.0, 10),     # rectangular 3D, three different line lengths
     ("C5_256", (256, 256, 256), 128.0, 2),  # many tiles per pass
+    ("C2", (384, 96), 25.0, 100),           # 6*4^a line lengths on both axes
+    ("C5_384", (96, 96, 96), 128.0, 20),    # the sweep's 3*2^7 family, coarse
+    ("C5_384", (384, 64, 128), 128.0, 4),   # 384-point strided lines next to pipelined axes
+    ("C5_384", (64, 128, 384), 128.0, 4),   # 384-point contiguous lines
 ]
 
 
