@@ -54,8 +54,8 @@ typedef struct {
 } sn_diag;
 
 /* Supported axis lengths: powers of two with 64 <= N <= 4096, and 6*4^a = 96, 384, 1536 (radix-4 stages
- * plus one radix-6 stage; the grid-size sweep's 384^3).  Otherwise sn_workspace_bytes returns 0 and
- * sn_create returns SN_ERR_DIMS otherwise).  Bytes of device workspace needed. */
+ * plus one radix-6 stage; the grid-size sweep's 384^3).  Any other length: sn_workspace_bytes
+ * returns 0 and sn_create returns SN_ERR_DIMS.  Bytes of device workspace needed. */
 size_t sn_workspace_bytes(int ndim, const int64_t *dims /* host, ndim entries */);
 
 /* Create a context.

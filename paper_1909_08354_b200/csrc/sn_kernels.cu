@@ -318,7 +318,7 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
 template <class K>
 static int launch_kernel(K kern, unsigned grid, int threads, size_t smem_bytes, const PassArgs &a)
 {
-    if (smem_bytes > 48 * 1024) {
+    if (smem_bytes > 40 * 1024) { // static shared memory (block_accumulate) counts against the 48 KB default too
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return (int)e;
     }

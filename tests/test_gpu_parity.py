@@ -258,7 +258,8 @@ def test_time_reversal(mods):
 
 # ------------------------------------------------------------------ diagnostics and edge cases
 
-@pytest.mark.parametrize("name,dims,L", [("C2", (128, 256), 20.0), ("C4", (64, 128, 64), 16.0)])
+@pytest.mark.parametrize("name,dims,L", [("C2", (128, 256), 20.0), ("C4", (64, 128, 64), 16.0),
+                                         ("C5_384", (96, 64, 384), 128.0), ("C5_384", (384, 96, 64), 128.0)])
 def test_diagnostics_match_oracle(mods, name, dims, L):
     snref, Oracle, inputs, sn = mods
     cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L)
