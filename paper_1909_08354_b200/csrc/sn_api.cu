@@ -123,6 +123,12 @@ struct sn_ctx {
     int sm_count;
     CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row;
     bool m_ok[2];
+    // CUDA graph of one interior step [N(dtau) K(dtau)] for launch-bound grids (<= 2^24 cells): captured once
+    // on a private stream, replayed on the caller's stream
+    bool use_graph;
+    cudaStream_t cap_stream;
+    cudaGraphExec_t step_graph;
+    int graph_launches; // kernels inside the graph
     // optional per-launch timing (sn_profile): event pairs around every launch, summed per pass kind
     bool profiling;
     std::vector<cudaEvent_t> *ev;       // pool, pairs (start, stop)
@@ -459,6 +465,41 @@ int potential_spectrum(sn_ctx *c)
     return SN_OK;
 }
 
+// capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
+int build_step_graph(sn_ctx *c)
+{
+    if (!c->cap_stream) SN_CUDA(cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+    const cudaStream_t user = c->stream;
+    const int64_t before = c->launches;
+    SN_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+    c->stream = c->cap_stream;
+    int rc = potential_spectrum(c);
+    if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/false, /*with_nl=*/true);
+    c->stream = user;
+    cudaGraph_t g = nullptr;
+    const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
+    c->graph_launches = (int)(c->launches - before);
+    c->launches = before;
+    if (rc != SN_OK) {
+        if (g) cudaGraphDestroy(g);
+        return rc;
+    }
+    if (e != cudaSuccess) return cuda_fail(e);
+    const cudaError_t e2 = cudaGraphInstantiate(&c->step_graph, g, 0);
+    cudaGraphDestroy(g);
+    if (e2 != cudaSuccess) {
+        c->step_graph = nullptr;
+        return cuda_fail(e2);
+    }
+    return SN_OK;
+}
+
+void drop_step_graph(sn_ctx *c)
+{
+    if (c->step_graph) cudaGraphExecDestroy(c->step_graph);
+    c->step_graph = nullptr;
+}
+
 } // namespace
 
 // ============================================================================ C ABI
@@ -523,6 +564,8 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
     if (rc == SN_OK) rc = upload_phase_tables(c);
     if (rc == SN_OK) {
         int dev = 0;
+        const char *ng = std::getenv("SN_NO_GRAPH"); // SN_NO_GRAPH=1: plain stream launches for every grid
+        c->use_graph = l.cells <= ((int64_t)1 << 24) && !(ng && ng[0] == '1');
         const char *np = std::getenv("SN_NO_PIPE"); // SN_NO_PIPE=1: first-path kernels only (A/B runs, tests)
         c->use_pipe = !(np && np[0] == '1');
         if (cudaGetDevice(&dev) != cudaSuccess ||
@@ -543,6 +586,8 @@ int sn_destroy(sn_ctx *c)
 {
     if (!c) return SN_ERR_NULL;
     cudaStreamSynchronize(c->stream);
+    drop_step_graph(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->ev) {
         for (cudaEvent_t e : *c->ev) cudaEventDestroy(e);
         delete c->ev;
@@ -559,6 +604,7 @@ int sn_set_dtau(sn_ctx *c, double dtau)
     const double old = c->dtau;
     c->dtau = dtau;
     SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c); // the nonlinear-phase coefficients are kernel arguments baked into the graph
     const int rc = upload_phase_tables(c);
     if (rc != SN_OK) c->dtau = old;
     return rc;
@@ -592,7 +638,15 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     if (nsteps == 0) return SN_OK;
     // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
     int rc = kinetic_sweep(c, /*half=*/true, /*with_nl=*/false);
-    for (int64_t i = 1; rc == SN_OK && i <= nsteps; i++) {
+    int64_t i = 1;
+    if (rc == SN_OK && c->use_graph && !c->profiling && nsteps >= 4) {
+        if (!c->step_graph) rc = build_step_graph(c);
+        for (; rc == SN_OK && i < nsteps; i++) {
+            SN_CUDA(cudaGraphLaunch(c->step_graph, c->stream));
+            c->launches += c->graph_launches;
+        }
+    }
+    for (; rc == SN_OK && i <= nsteps; i++) {
         rc = potential_spectrum(c);
         if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/i == nsteps, /*with_nl=*/true);
     }

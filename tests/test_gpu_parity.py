@@ -316,3 +316,28 @@ def test_device_state_round_trip_and_launch_count(mods):
     # 3D: 3 kinetic passes + 4 steps x (r2c, y fwd, x Poisson, y inv + 3 kinetic passes)
     assert sim.launch_count() - n0 == 3 + 4 * 7
     sim.close()
+
+
+@pytest.mark.parametrize("dims,L,name", [((512, 128), 50.0, "C3"), ((64, 256, 128), 32.0, "C4")])
+def test_first_path_and_pipelined_kernels_agree(mods, dims, L, name, monkeypatch):
+    """SN_NO_PIPE=1 (read at sn_create) routes every pass to the first-path kernels of sn_kernels.cu; the
+    default uses the TMA-pipelined kernels of sn_pipe.cu.  Same arithmetic order inside a line, so the two
+    agree to a few ulp, and both meet the oracle tolerance."""
+    snref, Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=6)
+    psi0 = cfg.initial_state()
+    out = {}
+    for mode in ("0", "1"):
+        monkeypatch.setenv("SN_NO_PIPE", mode)
+        sim = sn.Simulation.from_config(cfg)
+        sim.set_state(psi0)
+        sim.step(cfg.steps)
+        out[mode] = sim.get_state()
+        sim.close()
+    orc = Oracle.from_config(cfg)
+    orc.set_state(psi0.astype(np.complex128))
+    orc.step(cfg.steps)
+    want = orc.get_state()
+    orc.close()
+    assert rel(out["0"], want) < TOL_STATE and rel(out["1"], want) < TOL_STATE
+    assert rel(out["0"], out["1"]) < 5e-6
