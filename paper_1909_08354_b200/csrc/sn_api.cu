@@ -183,8 +183,9 @@ encode_tiled_fn get_encode_fn()
     return fn;
 }
 
-// complex64 array [outer][rows][cols] seen as float32 [outer][rows][2*cols]; box = 16 complex x box_rows x 1
-int make_map(CUtensorMap *m, void *ptr, int64_t outer, int64_t rows, int64_t cols, int box_rows)
+// complex64 array [outer][rows][cols] seen as float32 [outer][rows][2*cols]; box = 2*cpw complex x box_rows x 1
+// (cpw column pairs = 16*cpw bytes per row, swizzled over exactly that width: 128B / 64B / 32B / none)
+int make_map(CUtensorMap *m, void *ptr, int64_t outer, int64_t rows, int64_t cols, int box_rows, int cpw)
 {
     encode_tiled_fn fn = get_encode_fn();
     if (!fn) {
@@ -193,10 +194,13 @@ int make_map(CUtensorMap *m, void *ptr, int64_t outer, int64_t rows, int64_t col
     }
     const cuuint64_t gdim[3] = {(cuuint64_t)(2 * cols), (cuuint64_t)rows, (cuuint64_t)outer};
     const cuuint64_t gstr[2] = {(cuuint64_t)(cols * 8), (cuuint64_t)(rows * cols * 8)};
-    const cuuint32_t box[3] = {32u, (cuuint32_t)box_rows, 1u};
+    const cuuint32_t box[3] = {(cuuint32_t)(4 * cpw), (cuuint32_t)box_rows, 1u};
+    const CUtensorMapSwizzle swz = cpw == 8 ? CU_TENSOR_MAP_SWIZZLE_128B
+                                 : cpw == 4 ? CU_TENSOR_MAP_SWIZZLE_64B
+                                 : cpw == 2 ? CU_TENSOR_MAP_SWIZZLE_32B : CU_TENSOR_MAP_SWIZZLE_NONE;
     const cuuint32_t estr[3] = {1u, 1u, 1u};
     const CUresult r = fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, ptr, gdim, gstr, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                          CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                          swz, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
                           CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         std::snprintf(g_cuda_msg, sizeof(g_cuda_msg), "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
@@ -211,17 +215,18 @@ int make_tensor_maps(sn_ctx *c)
     int rc;
     c->m_ok[0] = c->m_ok[1] = false;
     auto pow2 = [](int64_t n) { return (n & (n - 1)) == 0; };
-    if (l.n[0] <= 512 && pow2(l.n[0]) && l.cols0 % 16 == 0) {
-        const int n0 = (int)l.n[0];
-        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, n0 < 256 ? n0 : 256))) return rc;
-        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, n0 / 2))) return rc;
-        if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1))) return rc;
+    auto cpw_of = [](int64_t n) { const int g = (int)(4096 / n); return g < 8 ? g : 8; }; // column pairs per box row
+    if (pow2(l.n[0]) && l.cols0 % (2 * (4096 / l.n[0])) == 0) {
+        const int n0 = (int)l.n[0], cpw = cpw_of(n0);
+        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, n0 < 256 ? n0 : 256, cpw))) return rc;
+        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, n0 / 2 < 256 ? n0 / 2 : 256, cpw))) return rc;
+        if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
         c->m_ok[0] = true;
     }
-    if (l.ndim == 3 && l.n[1] <= 512 && pow2(l.n[1]) && l.n[2] % 16 == 0) {
-        const int n1 = (int)l.n[1];
-        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
-        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], n1 < 256 ? n1 : 256))) return rc;
+    if (l.ndim == 3 && pow2(l.n[1]) && l.n[2] % (2 * (4096 / l.n[1])) == 0) {
+        const int n1 = (int)l.n[1], cpw = cpw_of(n1);
+        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], n1 < 256 ? n1 : 256, cpw))) return rc;
+        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], n1 < 256 ? n1 : 256, cpw))) return rc;
         c->m_ok[1] = true;
     }
     return SN_OK;

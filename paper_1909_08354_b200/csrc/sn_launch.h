@@ -81,7 +81,7 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
     case P_S_KIN:
     case P_H_NLKIN:
     case P_H_R2C:
-        return N <= 512 && ncols % (2 * (4096 / N)) == 0; // a tile is 2 * 512/(N/8) columns wide
+        return ncols % (2 * (4096 / N)) == 0; // a tile is 2 * 512/(N/8) columns wide
     case P_X_KIN:
     case P_X_POISSON:
         return nlines % 2 == 0;

@@ -30,36 +30,50 @@ namespace snk {
 
 constexpr int PIPE_THREADS = 512;
 constexpr int PIPE_WARPS = PIPE_THREADS / 32;
-constexpr int TILE_BYTES = 65536; // N rows x 2G columns x 8 B, for every N <= 512
+constexpr int TILE_BYTES = 65536; // N rows x 2G columns x 8 B, for every N
 
 template <int N>
 struct Geo {
     static constexpr int T = N / 8;                       // threads per line pair
     static constexpr int G = PIPE_THREADS / T;            // line pairs (groups) per tile
-    static constexpr int SUB = G / 8;                     // 128-byte wide sub-tiles
+    static constexpr int CPW = G < 8 ? G : 8;             // column pairs per sub-tile row (8 for N <= 512)
+    static constexpr int RBY = 16 * CPW;                  // bytes of a sub-tile row: 128, 64, 32, 16
+    static constexpr int SUB = G / CPW;                   // sub-tiles per tile
     static constexpr int RB = N < 256 ? N : 256;          // rows per TMA box
     static constexpr int NBOX = N / RB;
-    static constexpr int SUB_F4 = N * 8;                  // float4 slots of a psi sub-tile
+    static constexpr int SUB_F4 = N * CPW;                // float4 slots of a psi sub-tile
+    static constexpr int SUB_BYTES = N * RBY;
     static constexpr int HROWS = N / 2 + 1;               // rows of the half spectrum
-    static constexpr int HS_SUB_BYTES = (HROWS * 128 + 1023) / 1024 * 1024;
+    static constexpr int HB = N / 2 < 256 ? N / 2 : 256;  // rows per TMA box of the half spectrum (rows 0..N/2-1)
+    static constexpr int NHBOX = (N / 2) / HB;
+    static constexpr int HS_SUB_BYTES = (HROWS * RBY + 1023) / 1024 * 1024;
     static constexpr int HS_SUB_F4 = HS_SUB_BYTES / 16;
-    static constexpr int HS_TX = SUB * HROWS * 128;       // bytes one hs tile load delivers
+    static constexpr int HS_TX = SUB * HROWS * RBY;       // bytes one hs tile load delivers
 };
 
-// slot (float4 index inside a sub-tile) of row r for column pair t: the TMA SWIZZLE_128B layout
-__device__ __forceinline__ int nat_slot(int r, int t) { return r * 8 + (t ^ (r & 7)); }
+// Slot (float4 index inside a sub-tile) of row r for column pair t < CPW: the layout the TMA swizzle of a
+// RBY-byte-wide box produces (SWIZZLE_128B / 64B / 32B / none): chunk t of row r sits at chunk t ^ swz(r).
+// In every case the 16-byte bank unit (slot mod 8) is a bijection of (r & 7) for fixed t, so 8 lanes on 8
+// consecutive rows never conflict.
+template <int CPW>
+__host__ __device__ constexpr int swz(int r)
+{
+    return CPW == 8 ? (r & 7) : CPW == 4 ? ((r >> 1) & 3) : CPW == 2 ? ((r >> 2) & 1) : 0;
+}
+template <int CPW>
+__device__ __forceinline__ int nat_slot(int r, int t) { return r * CPW + (t ^ swz<CPW>(r)); }
 
 // Exchange accessor for a line PAIR living in its own slots of a swizzled sub-tile: position pos
 // lives in the slot of row pos ^ ((pos >> 3) & 7).
-template <int T>
+template <int T, int CPW>
 struct SmemSub {
     float4 *sub;
     int t, bar_id;
-    static constexpr int TMASK = 7;
+    static constexpr int TMASK = CPW - 1;
     __host__ __device__ static constexpr int lin(int pos)
     {
         const int r = pos ^ ((pos >> 3) & 7);
-        return (r << 3) | (r & 7);
+        return (r * CPW) | swz<CPW>(r);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ t; }
     __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { sub[i] = pack4(a, b); }
@@ -78,15 +92,15 @@ struct SmemSub {
 
 // Exchange accessor for ONE line (float2 per position) living in the first N/2 slots of a group's
 // column pair: position pos -> row q ^ ((q >> 2) & 7), q = pos >> 1, half (pos ^ (pos >> 6)) & 1.
-template <int T>
+template <int T, int CPW>
 struct SmemSubOne {
     float2 *sub2; // the sub-tile as float2
     int t, bar_id;
-    static constexpr int TMASK = 7 << 1;
+    static constexpr int TMASK = (CPW - 1) << 1;
     __host__ __device__ static constexpr int lin(int pos)
     {
         const int q = pos >> 1, r = q ^ ((q >> 2) & 7);
-        return (((r << 3) | (r & 7)) << 1) | ((pos ^ (pos >> 6)) & 1);
+        return (((r * CPW) | swz<CPW>(r)) << 1) | ((pos ^ (pos >> 6)) & 1);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ (t << 1); }
     __device__ __forceinline__ void st_i(int i, float2 a, float2) const { sub2[i] = a; }
@@ -142,11 +156,11 @@ template <int N, int MODE, int DIR, bool HILO>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 3;
+    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 3;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * TILE_BYTES), *done = full + NST;
-    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g / CPW, t = g % CPW;
 
     if (tid == 0) {
         for (int i = 0; i < NST; i++) {
@@ -172,8 +186,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
         for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
             for (int bx = 0; bx < NBOX; bx++)
-                tma_load_3d(base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, &p.m_data, full + b,
-                            2 * (col0 + 16 * ss), bx * RB, outer);
+                tma_load_3d(base + b * TILE_BYTES + ss * g_::SUB_BYTES + bx * RB * RBY, &p.m_data, full + b,
+                            2 * (col0 + 2 * CPW * ss), bx * RB, outer);
     };
     if (tid == 0) {
         if (nk > 0) issue_load(0);
@@ -184,15 +198,15 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
         const int b = k % NST;
         const uint32_t par = (k / NST) & 1;
         float4 *sub = reinterpret_cast<float4 *>(base + b * TILE_BYTES) + s * g_::SUB_F4;
-        SmemSub<T> sm{sub, t, 1 + g};
+        SmemSub<T, CPW> sm{sub, t, 1 + g};
         mbar_wait(full + b, par);
 
         const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
-        float4 *mine = sub + nat_slot(jf, t);     // row jf; rows jf + T m are 8 T m slots further (T % 8 == 0)
+        float4 *mine = sub + nat_slot<CPW>(jf, t);     // row jf; rows jf + T m are CPW T m slots further (T % 8 == 0)
         float2 a[8], c[8];
 #pragma unroll
         for (int m = 0; m < 8; m++) {
-            const float4 v = mine[8 * T * m];
+            const float4 v = mine[CPW * T * m];
             a[m] = lo2(v);
             c[m] = hi2(v);
         }
@@ -213,7 +227,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
         __syncwarp();
 #pragma unroll
-        for (int m = 0; m < 8; m++) mine[8 * T * m] = pack4(a[m], c[m]);
+        for (int m = 0; m < 8; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
         warp_arrive_done(done + b);
 
         if (tid == 0) {
@@ -224,7 +238,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
             for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
                 for (int bx = 0; bx < NBOX; bx++)
-                    tma_store_3d(&p.m_data, base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss),
+                    tma_store_3d(&p.m_data, base + b * TILE_BYTES + ss * g_::SUB_BYTES + bx * RB * RBY, 2 * (col0 + 2 * CPW * ss),
                                  bx * RB, outer);
             bulk_commit();
             if (k + 2 < nk) {
@@ -252,14 +266,14 @@ template <int N, int MODE>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int STAGE_BYTES = TILE_BYTES + SUB * g_::HS_SUB_BYTES;
     constexpr bool LOAD_HS = true;
     static_assert(MODE == P_H_NLKIN, "k_pipe_haxis serves P_H_NLKIN");
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
-    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g / CPW, t = g % CPW;
 
     if (tid == 0) {
         for (int i = 0; i < NST; i++) {
@@ -280,11 +294,13 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
         for (int ss = 0; ss < SUB; ss++) {
 #pragma unroll
             for (int bx = 0; bx < NBOX; bx++)
-                tma_load_3d(st + ss * N * 128 + bx * RB * 128, &p.m_data, full + b, 2 * (col0 + 16 * ss), bx * RB, 0);
+                tma_load_3d(st + ss * g_::SUB_BYTES + bx * RB * RBY, &p.m_data, full + b, 2 * (col0 + 2 * CPW * ss), bx * RB, 0);
             if (LOAD_HS) {
                 uint8_t *hs = st + TILE_BYTES + ss * g_::HS_SUB_BYTES;
-                tma_load_3d(hs, &p.m_hs, full + b, 2 * (col0 + 16 * ss), 0, 0);
-                tma_load_3d(hs + (N / 2) * 128, &p.m_hs_row, full + b, 2 * (col0 + 16 * ss), N / 2, 0);
+#pragma unroll
+                for (int bx = 0; bx < g_::NHBOX; bx++)
+                    tma_load_3d(hs + bx * g_::HB * RBY, &p.m_hs, full + b, 2 * (col0 + 2 * CPW * ss), bx * g_::HB, 0);
+                tma_load_3d(hs + (N / 2) * RBY, &p.m_hs_row, full + b, 2 * (col0 + 2 * CPW * ss), N / 2, 0);
             }
         }
     };
@@ -299,21 +315,21 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
         uint8_t *st = base + b * STAGE_BYTES;
         float4 *sub = reinterpret_cast<float4 *>(st) + s * g_::SUB_F4;
         float4 *hsub = reinterpret_cast<float4 *>(st + TILE_BYTES) + s * g_::HS_SUB_F4;
-        SmemSub<T> sm{sub, t, 1 + g};
+        SmemSub<T, CPW> sm{sub, t, 1 + g};
         mbar_wait(full + b, par);
 
         const int jf = opaque(j), ji = opaque(j), jz = opaque(j); // per-tile copies: see opaque()
-        float4 *mine = sub + nat_slot(jf, t);
+        float4 *mine = sub + nat_slot<CPW>(jf, t);
         {
             float2 z[8];
             // rows jz + T m (m < 4) and N - jz - T m (m >= 4): the mirrored rows step DOWN by 8 T slots
-            const float4 *hup = hsub + nat_slot(jz, t), *hdn = hsub + nat_slot(N / 2 - jz, t);
+            const float4 *hup = hsub + nat_slot<CPW>(jz, t), *hdn = hsub + nat_slot<CPW>(N / 2 - jz, t);
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const float4 u = m < 4 ? hup[8 * T * m] : hdn[-8 * T * (m - 4)];
+                const float4 u = m < 4 ? hup[CPW * T * m] : hdn[-CPW * T * (m - 4)];
                 z[m] = m < 4 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
             }
-            SmemSubOne<T> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
+            SmemSubOne<T, CPW> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
             fft_single<N, -1, false>(z, jz, p.a.tw, sm1);
             // z[m] = (phi[col 2t], phi[col 2t+1]) at row j + T m.  The previous tile's store has had the
             // whole c2r to leave its stage: reload it now.
@@ -324,7 +340,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             float2 a[8], c[8];
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const float4 v = mine[8 * T * m];
+                const float4 v = mine[CPW * T * m];
                 a[m] = nl_phase(lo2(v), z[m].x, p.a.nl);
                 c[m] = nl_phase(hi2(v), z[m].y, p.a.nl);
             }
@@ -333,7 +349,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
             __syncwarp();
 #pragma unroll
-            for (int m = 0; m < 8; m++) mine[8 * T * m] = pack4(a[m], c[m]);
+            for (int m = 0; m < 8; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
         }
         warp_arrive_done(done + b);
 
@@ -344,7 +360,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
             for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
                 for (int bx = 0; bx < NBOX; bx++)
-                    tma_store_3d(&p.m_data, st + ss * N * 128 + bx * RB * 128, 2 * (col0 + 16 * ss), bx * RB, 0);
+                    tma_store_3d(&p.m_data, st + ss * g_::SUB_BYTES + bx * RB * RBY, 2 * (col0 + 2 * CPW * ss), bx * RB, 0);
             bulk_commit();
         }
     }
@@ -359,14 +375,14 @@ template <int N>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int OUT_BYTES = SUB * g_::HS_SUB_BYTES;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint8_t *outb = base + NST * TILE_BYTES;
     uint64_t *full = reinterpret_cast<uint64_t *>(outb + NST * OUT_BYTES), *consumed = full + NST, *done = full + 2 * NST,
              *freeb = full + 3 * NST;
-    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g >> 3, t = g & 7;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g / CPW, t = g % CPW;
 
     if (tid == 0) {
         for (int i = 0; i < NST; i++) {
@@ -388,8 +404,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
         for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
             for (int bx = 0; bx < NBOX; bx++)
-                tma_load_3d(base + b * TILE_BYTES + ss * N * 128 + bx * RB * 128, &p.m_data, full + b,
-                            2 * (col0 + 16 * ss), bx * RB, 0);
+                tma_load_3d(base + b * TILE_BYTES + ss * g_::SUB_BYTES + bx * RB * RBY, &p.m_data, full + b,
+                            2 * (col0 + 2 * CPW * ss), bx * RB, 0);
     };
     if (tid == 0) {
         if (nk > 0) issue_load(0);
@@ -405,10 +421,10 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
         mbar_wait(full + b, par);
         float2 z[8];
         {
-            const float4 *mine = sub + nat_slot(jf, t);
+            const float4 *mine = sub + nat_slot<CPW>(jf, t);
 #pragma unroll
             for (int m = 0; m < 8; m++) {
-                const float4 v = mine[8 * T * m];
+                const float4 v = mine[CPW * T * m];
                 z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
             }
         }
@@ -416,7 +432,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
         if ((tid & 31) == 0) mbar_arrive(consumed + b);
         if (k >= NST) mbar_wait(freeb + b, ((k / NST) - 1) & 1); // the store of tile k-2 has left this output buffer
 
-        SmemSubOne<T> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
+        SmemSubOne<T, CPW> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
         fft_single<N, +1, false>(z, jf, p.a.tw, sm1);
         if (tid == 0 && k + NST < nk) {
             mbar_wait(consumed + b, par);
@@ -435,7 +451,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
 #pragma unroll
         for (int m = 0; m < 5; m++)
             if (m < 4 || j == 0)
-                hsub[nat_slot(jf + T * m, t)] =
+                hsub[nat_slot<CPW>(jf + T * m, t)] =
                     make_float4(z[m].x + y[m].x, z[m].y - y[m].y, z[m].y + y[m].y, y[m].x - z[m].x);
         warp_arrive_done(done + b);
 
@@ -445,8 +461,10 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
 #pragma unroll
             for (int ss = 0; ss < SUB; ss++) {
                 const uint8_t *hs = outb + b * OUT_BYTES + ss * g_::HS_SUB_BYTES;
-                tma_store_3d(&p.m_hs, hs, 2 * (col0 + 16 * ss), 0, 0);
-                tma_store_3d(&p.m_hs_row, hs + (N / 2) * 128, 2 * (col0 + 16 * ss), N / 2, 0);
+#pragma unroll
+                for (int bx = 0; bx < g_::NHBOX; bx++)
+                    tma_store_3d(&p.m_hs, hs + bx * g_::HB * RBY, 2 * (col0 + 2 * CPW * ss), bx * g_::HB, 0);
+                tma_store_3d(&p.m_hs_row, hs + (N / 2) * RBY, 2 * (col0 + 2 * CPW * ss), N / 2, 0);
             }
             bulk_commit();
             if (k >= 1) {
@@ -583,7 +601,7 @@ int launch_pipe(const PipeArgs &a)
     constexpr size_t S3 = 3 * (size_t)TILE_BYTES + SLACK;
     if (a.a.kind == P_X_KIN) return launch_pipe_kernel(k_pipe_contig<N, P_X_KIN>, S3, a);
     if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON>, S3, a);
-    if constexpr (N <= 512) {
+    {
         constexpr size_t S2H = 2 * ((size_t)TILE_BYTES + Geo<N>::SUB * Geo<N>::HS_SUB_BYTES) + SLACK;
         switch (a.a.kind) {
         case P_S_KIN: return launch_pipe_kernel(k_pipe_strided<N, P_S_KIN, +1, true>, S3, a);
