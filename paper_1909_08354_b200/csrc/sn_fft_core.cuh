@@ -183,23 +183,39 @@ __host__ __device__ constexpr int twiddle_entries(int N)
 // thread's own points j + T*(q + r*NB) = bq + r*N/R; twiddle exp(-/+ 2 pi i r (bq % NS)/(NS R)),
 // stored at tw[(r-1)*NS + (bq % NS)] so that lanes with consecutive j read consecutive entries.
 // ONE = true: only line a is transformed (b is never touched).
-template <int N, int R, int NS, int DIR, bool HILO, bool ONE, int P>
-__device__ __forceinline__ void stage_compute(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw)
+#ifndef SN_TW_PREFETCH
+#define SN_TW_PREFETCH 1 // load a stage's twiddles between the exchange's stores and loads (data registers are dead there)
+#endif
+
+template <int N, int R, int NS, bool HILO, int P>
+__device__ __forceinline__ void load_twiddles(float4 (&w)[(P / R) * (R - 1)], int j, const float4 *__restrict__ tw)
 {
     constexpr int T = N / P, NB = P / R;
 #pragma unroll
     for (int q = 0; q < NB; q++) {
+        const float4 *src = tw + ((j + T * q) & (NS - 1));
+#pragma unroll
+        for (int r = 1; r < R; r++) {
+            if (HILO) {
+                w[q * (R - 1) + r - 1] = __ldg(src + (r - 1) * NS);
+            } else {
+                const float2 h = __ldg(reinterpret_cast<const float2 *>(src + (r - 1) * NS));
+                w[q * (R - 1) + r - 1] = make_float4(h.x, h.y, 0.f, 0.f);
+            }
+        }
+    }
+}
+
+template <int N, int R, int NS, int DIR, bool HILO, bool ONE, int P>
+__device__ __forceinline__ void stage_compute(float2 (&a)[P], float2 (&b)[P], const float4 (&w)[(P / R) * (R - 1)])
+{
+    constexpr int NB = P / R;
+#pragma unroll
+    for (int q = 0; q < NB; q++) {
         if constexpr (NS > 1) {
-            const float4 *w = tw + ((j + T * q) & (NS - 1));
 #pragma unroll
             for (int r = 1; r < R; r++) {
-                float4 ww;
-                if (HILO) {
-                    ww = __ldg(w + (r - 1) * NS);
-                } else {
-                    const float2 h = __ldg(reinterpret_cast<const float2 *>(w + (r - 1) * NS));
-                    ww = make_float4(h.x, h.y, 0.f, 0.f);
-                }
+                const float4 ww = w[q * (R - 1) + r - 1];
                 a[q + r * NB] = twmul<DIR, HILO>(a[q + r * NB], ww);
                 if (!ONE) b[q + r * NB] = twmul<DIR, HILO>(b[q + r * NB], ww);
             }
@@ -237,7 +253,7 @@ __device__ __forceinline__ int comb(int tb, int K, int PM)
 // Stockham exchange after a stage (NS, R): output r of butterfly bq goes to position
 // (bq / NS) * NS * R + (bq % NS) + r * NS; afterwards thread j re-reads points j + T*m.
 template <int N, int R, int NS, class SM, int P>
-__device__ __forceinline__ void stage_exchange(float2 (&a)[P], float2 (&b)[P], int j, SM &sm)
+__device__ __forceinline__ void exchange_store(float2 (&a)[P], float2 (&b)[P], int j, SM &sm)
 {
     constexpr int T = N / P, NB = P / R;
     constexpr int WPM = ((T - 1) & ~(NS - 1)) * R | ((T - 1) & (NS - 1)); // position bits of butterfly j's base
@@ -249,10 +265,29 @@ __device__ __forceinline__ void stage_exchange(float2 (&a)[P], float2 (&b)[P], i
 #pragma unroll
         for (int r = 0; r < R; r++) sm.st_i(comb<SM>(tbw, kq + r * NS, WPM), a[q + r * NB], b[q + r * NB]);
     }
+}
+template <int N, class SM, int P>
+__device__ __forceinline__ void exchange_load(float2 (&a)[P], float2 (&b)[P], int j, SM &sm)
+{
+    constexpr int T = N / P;
     sm.sync();
     const int tbr = sm.idx(j);
 #pragma unroll
     for (int m = 0; m < P; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), a[m], b[m]);
+}
+
+// exchange after stage (NSP, RP), then stage NS = NSP * RP and everything after it
+template <int N, int NSP, int RP, int DIR, bool HILO, bool ONE, class SM, int P>
+__device__ __forceinline__ void fft_next(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
+{
+    constexpr int NS = NSP * RP, R = radix_for(N, NS);
+    float4 w[(P / R) * (R - 1)];
+    exchange_store<N, RP, NSP>(a, b, j, sm);
+    if (SN_TW_PREFETCH) load_twiddles<N, R, NS, HILO, P>(w, j, tw);
+    exchange_load<N>(a, b, j, sm);
+    if (!SN_TW_PREFETCH) load_twiddles<N, R, NS, HILO, P>(w, j, tw);
+    stage_compute<N, R, NS, DIR, HILO, ONE>(a, b, w);
+    if constexpr (NS * R < N) fft_next<N, NS, R, DIR, HILO, ONE, SM>(a, b, j, tw + NS * (R - 1), sm);
 }
 
 template <int N, int NS, int DIR, bool HILO, bool ONE, class SM, int P>
@@ -260,12 +295,11 @@ __device__ __forceinline__ void fft_stages(float2 (&a)[P], float2 (&b)[P], int j
                                            SM &sm)
 {
     static_assert(P == ppt_for(N), "points per thread");
-    constexpr int R = radix_for(N, NS);
-    stage_compute<N, R, NS, DIR, HILO, ONE>(a, b, j, tw);
-    if constexpr (NS * R < N) {
-        stage_exchange<N, R, NS, SM>(a, b, j, sm);
-        fft_stages<N, NS * R, DIR, HILO, ONE, SM>(a, b, j, tw + (NS > 1 ? NS * (R - 1) : 0), sm);
-    }
+    static_assert(NS == 1, "entry point is the first (untwiddled) stage");
+    constexpr int R = radix_for(N, 1);
+    const float4 none[(P / R) * (R - 1)] = {};
+    stage_compute<N, R, 1, DIR, HILO, ONE>(a, b, none);
+    if constexpr (R < N) fft_next<N, 1, R, DIR, HILO, ONE, SM>(a, b, j, tw, sm);
 }
 
 // Unscaled DFT of two lines.  In: thread j holds points j + T*m of each line (T = N/P, P = ppt_for(N)).
