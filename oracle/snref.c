@@ -28,6 +28,9 @@
  * Diagnostics [Q10]: norm = sum |psi|^2 dV;
  *      H = -A sum_k k^2 |psi^_k|^2 dV/prod N + (B/2) sum phi rho dV + sum F(rho) dV,
  *      F(rho) = sum_j g_j rho^(j+1)/(j+1).
+ * NEXT-1 extension (eq. (15),(16)): G may also carry g_log ln(rho) + g_pow rho^p
+ * (pressure potential) and the N phase a fixed external potential V(x) (phi_C); e_local then
+ * includes their energies sum (F(rho) + V rho) dV.
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force DFT, plane wave, free and
  * boosted Gaussian closed forms, single-mode Poisson/Helmholtz, norm conservation, Strang
@@ -66,6 +69,10 @@ typedef struct snref_ctx {
     int n_g;
     double dtau;
     int64_t cells;
+    /* NEXT-1 terms of the local potential (eq. (15),(16)): pressure potential
+     * w ln(rho) / (n w/(n-1)) rho^(n-1), and a fixed external potential phi_C(r) (eq. (11)) */
+    double g_log, rho_floor, g_pow, p_pow;
+    double *vext; /* NULL or cells doubles */
     cplx *psi;   /* state */
     cplx *work;  /* rho^ / phi^ scratch */
     int has_state;
@@ -219,18 +226,31 @@ static double ksq_at(const snref_ctx *c, int64_t idx)
     return k2;
 }
 
+/* G(rho) = sum_j g_j rho^j  +  g_log ln(rho_f)  +  g_pow rho_f^p,   rho_f = max(rho, rho_floor)
+ * (polynomial: PAPER.md:54; logarithmic and power-law terms: V_pressure of eq. (16), PAPER.md:106;
+ *  the floor is reading Q15 of DESIGN.md: the paper does not say how ln(0) is avoided) */
 static double G_of(const snref_ctx *c, double rho)
 {
     double s = 0.0, p = 1.0;
     for (int j = 0; j < c->n_g; j++) { p *= rho; s += c->g[j] * p; }
+    if (c->g_log != 0.0 || c->g_pow != 0.0) {
+        double rf = fmax(rho, c->rho_floor);
+        if (c->g_log != 0.0) s += c->g_log * log(rf);
+        if (c->g_pow != 0.0) s += c->g_pow * pow(rf, c->p_pow);
+    }
     return s;
 }
 
-/* F(rho) = sum_j g_j rho^(j+1)/(j+1), F' = G */
+/* F(rho) with F' = G: sum_j g_j rho^(j+1)/(j+1) + g_log (rho ln rho_f - rho) + g_pow rho rho_f^p/(p+1) */
 static double F_of(const snref_ctx *c, double rho)
 {
     double s = 0.0, p = rho;
     for (int j = 0; j < c->n_g; j++) { p *= rho; s += c->g[j] * p / (double)(j + 2); }
+    if (c->g_log != 0.0 || c->g_pow != 0.0) {
+        double rf = fmax(rho, c->rho_floor);
+        if (c->g_log != 0.0) s += c->g_log * (rho * log(rf) - rho);
+        if (c->g_pow != 0.0) s += c->g_pow * rho * pow(rf, c->p_pow) / (c->p_pow + 1.0);
+    }
     return s;
 }
 
@@ -256,6 +276,7 @@ int snref_create(snref_ctx **out, int ndim, const int64_t *dims, const double *L
     c->ndim = ndim;
     for (int d = 0; d < ndim; d++) { c->n[d] = dims[d]; c->L[d] = L[d]; }
     c->A = A; c->B = B; c->C = C; c->D = D; c->n_g = n_g; c->dtau = dtau; c->cells = cells;
+    c->rho_floor = 1e-30; c->p_pow = 1.0;
     for (int j = 0; j < n_g; j++) c->g[j] = g[j];
     /* Q5: C > 0 hitting a grid mode makes eq. (2) unsolvable */
     if (C > 0.0) {
@@ -271,9 +292,34 @@ int snref_create(snref_ctx **out, int ndim, const int64_t *dims, const double *L
     return SNREF_OK;
 }
 
+/* G += g_log ln(max(rho, rho_floor)) + g_pow max(rho, rho_floor)^p_pow   (eq. (16)) */
+int snref_set_local_terms(snref_ctx *c, double g_log, double rho_floor, double g_pow, double p_pow)
+{
+    if (!c) return SNREF_ERR_NULL;
+    if (!isfinite(g_log) || !isfinite(rho_floor) || !isfinite(g_pow) || !isfinite(p_pow)) return SNREF_ERR_PARAM;
+    if (rho_floor <= 0.0 || p_pow == -1.0) return SNREF_ERR_PARAM;
+    c->g_log = g_log; c->rho_floor = rho_floor; c->g_pow = g_pow; c->p_pow = p_pow;
+    return SNREF_OK;
+}
+
+/* fixed external potential V(x) (cells doubles, copied; NULL removes it): the N sub-step phase becomes
+ * exp(-i s (B phi + G(rho) + V))   (phi_C of eq. (11),(15)) */
+int snref_set_external_potential(snref_ctx *c, const double *v)
+{
+    if (!c) return SNREF_ERR_NULL;
+    free(c->vext);
+    c->vext = NULL;
+    if (!v) return SNREF_OK;
+    c->vext = (double *)malloc(sizeof(double) * (size_t)c->cells);
+    if (!c->vext) return SNREF_ERR_NOMEM;
+    memcpy(c->vext, v, sizeof(double) * (size_t)c->cells);
+    return SNREF_OK;
+}
+
 int snref_destroy(snref_ctx *c)
 {
     if (!c) return SNREF_ERR_NULL;
+    free(c->vext);
     free(c->psi);
     free(c->work);
     free(c);
@@ -351,7 +397,7 @@ static int nonlinear(snref_ctx *c, double s)
     for (int64_t i = 0; i < c->cells; i++) {
         double re = creal(c->psi[i]), im = cimag(c->psi[i]);
         double rho = re * re + im * im;
-        double th = -s * (c->B * creal(c->work[i]) + G_of(c, rho));
+        double th = -s * (c->B * creal(c->work[i]) + G_of(c, rho) + (c->vext ? c->vext[i] : 0.0));
         c->psi[i] *= cos(th) + I * sin(th);
     }
     return SNREF_OK;
@@ -398,7 +444,7 @@ int snref_diagnostics(snref_ctx *c, snref_diag *out)
         double rho = re * re + im * im;
         norm += rho;
         enl += creal(c->work[i]) * rho;
-        eloc += F_of(c, rho);
+        eloc += F_of(c, rho) + (c->vext ? c->vext[i] * rho : 0.0);
     }
     /* kinetic part in k-space, on a copy of psi */
     memcpy(c->work, c->psi, sizeof(cplx) * (size_t)c->cells);

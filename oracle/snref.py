@@ -48,6 +48,8 @@ def lib() -> ctypes.CDLL:
         L.snref_step.argtypes = [vp, ctypes.c_int64]
         L.snref_potential.argtypes = [vp, vp]
         L.snref_diagnostics.argtypes = [vp, ctypes.POINTER(SnrefDiag)]
+        L.snref_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.snref_set_external_potential.argtypes = [vp, vp]
         L.snref_num_threads.restype = ctypes.c_int
         L.snref_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -133,6 +135,20 @@ class Oracle:
 
     def set_dtau(self, dtau: float) -> None:
         _chk(lib().snref_set_dtau(self._h, float(dtau)), "snref_set_dtau")
+
+    def set_local_terms(self, g_log: float = 0.0, rho_floor: float = 1e-30, g_pow: float = 0.0,
+                        p_pow: float = 1.0) -> None:
+        """G(rho) += g_log ln(max(rho, rho_floor)) + g_pow max(rho, rho_floor)**p_pow (eq. (16))."""
+        _chk(lib().snref_set_local_terms(self._h, g_log, rho_floor, g_pow, p_pow), "snref_set_local_terms")
+
+    def set_external_potential(self, v) -> None:
+        """Fixed external potential V(x) added to the N sub-step phase (phi_C of eq. (15)); None removes it."""
+        if v is None:
+            _chk(lib().snref_set_external_potential(self._h, None), "snref_set_external_potential")
+            return
+        a = np.ascontiguousarray(v, dtype=np.float64)
+        assert a.shape == self.dims, (a.shape, self.dims)
+        _chk(lib().snref_set_external_potential(self._h, a.ctypes.data), "snref_set_external_potential")
 
     def potential(self) -> np.ndarray:
         out = np.empty(self.dims, dtype=np.float64)

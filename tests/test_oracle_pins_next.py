@@ -1,0 +1,135 @@
+"""Pins for the oracle's NEXT-1 terms (eq. (15),(16)) -- CPU only.
+
+  W1  plane wave: exact solution of the full system for ANY local G, so it fixes the sign and the
+      factor of the logarithmic and power-law terms of V_pressure (eq. (16)) and of a uniform V.
+  W2  harmonic oscillator: with V = omega^2 r^2/2 and A = -1/2 the Gaussian ground state only
+      acquires the phase exp(-i d omega tau/2); a displaced Gaussian (coherent state) moves as
+      x0 cos(omega tau).  Fixes the sign of V in the N sub-step.
+  W3  gausson of the logarithmic Schroedinger equation: i psi_t = -1/2 lap psi + g_log ln(rho) psi
+      has the stationary Gaussian a exp(-r^2/(2 sigma^2)) exp(-i E tau) when g_log = -1/(2 sigma^2),
+      E = d/(2 sigma^2) + 2 g_log ln(a) (insert and compare powers of r).
+  W4  energy with the new terms: closed forms for a Gaussian (F_log, F_pow, V rho).
+None of these re-types the oracle: each expected value is a closed form evaluated here in numpy.
+"""
+import numpy as np
+import pytest
+
+from oracle.snref import Oracle
+from paper_1909_08354_b200 import inputs
+
+
+def rel(a, b):
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(np.asarray(b).ravel()))
+
+
+def grid(dims, L):
+    return np.meshgrid(*[inputs.coords(n, L) for n in dims], indexing="ij")
+
+
+@pytest.mark.parametrize("dims", [(16, 24), (8, 12, 16)])
+def test_w1_plane_wave_with_log_and_power_terms(dims):
+    L, A, B, C, D = 10.0, -0.7, 1.3, -1.0, 0.9
+    g, g_log, g_pow, p = (0.2,), 0.31, -0.45, 2.0 / 3.0
+    amp, dtau, n = 0.8, 7e-3, 9
+    X = grid(dims, L)
+    q = [2 * np.pi / L * m for m in (2, -1, 3)[:len(dims)]]
+    psi0 = amp * np.exp(1j * sum(qa * xa for qa, xa in zip(q, X)))
+    v0 = 0.37                                             # uniform external potential: a pure phase rate
+    o = Oracle(dims, L, A, B, C, D, g, dtau)
+    o.set_local_terms(g_log=g_log, rho_floor=1e-12, g_pow=g_pow, p_pow=p)
+    o.set_external_potential(np.full(dims, v0))
+    o.set_state(psi0)
+    o.step(n)
+    rho = amp ** 2
+    G = g[0] * rho + g_log * np.log(rho) + g_pow * rho ** p
+    rate = A * sum(qa * qa for qa in q) - B * D * rho / C - G - v0
+    assert rel(o.get_state(), psi0 * np.exp(1j * rate * n * dtau)) < 1e-12
+    o.close()
+
+
+def test_w2_harmonic_ground_state_and_coherent_state():
+    dims, L, w = (64, 64), 16.0, 1.5
+    X, Y = grid(dims, L)
+    V = 0.5 * w * w * (X * X + Y * Y)
+    g0 = np.sqrt(w / np.pi) * np.exp(-0.5 * w * (X * X + Y * Y))
+    errs = []
+    for dtau in (8e-3, 4e-3):
+        o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), dtau)
+        o.set_external_potential(V)
+        o.set_state(g0)
+        n = int(round(0.8 / dtau))
+        o.step(n)
+        errs.append(rel(o.get_state(), g0 * np.exp(-1j * w * n * dtau)))   # d*omega/2 with d = 2
+        o.close()
+    assert errs[1] < 1e-5 and 3.7 < errs[0] / errs[1] < 4.3               # O(dtau^2) splitting error only
+    # coherent state: centre follows x0 cos(omega tau), norm 1
+    x0, dtau = 1.2, 2e-3
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), dtau)
+    o.set_external_potential(V)
+    o.set_state(np.sqrt(w / np.pi) * np.exp(-0.5 * w * ((X - x0) ** 2 + Y * Y)))
+    n = 500
+    o.step(n)
+    rho = np.abs(o.get_state()) ** 2
+    dV = (L / 64) ** 2
+    assert abs(rho.sum() * dV - 1.0) < 1e-10
+    assert abs((rho * X).sum() * dV - x0 * np.cos(w * n * dtau)) < 1e-5
+    assert abs((rho * Y).sum() * dV) < 1e-10
+    o.close()
+
+
+@pytest.mark.parametrize("dims,L", [((96, 96), 24.0), ((32, 32, 32), 20.0)])
+def test_w3_gausson_of_the_logarithmic_equation(dims, L):
+    d, sigma, a = len(dims), 1.6, 0.9
+    g_log = -1.0 / (2 * sigma * sigma)
+    E = d / (2 * sigma * sigma) + 2 * g_log * np.log(a)
+    X = grid(dims, L)
+    r2 = sum(x * x for x in X)
+    psi0 = a * np.exp(-r2 / (2 * sigma * sigma))
+    errs = []
+    for dtau in (2e-2, 1e-2):
+        o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), dtau)
+        o.set_local_terms(g_log=g_log, rho_floor=1e-300)
+        o.set_state(psi0)
+        n = int(round(1.0 / dtau))
+        o.step(n)
+        errs.append(rel(o.get_state(), psi0 * np.exp(-1j * E * n * dtau)))
+        o.close()
+    assert errs[1] < 5e-5 and 3.6 < errs[0] / errs[1] < 4.4
+
+
+def test_w3_sign_of_log_term_matters():
+    dims, L, sigma = (64, 64), 20.0, 1.6
+    X, Y = grid(dims, L)
+    psi0 = 0.9 * np.exp(-(X * X + Y * Y) / (2 * sigma * sigma))
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)
+    o.set_local_terms(g_log=+1.0 / (2 * sigma * sigma), rho_floor=1e-300)   # wrong sign: the packet spreads
+    o.set_state(psi0)
+    o.step(100)
+    assert np.abs(o.get_state()).max() < 0.9 * 0.9   # the stationary gausson keeps 0.9
+    o.close()
+
+
+def test_w4_energy_closed_forms_and_conservation():
+    dims, L, s = (96, 96), 24.0, 1.3
+    X, Y = grid(dims, L)
+    r2 = X * X + Y * Y
+    a = 0.7
+    psi0 = a * np.exp(-r2 / (2 * s * s))                   # rho = a^2 exp(-r^2/s^2)
+    w, g_log, g_pow, p = 0.8, 0.25, 0.6, 1.5
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 2e-3)
+    o.set_local_terms(g_log=g_log, rho_floor=1e-300, g_pow=g_pow, p_pow=p)
+    o.set_external_potential(0.5 * w * w * r2)
+    o.set_state(psi0)
+    d0 = o.diagnostics()
+    M = np.pi * a * a * s * s                              # int rho
+    # int rho ln rho = M (2 ln a - 1) [int r^2/s^2 rho = M];  int rho^(p+1) = pi a^(2p+2) s^2/(p+1);  int r^2 rho = M s^2
+    e_log = g_log * (M * (2 * np.log(a) - 1.0) - M)
+    e_pow = g_pow * np.pi * a ** (2 * p + 2) * s * s / (p + 1) / (p + 1)
+    e_ext = 0.5 * w * w * M * s * s
+    assert abs(d0["e_local"] - (e_log + e_pow + e_ext)) < 1e-9 * abs(e_ext)
+    assert abs(d0["e_kin"] - 0.5 * M / (s * s)) < 1e-9     # -A int |grad psi|^2 = (1/2) M/s^2 in 2D
+    o.step(400)
+    d1 = o.diagnostics()
+    assert abs(d1["e_total"] - d0["e_total"]) < 2e-6 * abs(d0["e_total"])   # O(dtau^2), bounded
+    assert abs(d1["norm"] - d0["norm"]) < 1e-12 * d0["norm"]
+    o.close()
