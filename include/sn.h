@@ -86,6 +86,17 @@ int sn_diagnostics(sn_ctx *ctx, sn_diag *out);
 /* Replace dtau (rebuilds the kinetic phase tables). */
 int sn_set_dtau(sn_ctx *ctx, double dtau);
 
+/* ---- NEXT-1 terms of the local potential (eq. (15),(16)) ----
+ * sn_set_local_terms: G(rho) += g_log ln(rho_f) + g_pow rho_f^p_pow, rho_f = max(rho, rho_floor) -- the pressure
+ *   potential V_pressure = w ln(rho) (n = 1) or (n w/(n-1)) rho^(n-1) of eq. (16).  rho_floor > 0 (reading Q15:
+ *   the paper does not say how ln(0) is avoided), p_pow != -1.  g_log = g_pow = 0 switches the terms off.
+ * sn_set_external_potential: a fixed real potential V(x) (float32, prod(dims) values, layout of psi; host or
+ *   device pointer, copied into the workspace) enters the N sub-step as exp(-i s (B phi + G(rho) + V)) -- phi_C
+ *   of eq. (11),(15).  NULL removes it.  With V set the axis-0 nonlinear pass runs the first-path kernel.
+ * Both rebuild the nonlinear-phase coefficients; e_local of sn_diagnostics then includes sum (F(rho) + V rho) dV. */
+int sn_set_local_terms(sn_ctx *ctx, double g_log, double rho_floor, double g_pow, double p_pow);
+int sn_set_external_potential(sn_ctx *ctx, const float *v, int src_on_device);
+
 int sn_destroy(sn_ctx *ctx);
 
 /* Text for an error code; for SN_ERR_CUDA the last CUDA error string seen by this thread. */

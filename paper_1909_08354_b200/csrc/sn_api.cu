@@ -50,7 +50,7 @@ struct Layout {
     int ndim;
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
-    size_t off_psi, off_hs, off_phi, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
+    size_t off_psi, off_hs, off_phi, off_vext, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
 };
 
 bool make_layout(int ndim, const int64_t *dims, Layout &L)
@@ -72,6 +72,7 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L)
     L.off_psi = o; o = align256(o + (size_t)L.cells * 8);
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
     L.off_phi = o; o = align256(o + (size_t)L.cells * 4);
+    L.off_vext = o; o = align256(o + (size_t)L.cells * 4);
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
         L.off_ph_full[d] = o; o = align256(o + (size_t)L.n[d] * 16);
@@ -107,6 +108,9 @@ struct sn_ctx {
     Layout lay;
     double L[3];
     double A, B, C, D, g[4], dtau;
+    double g_log, rho_floor, g_pow, p_pow; // NEXT-1 local terms (eq. (16)); off when g_log == g_pow == 0
+    bool has_vext;                          // external potential set (eq. (15) phi_C)
+    float *vext;
     int n_g;
     char *ws;
     cudaStream_t stream;
@@ -262,7 +266,8 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         const bool strided = a.kind == snk::P_S_FFT || a.kind == snk::P_S_KIN;
         const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C;
         const int axis = strided ? a.axis : 0;
-        const bool maps = (strided || haxis) ? c->m_ok[axis] : true;
+        const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
+                          !(a.kind == snk::P_H_NLKIN && c->has_vext); // the external potential is read by the first-path kernel only
         if (maps && (N & (N - 1)) == 0 && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
@@ -333,6 +338,14 @@ int upload_phase_tables(sn_ctx *c)
         SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vectors die at the end of this iteration
     }
     c->nl.hb = (float)(-0.5 * c->dtau * c->B);
+    c->nl.flags = ((c->g_log != 0.0 || c->g_pow != 0.0) ? 1 : 0) | (c->has_vext ? 2 : 0);
+    c->nl.hlog = (float)(-0.5 * c->dtau * c->g_log);
+    c->nl.hpow = (float)(-0.5 * c->dtau * c->g_pow);
+    c->nl.floor_ = (float)c->rho_floor;
+    c->nl.ppow = (float)c->p_pow;
+    c->nl.hv = (float)(-0.5 * c->dtau);
+    c->nl.flog = (float)c->g_log;
+    c->nl.fpow = (float)(c->g_pow / (c->p_pow + 1.0));
     for (int j = 0; j < 4; j++) {
         c->nl.hg[j] = j < c->n_g ? (float)(-0.5 * c->dtau * c->g[j]) : 0.f;
         c->nl.fg[j] = j < c->n_g ? (float)(c->g[j] / (double)(j + 2)) : 0.f;
@@ -398,6 +411,7 @@ PassArgs base_args(const sn_ctx *c)
     a.C = (float)c->C;
     a.nl = c->nl;
     a.diag = c->diag;
+    a.vext = c->has_vext ? c->vext : nullptr;
     return a;
 }
 
@@ -557,6 +571,8 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
     c->psi = reinterpret_cast<float2 *>(c->ws + l.off_psi);
     c->hs = reinterpret_cast<float2 *>(c->ws + l.off_hs);
     c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
+    c->vext = reinterpret_cast<float *>(c->ws + l.off_vext);
+    c->rho_floor = 1e-30; c->p_pow = 1.0;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
         c->ph_full[d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph_full[d]);
@@ -613,6 +629,32 @@ int sn_set_dtau(sn_ctx *c, double dtau)
     const int rc = upload_phase_tables(c);
     if (rc != SN_OK) c->dtau = old;
     return rc;
+}
+
+int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, double p_pow)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!std::isfinite(g_log) || !std::isfinite(rho_floor) || !std::isfinite(g_pow) || !std::isfinite(p_pow))
+        return SN_ERR_PARAM;
+    if (rho_floor <= 0.0 || p_pow == -1.0) return SN_ERR_PARAM;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c);
+    c->g_log = g_log; c->rho_floor = rho_floor; c->g_pow = g_pow; c->p_pow = p_pow;
+    return upload_phase_tables(c);
+}
+
+int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
+{
+    if (!c) return SN_ERR_NULL;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c);
+    if (v) {
+        SN_CUDA(cudaMemcpyAsync(c->vext, v, (size_t)c->lay.cells * 4,
+                                src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    c->has_vext = v != nullptr;
+    return upload_phase_tables(c);
 }
 
 int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)

@@ -197,12 +197,25 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
             const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
             const float r[4] = {abs2(lo2(u)), abs2(hi2(u)), abs2(lo2(v)), abs2(hi2(v))};
             const float ph[4] = {fa[m].x, fa[m].y, fb[m].x, fb[m].y};
+            float ve[4] = {0.f, 0.f, 0.f, 0.f};
+            if (p.nl.flags & 2) {
+                const float2 *v2 = reinterpret_cast<const float2 *>(p.vext) + col4 + (long long)(j + T * m) * rs4;
+                const float2 e0 = __ldg(v2 + t), e1 = __ldg(v2 + CP + t);
+                ve[0] = e0.x; ve[1] = e0.y; ve[2] = e1.x; ve[3] = e1.y;
+            }
 #pragma unroll
             for (int c = 0; c < 4; c++) {
                 s_rho += r[c];
                 s_pr = fmaf(ph[c], r[c], s_pr);
                 const float f = fmaf(r[c], fmaf(r[c], fmaf(r[c], p.nl.fg[3], p.nl.fg[2]), p.nl.fg[1]), p.nl.fg[0]);
                 s_f = fmaf(r[c] * r[c], f, s_f);
+                if (p.nl.flags) { // F_log = g_log (rho ln rho_f - rho), F_pow = g_pow rho rho_f^p/(p+1), V rho
+                    const float rf = fmaxf(r[c], p.nl.floor_);
+                    float e = ve[c];
+                    if (p.nl.flog != 0.f) e += p.nl.flog * (logf(rf) - 1.f);
+                    if (p.nl.fpow != 0.f) e = fmaf(p.nl.fpow, powf(rf, p.nl.ppow), e);
+                    s_f = fmaf(r[c], e, s_f);
+                }
             }
         }
         double v[3] = {(double)s_rho, (double)s_pr, (double)s_f};
@@ -219,8 +232,11 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
         for (int m = 0; m < P; m++) {
             const float4 v = g4[(long long)(j + T * m) * rs4];
             const float2 ph = half == 0 ? fa[m] : fb[m];
-            a[m] = nl_phase(lo2(v), ph.x, p.nl);
-            b[m] = nl_phase(hi2(v), ph.y, p.nl);
+            float2 ve = make_float2(0.f, 0.f);
+            if (p.nl.flags & 2)
+                ve = __ldg(reinterpret_cast<const float2 *>(p.vext) + col4 + half * CP + t + (long long)(j + T * m) * rs4);
+            a[m] = nl_phase(lo2(v), ph.x, p.nl, ve.x);
+            b[m] = nl_phase(hi2(v), ph.y, p.nl, ve.y);
         }
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
 #pragma unroll

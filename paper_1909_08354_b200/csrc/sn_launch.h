@@ -26,6 +26,12 @@ struct NLParams {
     float hb;
     float hg[4];
     float fg[4]; // F(rho) = rho^2 (fg[0] + rho (fg[1] + ...)), fg[j] = g_j/(j+2)   (diagnostics)
+    // NEXT-1 terms (eq. (15),(16) PAPER.md:102-107), all zero / off by default (flags == 0):
+    int flags;        // bit 0: logarithmic / power-law terms present; bit 1: external potential present
+    float hlog, hpow; // half-angle coefficients -dtau/2 * g_log, -dtau/2 * g_pow
+    float floor_, ppow; // rho_f = max(rho, floor_); rho_f^ppow
+    float hv;         // -dtau/2 (multiplies the external potential)
+    float flog, fpow; // diagnostics: g_log, g_pow/(ppow+1)
 };
 
 struct PassArgs {
@@ -49,6 +55,7 @@ struct PassArgs {
     float pscale;           // P_X_POISSON: D * 0.5 / prod(N)   (0.5 from the packed r2c)
     NLParams nl;
     float *phi_out;         // DEVICE: P_H_POT
+    const float *vext;      // DEVICE: external potential (same layout as psi, float) or nullptr
     double *diag;           // DEVICE: accumulators
     cudaStream_t stream;
 };

@@ -23,7 +23,7 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG")
@@ -71,6 +71,8 @@ def lib() -> ctypes.CDLL:
         L.sn_profile_read.argtypes = [vp, dp, i64p, ctypes.c_int]
         L.sn_debug_fft.argtypes = [vp, ctypes.c_int]
         L.sn_debug_potential.argtypes = [vp, vp, ctypes.c_int]
+        L.sn_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
+        L.sn_set_external_potential.argtypes = [vp, vp, ctypes.c_int]
         _lib = L
     return _lib
 
@@ -168,6 +170,27 @@ class Simulation:
 
     def set_dtau(self, dtau: float) -> None:
         _chk(lib().sn_set_dtau(self._h, float(dtau)), "sn_set_dtau")
+
+    def set_local_terms(self, g_log: float = 0.0, rho_floor: float = 1e-30, g_pow: float = 0.0,
+                        p_pow: float = 1.0) -> None:
+        """G(rho) += g_log ln(max(rho, rho_floor)) + g_pow max(rho, rho_floor)**p_pow (eq. (16))."""
+        _chk(lib().sn_set_local_terms(self._h, float(g_log), float(rho_floor), float(g_pow), float(p_pow)),
+             "sn_set_local_terms")
+
+    def set_external_potential(self, v) -> None:
+        """Fixed external potential V(x): numpy float32 array (host), torch float32 CUDA tensor, or None."""
+        if v is None:
+            _chk(lib().sn_set_external_potential(self._h, None, 0), "sn_set_external_potential")
+        elif isinstance(v, np.ndarray):
+            a = np.ascontiguousarray(v, dtype=np.float32)
+            assert a.shape == self.dims, (a.shape, self.dims)
+            _chk(lib().sn_set_external_potential(self._h, ctypes.c_void_p(a.ctypes.data), 0),
+                 "sn_set_external_potential")
+        else:
+            import torch
+            assert v.dtype == torch.float32 and v.is_contiguous() and tuple(v.shape) == self.dims
+            _chk(lib().sn_set_external_potential(self._h, ctypes.c_void_p(v.data_ptr()), 1 if v.is_cuda else 0),
+                 "sn_set_external_potential")
 
     def diagnostics(self) -> dict:
         d = SnDiag()
