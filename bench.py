@@ -176,6 +176,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--extras", action="store_true",
+                    help="NEXT-1 row: also run with the pressure potential 0.02 ln(rho) (eq. (16)) and the "
+                         "phi_C table of eq. (11) as external potential (DESIGN.md section 9)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -213,6 +216,15 @@ def main():
 
     stream = torch.cuda.current_stream()
     sim = sn.Simulation.from_config(cfg, device=dev, stream=stream)
+    if args.extras:
+        # eq. (16) n = 1: V_pressure = w ln(rho), w = 0.02; eq. (11): phi_C = ln[1 - (r0/(r + r0))^lambda], lambda = 1,
+        # r0 = 2, radius softened to sqrt(r^2 + 1) (the grid has a point at r = 0)
+        ax = [inputs.coords(n, cfg.L) for n in cfg.dims]
+        r2 = sum(np.square(a).reshape([-1 if i == k else 1 for i in range(nd)]) for k, a in enumerate(ax))
+        V = np.log(1.0 - 2.0 / (np.sqrt(r2 + 1.0) + 2.0)).astype(np.float32)
+        sim.set_local_terms(0.02, 1e-12, 0.0, 1.0)
+        sim.set_external_potential(V)
+        del V, r2
     sim.set_state(dev_in)
     sim.step(W)                                         # untimed warm-up steps
     barrier()
@@ -260,7 +272,7 @@ def main():
         hs_frac = (cfg.dims[0] // 2 + 1) / (cfg.dims[0] / 2)   # exact half-spectrum factor on the 4-byte terms
         bpc = PASS_BYTES_PER_CELL[dom]
         if dom == "H_NLKIN":
-            bpc = 16.0 + 4.0 * hs_frac
+            bpc = 16.0 + 4.0 * hs_frac + (4.0 if args.extras else 0.0)   # + the external potential table
         elif dom == "H_R2C":
             bpc = 8.0 + 4.0 * hs_frac
         elif dom in ("S_FFT", "X_POISSON"):
@@ -270,7 +282,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
-            "config": {"workload": f"{cfg.name}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
+            "config": {"workload": f"{cfg.name}{'+next1(0.02 ln rho, phi_C table)' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
                                    f"B={cfg.B}, C={cfg.C}, D={cfg.D:.6g}, g={list(cfg.g)}, dtau={cfg.dtau}",
                        "dims": list(cfg.dims), "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
@@ -282,7 +294,7 @@ def main():
             "roofline": {
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" else None,
+                "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras else None,
                 "traffic_source": "ncu --set full dram bytes per launch, profiles/r01b_ncu_full_C5_512.md",
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,

@@ -110,6 +110,7 @@ struct sn_ctx {
     double A, B, C, D, g[4], dtau;
     double g_log, rho_floor, g_pow, p_pow; // NEXT-1 local terms (eq. (16)); off when g_log == g_pow == 0
     bool has_vext;                          // external potential set (eq. (15) phi_C)
+    bool v_in_xkin;                         // its phase is applied by the pipelined contiguous-axis kinetic pass
     float *vext;
     int n_g;
     char *ws;
@@ -267,7 +268,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C;
         const int axis = strided ? a.axis : 0;
         const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
-                          !(a.kind == snk::P_H_NLKIN && c->has_vext); // the external potential is read by the first-path kernel only
+                          !(a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin); // then the first-path kernel reads V
         if (maps && (N & (N - 1)) == 0 && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
@@ -428,7 +429,8 @@ void set_axis_geometry(const sn_ctx *c, PassArgs &a, int axis, int64_t n0)
 }
 
 // one kinetic sweep over all axes; with_nl fuses the nonlinear phase (and the c2r of phi^) into axis 0
-int kinetic_sweep(sn_ctx *c, bool half, bool with_nl)
+// before_n: the sweep is followed by an N sub-step (the external-potential phase may ride on its last pass)
+int kinetic_sweep(sn_ctx *c, bool half, bool with_nl, bool before_n)
 {
     const Layout &l = c->lay;
     int rc;
@@ -438,11 +440,15 @@ int kinetic_sweep(sn_ctx *c, bool half, bool with_nl)
         a.hs = c->hs;
         a.tw = c->tw[d];
         a.phase = half ? c->ph_half[d] : c->ph_full[d];
+        if (c->v_in_xkin) a.nl.flags &= ~2; // the axis-0 pass leaves V to the contiguous pass
+        a.vext = nullptr;
         if (d == l.ndim - 1) {
             a.kind = snk::P_X_KIN;
             a.nlines = (int)(l.cells / l.nx);
+            if (c->v_in_xkin && before_n) a.vext = c->vext;
         } else {
             a.kind = (d == 0 && with_nl) ? snk::P_H_NLKIN : snk::P_S_KIN;
+            if (a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin) a.vext = c->vext;
             set_axis_geometry(c, a, d, l.n[0]);
         }
         if ((rc = run_pass(c, (int)l.n[d], a))) return rc;
@@ -493,7 +499,7 @@ int build_step_graph(sn_ctx *c)
     SN_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->cap_stream;
     int rc = potential_spectrum(c);
-    if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/false, /*with_nl=*/true);
+    if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/false, /*with_nl=*/true, /*before_n=*/true);
     c->stream = user;
     cudaGraph_t g = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
@@ -654,6 +660,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
     c->has_vext = v != nullptr;
+    c->v_in_xkin = c->has_vext && c->use_pipe && (c->lay.nx & (c->lay.nx - 1)) == 0;
     return upload_phase_tables(c);
 }
 
@@ -684,7 +691,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
     // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
-    int rc = kinetic_sweep(c, /*half=*/true, /*with_nl=*/false);
+    int rc = kinetic_sweep(c, /*half=*/true, /*with_nl=*/false, /*before_n=*/true);
     int64_t i = 1;
     if (rc == SN_OK && c->use_graph && !c->profiling && nsteps >= 4) {
         if (!c->step_graph) rc = build_step_graph(c);
@@ -695,7 +702,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     }
     for (; rc == SN_OK && i <= nsteps; i++) {
         rc = potential_spectrum(c);
-        if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/i == nsteps, /*with_nl=*/true);
+        if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/i == nsteps, /*with_nl=*/true, /*before_n=*/i < nsteps);
     }
     return rc;
 }

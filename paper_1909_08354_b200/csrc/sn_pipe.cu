@@ -262,7 +262,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
 // that tile k was stored from is reloaded with tile k+2 from a point INSIDE tile k+1's compute, so
 // the issuer never waits for its own store to drain.
 
-template <int N, int MODE>
+template <int N, int MODE, bool EXTRA>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
@@ -341,8 +341,8 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
 #pragma unroll
             for (int m = 0; m < 8; m++) {
                 const float4 v = mine[CPW * T * m];
-                a[m] = nl_phase(lo2(v), z[m].x, p.a.nl);
-                c[m] = nl_phase(hi2(v), z[m].y, p.a.nl);
+                a[m] = nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl);
+                c[m] = nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl);
             }
             fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
             apply_phase<T>(a, c, jf, p.a.phase);
@@ -490,13 +490,18 @@ struct GeoX {
     static_assert(LINES * N * 8 == TILE_BYTES, "tile size");
 };
 
-template <int N, int MODE>
+// VEXT (P_X_KIN only): this is the last kinetic pass before an N sub-step, so psi is back in real space when
+// the inverse transform ends: the phase exp(-i dtau V(x)) of a fixed external potential (phi_C of eq. (15),
+// PAPER.md:102) commutes with the nonlinear phase and is applied here, where V arrives as contiguous lines
+// (a second bulk copy per tile: 2 stages of 64 KB psi + 32 KB V instead of 3 stages of psi).
+template <int N, int MODE, bool VEXT>
 __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_constant__ PipeArgs p)
 {
-    constexpr int T = GeoX<N>::T, LINES = GeoX<N>::LINES, NST = 3;
+    constexpr int T = GeoX<N>::T, LINES = GeoX<N>::LINES, NST = VEXT ? 2 : 3;
+    constexpr int STAGE_BYTES = VEXT ? TILE_BYTES + TILE_BYTES / 2 : TILE_BYTES;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
-    uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * TILE_BYTES), *done = full + NST;
+    uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
     const int tid = threadIdx.x, g = tid / T, j = tid % T;
 
     if (tid == 0) {
@@ -518,8 +523,9 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
         long long line0;
         const uint32_t bytes = (uint32_t)tile_lines(k, line0) * N * 8;
         const int b = k % NST;
-        mbar_arrive_expect_tx(full + b, bytes);
-        bulk_load_1d(base + b * TILE_BYTES, p.a.data + line0 * N, bytes, full + b);
+        mbar_arrive_expect_tx(full + b, VEXT ? bytes + bytes / 2 : bytes);
+        bulk_load_1d(base + b * STAGE_BYTES, p.a.data + line0 * N, bytes, full + b);
+        if (VEXT) bulk_load_1d(base + b * STAGE_BYTES + TILE_BYTES, p.a.vext + line0 * N, bytes / 2, full + b);
     };
     if (tid == 0) {
         if (nk > 0) issue_load(0);
@@ -531,7 +537,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
         const uint32_t par = (k / NST) & 1;
         long long line0;
         const int nl = tile_lines(k, line0);
-        float4 *grp = reinterpret_cast<float4 *>(base + b * TILE_BYTES) + g * N; // two lines = N float4
+        float4 *grp = reinterpret_cast<float4 *>(base + b * STAGE_BYTES) + g * N; // two lines = N float4
         float2 *la = reinterpret_cast<float2 *>(grp), *lb = la + N;
         SmemLine<T> sm{grp, 1 + g, T == PIPE_THREADS};
         mbar_wait(full + b, par);
@@ -548,6 +554,14 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
                 fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
                 apply_phase<T>(a, c, jf, p.a.phase);
                 fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
+                if (VEXT) {
+                    const float *va = reinterpret_cast<const float *>(base + b * STAGE_BYTES + TILE_BYTES) + 2 * g * N;
+#pragma unroll
+                    for (int m = 0; m < 8; m++) {
+                        a[m] = rotate_half_angle(a[m], p.a.nl.hv * va[ji + T * m]);
+                        c[m] = rotate_half_angle(c[m], p.a.nl.hv * va[N + ji + T * m]);
+                    }
+                }
             } else { // P_X_POISSON
                 fft_pair<N, +1, false>(a, c, jf, p.a.tw, sm);
                 const float ka = __ldg(p.a.kother2 + line0 + 2 * g), kb = __ldg(p.a.kother2 + line0 + 2 * g + 1);
@@ -572,10 +586,11 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
 
         if (tid == 0) {
             mbar_wait(done + b, par);
-            bulk_store_1d(p.a.data + line0 * N, base + b * TILE_BYTES, (uint32_t)nl * N * 8);
+            bulk_store_1d(p.a.data + line0 * N, base + b * STAGE_BYTES, (uint32_t)nl * N * 8);
             bulk_commit();
             if (k + 2 < nk) {
-                bulk_wait_read<1>();
+                if (NST == 3) bulk_wait_read<1>(); // tile k+2 goes where tile k-1 was stored from
+                else bulk_wait_read<0>();          // two stages: tile k+2 reuses this stage
                 issue_load(k + 2);
             }
         }
@@ -599,8 +614,10 @@ int launch_pipe(const PipeArgs &a)
 {
     constexpr size_t SLACK = 1024 + 64; // alignment of the ring + the mbarriers
     constexpr size_t S3 = 3 * (size_t)TILE_BYTES + SLACK;
-    if (a.a.kind == P_X_KIN) return launch_pipe_kernel(k_pipe_contig<N, P_X_KIN>, S3, a);
-    if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON>, S3, a);
+    if (a.a.kind == P_X_KIN)
+        return a.a.vext ? launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, true>, S3, a)
+                        : launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, false>, S3, a);
+    if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON, false>, S3, a);
     {
         constexpr size_t S2H = 2 * ((size_t)TILE_BYTES + Geo<N>::SUB * Geo<N>::HS_SUB_BYTES) + SLACK;
         switch (a.a.kind) {
@@ -611,7 +628,9 @@ int launch_pipe(const PipeArgs &a)
                                 : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, false>, S3, a);
             return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, true>, S3, a)
                             : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, false>, S3, a);
-        case P_H_NLKIN: return launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN>, S2H, a);
+        case P_H_NLKIN:
+            return (a.a.nl.flags & 1) ? launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, true>, S2H, a)
+                                      : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, S2H, a);
         case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, S2H, a);
         default: break;
         }
