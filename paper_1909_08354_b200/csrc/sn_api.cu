@@ -219,19 +219,17 @@ int make_tensor_maps(sn_ctx *c)
     const Layout &l = c->lay;
     int rc;
     c->m_ok[0] = c->m_ok[1] = false;
-    auto pow2 = [](int64_t n) { return (n & (n - 1)) == 0; };
-    auto cpw_of = [](int64_t n) { const int g = (int)(4096 / n); return g < 8 ? g : 8; }; // column pairs per box row
-    if (pow2(l.n[0]) && l.cols0 % (2 * (4096 / l.n[0])) == 0) {
-        const int n0 = (int)l.n[0], cpw = cpw_of(n0);
-        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, n0 < 256 ? n0 : 256, cpw))) return rc;
-        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, n0 / 2 < 256 ? n0 / 2 : 256, cpw))) return rc;
+    if (l.cols0 % (2 * snk::pipe_groups((int)l.n[0])) == 0) {
+        const int n0 = (int)l.n[0], cpw = snk::pipe_cpw(n0);
+        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, snk::pipe_box_rows(n0 / 2), cpw))) return rc;
         if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
         c->m_ok[0] = true;
     }
-    if (l.ndim == 3 && pow2(l.n[1]) && l.n[2] % (2 * (4096 / l.n[1])) == 0) {
-        const int n1 = (int)l.n[1], cpw = cpw_of(n1);
-        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], n1 < 256 ? n1 : 256, cpw))) return rc;
-        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], n1 < 256 ? n1 : 256, cpw))) return rc;
+    if (l.ndim == 3 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
+        const int n1 = (int)l.n[1], cpw = snk::pipe_cpw(n1);
+        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
         c->m_ok[1] = true;
     }
     return SN_OK;
@@ -269,26 +267,29 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         const int axis = strided ? a.axis : 0;
         const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
                           !(a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin); // then the first-path kernel reads V
-        if (maps && (N & (N - 1)) == 0 && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
+        if (maps && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
             pa.a = a;
             if (strided) {
                 pa.m_data = axis == 1 ? (a.data == c->hs ? c->m_hs1 : c->m_psi[1]) : c->m_psi[0];
-                pa.tiles_per_outer = a.ncols / (2 * (4096 / N));
+                pa.tiles_per_outer = a.ncols / (2 * snk::pipe_groups(N));
                 pa.n_tiles = pa.tiles_per_outer * a.n_outer;
             } else if (haxis) {
                 pa.m_data = c->m_psi[0];
                 pa.m_hs = c->m_hs0;
                 pa.m_hs_row = c->m_hs0_row;
-                pa.tiles_per_outer = a.ncols / (2 * (4096 / N));
+                pa.tiles_per_outer = a.ncols / (2 * snk::pipe_groups(N));
                 pa.n_tiles = pa.tiles_per_outer;
             } else {
-                const int lines = 2 * (4096 / N);
+                const int lines = 2 * snk::pipe_groups(N);
                 pa.n_tiles = (int)((a.nlines + lines - 1) / lines);
             }
             pa.grid = pa.n_tiles < c->sm_count ? pa.n_tiles : c->sm_count;
             switch (N) {
+            case 96: rc = snk::launch_pipe<96>(pa); break;
+            case 384: rc = snk::launch_pipe<384>(pa); break;
+            case 1536: rc = snk::launch_pipe<1536>(pa); break;
             case 64: rc = snk::launch_pipe<64>(pa); break;
             case 128: rc = snk::launch_pipe<128>(pa); break;
             case 256: rc = snk::launch_pipe<256>(pa); break;
@@ -660,7 +661,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
     c->has_vext = v != nullptr;
-    c->v_in_xkin = c->has_vext && c->use_pipe && (c->lay.nx & (c->lay.nx - 1)) == 0;
+    c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0; // the pipelined contiguous pass serves 2^n only
     return upload_phase_tables(c);
 }
 

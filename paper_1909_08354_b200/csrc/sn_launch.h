@@ -81,14 +81,30 @@ struct PipeArgs {
 };
 
 // true when launch_pipe<N> serves this kind/geometry (otherwise use launch_pass<N>)
+// geometry of the pipelined kernels, shared by the scheduler (tensor maps, tile counts) and sn_pipe.cu:
+// 8 points per thread and 512 threads for N = 2^n; 12 points per thread and 256 threads for N = 6*4^a
+__host__ __device__ constexpr int pipe_ppt(int N) { return N % 3 == 0 ? 12 : 8; }
+__host__ __device__ constexpr int pipe_threads(int N) { return N % 3 == 0 ? 256 : 512; }
+__host__ __device__ constexpr int pipe_groups(int N) { return pipe_threads(N) / (N / pipe_ppt(N)); } // line pairs per tile
+__host__ __device__ constexpr int pipe_cpw(int N) { return pipe_groups(N) < 8 ? pipe_groups(N) : 8; }
+__host__ __device__ constexpr int pipe_box_rows(int rows) // largest divisor of `rows` that is <= 256 (rows = 2^a 3^b)
+{
+    int r = rows;
+    while (r > 256) r = (r % 2 == 0) ? r / 2 : r / 3;
+    return r;
+}
+
 inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 {
+    // 6*4^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
+    // first-path kernels (2+ CTAs per SM) for the heavy axis-0 pass (0.94 vs 1.24 ms); the others stay first-path
+    if (N % 3 == 0 && kind != P_H_NLKIN) return false;
     switch (kind) {
     case P_S_FFT:
     case P_S_KIN:
     case P_H_NLKIN:
     case P_H_R2C:
-        return ncols % (2 * (4096 / N)) == 0; // a tile is 2 * 512/(N/8) columns wide
+        return ncols % (2 * pipe_groups(N)) == 0; // a tile is 2 G columns wide
     case P_X_KIN:
     case P_X_POISSON:
         return nlines % 2 == 0;

@@ -28,27 +28,29 @@
 
 namespace snk {
 
-constexpr int PIPE_THREADS = 512;
-constexpr int PIPE_WARPS = PIPE_THREADS / 32;
-constexpr int TILE_BYTES = 65536; // N rows x 2G columns x 8 B, for every N
 
 template <int N>
 struct Geo {
-    static constexpr int T = N / 8;                       // threads per line pair
-    static constexpr int G = PIPE_THREADS / T;            // line pairs (groups) per tile
+    static constexpr int P = pipe_ppt(N);                 // points per thread and line
+    static constexpr int NTHR = pipe_threads(N);          // threads per CTA
+    static constexpr int NWARP = NTHR / 32;
+    static constexpr int T = N / P;                       // threads per line pair
+    static constexpr int G = NTHR / T;                    // line pairs (groups) per tile
+    static constexpr int TILE_BYTES = N * 2 * G * 8;      // 64 KB (N = 2^n) or 48 KB (N = 6*4^a)
     static constexpr int CPW = G < 8 ? G : 8;             // column pairs per sub-tile row (8 for N <= 512)
     static constexpr int RBY = 16 * CPW;                  // bytes of a sub-tile row: 128, 64, 32, 16
     static constexpr int SUB = G / CPW;                   // sub-tiles per tile
-    static constexpr int RB = N < 256 ? N : 256;          // rows per TMA box
+    static constexpr int RB = pipe_box_rows(N);           // rows per TMA box
     static constexpr int NBOX = N / RB;
     static constexpr int SUB_F4 = N * CPW;                // float4 slots of a psi sub-tile
     static constexpr int SUB_BYTES = N * RBY;
     static constexpr int HROWS = N / 2 + 1;               // rows of the half spectrum
-    static constexpr int HB = N / 2 < 256 ? N / 2 : 256;  // rows per TMA box of the half spectrum (rows 0..N/2-1)
+    static constexpr int HB = pipe_box_rows(N / 2);       // rows per TMA box of the half spectrum (rows 0..N/2-1)
     static constexpr int NHBOX = (N / 2) / HB;
     static constexpr int HS_SUB_BYTES = (HROWS * RBY + 1023) / 1024 * 1024;
     static constexpr int HS_SUB_F4 = HS_SUB_BYTES / 16;
     static constexpr int HS_TX = SUB * HROWS * RBY;       // bytes one hs tile load delivers
+    static_assert(T % 8 == 0 && G * T == NTHR && SUB * CPW == G && NBOX * RB == N && NHBOX * HB == N / 2, "geometry");
 };
 
 // Slot (float4 index inside a sub-tile) of row r for column pair t < CPW: the layout the TMA swizzle of a
@@ -136,11 +138,11 @@ __device__ __forceinline__ void warp_arrive_done(uint64_t *bar)
 }
 
 // kinetic phase on a line pair: a, b *= phase[j + T m]   (S2 of SURVEY.md 8(a), separable per axis)
-template <int T>
-__device__ __forceinline__ void apply_phase(float2 (&a)[8], float2 (&b)[8], int j, const float4 *__restrict__ phase)
+template <int T, int P>
+__device__ __forceinline__ void apply_phase(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ phase)
 {
 #pragma unroll
-    for (int m = 0; m < 8; m++) {
+    for (int m = 0; m < P; m++) {
         const float4 ph = __ldg(phase + j + T * m);
         a[m] = twmul<+1, true>(a[m], ph);
         b[m] = twmul<+1, true>(b[m], ph);
@@ -153,10 +155,10 @@ __device__ __forceinline__ void apply_phase(float2 (&a)[8], float2 (&b)[8], int 
 // released the stage, stores it, and reloads the stage that tile k-1 was stored from with tile k+2.
 
 template <int N, int MODE, int DIR, bool HILO>
-__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_constant__ PipeArgs p)
+__global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 3;
+    constexpr int P = g_::P, TILE_BYTES = g_::TILE_BYTES, PIPE_WARPS = g_::NWARP, T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 3;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * TILE_BYTES), *done = full + NST;
@@ -203,9 +205,9 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
 
         const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
         float4 *mine = sub + nat_slot<CPW>(jf, t);     // row jf; rows jf + T m are CPW T m slots further (T % 8 == 0)
-        float2 a[8], c[8];
+        float2 a[P], c[P];
 #pragma unroll
-        for (int m = 0; m < 8; m++) {
+        for (int m = 0; m < P; m++) {
             const float4 v = mine[CPW * T * m];
             a[m] = lo2(v);
             c[m] = hi2(v);
@@ -215,19 +217,19 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
             if (DIR < 0) {
                 const float sc = p.a.scale;
 #pragma unroll
-                for (int m = 0; m < 8; m++) {
+                for (int m = 0; m < P; m++) {
                     a[m].x *= sc; a[m].y *= sc; c[m].x *= sc; c[m].y *= sc;
                 }
             }
         } else { // P_S_KIN
             fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-            apply_phase<T>(a, c, jf, p.a.phase);
+            apply_phase<T, P>(a, c, jf, p.a.phase);
             fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
         }
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
         __syncwarp();
 #pragma unroll
-        for (int m = 0; m < 8; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
+        for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
         warp_arrive_done(done + b);
 
         if (tid == 0) {
@@ -263,10 +265,10 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_strided(const __grid_c
 // the issuer never waits for its own store to drain.
 
 template <int N, int MODE, bool EXTRA>
-__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_constant__ PipeArgs p)
+__global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int P = g_::P, TILE_BYTES = g_::TILE_BYTES, PIPE_WARPS = g_::NWARP, T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int STAGE_BYTES = TILE_BYTES + SUB * g_::HS_SUB_BYTES;
     constexpr bool LOAD_HS = true;
     static_assert(MODE == P_H_NLKIN, "k_pipe_haxis serves P_H_NLKIN");
@@ -321,13 +323,13 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
         const int jf = opaque(j), ji = opaque(j), jz = opaque(j); // per-tile copies: see opaque()
         float4 *mine = sub + nat_slot<CPW>(jf, t);
         {
-            float2 z[8];
-            // rows jz + T m (m < 4) and N - jz - T m (m >= 4): the mirrored rows step DOWN by 8 T slots
+            float2 z[P];
+            // rows jz + T m (m < P/2) and N - jz - T m (m >= P/2): the mirrored rows step DOWN by CPW T slots
             const float4 *hup = hsub + nat_slot<CPW>(jz, t), *hdn = hsub + nat_slot<CPW>(N / 2 - jz, t);
 #pragma unroll
-            for (int m = 0; m < 8; m++) {
-                const float4 u = m < 4 ? hup[CPW * T * m] : hdn[-CPW * T * (m - 4)];
-                z[m] = m < 4 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
+            for (int m = 0; m < P; m++) {
+                const float4 u = m < P / 2 ? hup[CPW * T * m] : hdn[-CPW * T * (m - P / 2)];
+                z[m] = m < P / 2 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
             }
             SmemSubOne<T, CPW> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
             fft_single<N, -1, false>(z, jz, p.a.tw, sm1);
@@ -337,19 +339,19 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
                 bulk_wait_read<0>();
                 issue_load(k + 1);
             }
-            float2 a[8], c[8];
+            float2 a[P], c[P];
 #pragma unroll
-            for (int m = 0; m < 8; m++) {
+            for (int m = 0; m < P; m++) {
                 const float4 v = mine[CPW * T * m];
                 a[m] = nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl);
                 c[m] = nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl);
             }
             fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-            apply_phase<T>(a, c, jf, p.a.phase);
+            apply_phase<T, P>(a, c, jf, p.a.phase);
             fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
             __syncwarp();
 #pragma unroll
-            for (int m = 0; m < 8; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
+            for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
         }
         warp_arrive_done(done + b);
 
@@ -372,10 +374,10 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_haxis(const __grid_con
 // a psi stage is reloaded as soon as every warp has pulled its values into registers, and the
 // transform runs in the OUTPUT buffer (a group's N/2+1 output slots hold its N float2 positions).
 template <int N>
-__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_constant__ PipeArgs p)
+__global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_r2c(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
-    constexpr int T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
+    constexpr int P = g_::P, TILE_BYTES = g_::TILE_BYTES, PIPE_WARPS = g_::NWARP, T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int OUT_BYTES = SUB * g_::HS_SUB_BYTES;
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
@@ -419,11 +421,11 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
         float4 *hsub = reinterpret_cast<float4 *>(outb + b * OUT_BYTES) + s * g_::HS_SUB_F4;
         const int jf = opaque(j);
         mbar_wait(full + b, par);
-        float2 z[8];
+        float2 z[P];
         {
             const float4 *mine = sub + nat_slot<CPW>(jf, t);
 #pragma unroll
-            for (int m = 0; m < 8; m++) {
+            for (int m = 0; m < P; m++) {
                 const float4 v = mine[CPW * T * m];
                 z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
             }
@@ -439,18 +441,18 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
             issue_load(k + NST);
         }
         // X[k] and Y[k] from Z[k] and Z[N-k]: pass Z through the buffer once more
-        float2 dummy = make_float2(0.f, 0.f), y[5];
+        float2 dummy = make_float2(0.f, 0.f), y[P / 2 + 1];
         sm1.sync();
 #pragma unroll
-        for (int m = 0; m < 8; m++) sm1.st(jf + T * m, z[m], dummy);
+        for (int m = 0; m < P; m++) sm1.st(jf + T * m, z[m], dummy);
         sm1.sync();
 #pragma unroll
-        for (int m = 0; m < 5; m++)
-            if (m < 4 || j == 0) sm1.ld((N - (jf + T * m)) & (N - 1), y[m], dummy);
+        for (int m = 0; m <= P / 2; m++)
+            if (m < P / 2 || j == 0) sm1.ld((N - (jf + T * m)) % N, y[m], dummy);
         sm1.sync();
 #pragma unroll
-        for (int m = 0; m < 5; m++)
-            if (m < 4 || j == 0)
+        for (int m = 0; m <= P / 2; m++)
+            if (m < P / 2 || j == 0)
                 hsub[nat_slot<CPW>(jf + T * m, t)] =
                     make_float4(z[m].x + y[m].x, z[m].y - y[m].y, z[m].y + y[m].y, y[m].x - z[m].x);
         warp_arrive_done(done + b);
@@ -484,10 +486,12 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_r2c(const __grid_const
 
 template <int N>
 struct GeoX {
-    static constexpr int T = N / 8;
-    static constexpr int G = PIPE_THREADS / T;
+    static constexpr int P = pipe_ppt(N);
+    static constexpr int NTHR = pipe_threads(N);
+    static constexpr int T = N / P;
+    static constexpr int G = NTHR / T;
     static constexpr int LINES = 2 * G;
-    static_assert(LINES * N * 8 == TILE_BYTES, "tile size");
+    static constexpr int TILE_BYTES = LINES * N * 8;
 };
 
 // VEXT (P_X_KIN only): this is the last kinetic pass before an N sub-step, so psi is back in real space when
@@ -495,8 +499,9 @@ struct GeoX {
 // PAPER.md:102) commutes with the nonlinear phase and is applied here, where V arrives as contiguous lines
 // (a second bulk copy per tile: 2 stages of 64 KB psi + 32 KB V instead of 3 stages of psi).
 template <int N, int MODE, bool VEXT>
-__global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_constant__ PipeArgs p)
+__global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid_constant__ PipeArgs p)
 {
+    constexpr int P = GeoX<N>::P, TILE_BYTES = GeoX<N>::TILE_BYTES, PIPE_THREADS = GeoX<N>::NTHR, PIPE_WARPS = PIPE_THREADS / 32;
     constexpr int T = GeoX<N>::T, LINES = GeoX<N>::LINES, NST = VEXT ? 2 : 3;
     constexpr int STAGE_BYTES = VEXT ? TILE_BYTES + TILE_BYTES / 2 : TILE_BYTES;
     extern __shared__ uint8_t smem_raw[];
@@ -544,20 +549,20 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
 
         if (2 * g < nl) {
             const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
-            float2 a[8], c[8];
+            float2 a[P], c[P];
 #pragma unroll
-            for (int m = 0; m < 8; m++) {
+            for (int m = 0; m < P; m++) {
                 a[m] = la[jf + T * m];
                 c[m] = lb[jf + T * m];
             }
             if (MODE == P_X_KIN) {
                 fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-                apply_phase<T>(a, c, jf, p.a.phase);
+                apply_phase<T, P>(a, c, jf, p.a.phase);
                 fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
                 if (VEXT) {
                     const float *va = reinterpret_cast<const float *>(base + b * STAGE_BYTES + TILE_BYTES) + 2 * g * N;
 #pragma unroll
-                    for (int m = 0; m < 8; m++) {
+                    for (int m = 0; m < P; m++) {
                         a[m] = rotate_half_angle(a[m], p.a.nl.hv * va[ji + T * m]);
                         c[m] = rotate_half_angle(c[m], p.a.nl.hv * va[N + ji + T * m]);
                     }
@@ -566,7 +571,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
                 fft_pair<N, +1, false>(a, c, jf, p.a.tw, sm);
                 const float ka = __ldg(p.a.kother2 + line0 + 2 * g), kb = __ldg(p.a.kother2 + line0 + 2 * g + 1);
 #pragma unroll
-                for (int m = 0; m < 8; m++) {
+                for (int m = 0; m < P; m++) {
                     const float kx2 = __ldg(p.a.ksq + jf + T * m);
                     const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
                     const float ga = da == 0.f ? 0.f : __fdividef(p.a.pscale, da);
@@ -577,7 +582,7 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
             }
             sm.sync(); // exchange layout (float4 per position) != line layout: whole group must be done reading
 #pragma unroll
-            for (int m = 0; m < 8; m++) {
+            for (int m = 0; m < P; m++) {
                 la[ji + T * m] = a[m];
                 lb[ji + T * m] = c[m];
             }
@@ -601,11 +606,11 @@ __global__ void __launch_bounds__(PIPE_THREADS, 1) k_pipe_contig(const __grid_co
 // ---------------------------------------------------------------------------- launchers
 
 template <class K>
-static int launch_pipe_kernel(K kern, size_t smem_bytes, const PipeArgs &a)
+static int launch_pipe_kernel(K kern, int threads, size_t smem_bytes, const PipeArgs &a)
 {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
     if (e != cudaSuccess) return (int)e;
-    kern<<<a.grid, PIPE_THREADS, smem_bytes, a.a.stream>>>(a);
+    kern<<<a.grid, threads, smem_bytes, a.a.stream>>>(a);
     return (int)cudaGetLastError();
 }
 
@@ -613,25 +618,26 @@ template <int N>
 int launch_pipe(const PipeArgs &a)
 {
     constexpr size_t SLACK = 1024 + 64; // alignment of the ring + the mbarriers
+    constexpr int TILE_BYTES = Geo<N>::TILE_BYTES, NT = pipe_threads(N);
     constexpr size_t S3 = 3 * (size_t)TILE_BYTES + SLACK;
     if (a.a.kind == P_X_KIN)
-        return a.a.vext ? launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, true>, S3, a)
-                        : launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, false>, S3, a);
-    if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON, false>, S3, a);
+        return a.a.vext ? launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, true>, NT, S3, a)
+                        : launch_pipe_kernel(k_pipe_contig<N, P_X_KIN, false>, NT, S3, a);
+    if (a.a.kind == P_X_POISSON) return launch_pipe_kernel(k_pipe_contig<N, P_X_POISSON, false>, NT, S3, a);
     {
         constexpr size_t S2H = 2 * ((size_t)TILE_BYTES + Geo<N>::SUB * Geo<N>::HS_SUB_BYTES) + SLACK;
         switch (a.a.kind) {
-        case P_S_KIN: return launch_pipe_kernel(k_pipe_strided<N, P_S_KIN, +1, true>, S3, a);
+        case P_S_KIN: return launch_pipe_kernel(k_pipe_strided<N, P_S_KIN, +1, true>, NT, S3, a);
         case P_S_FFT:
             if (a.a.dir > 0)
-                return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, true>, S3, a)
-                                : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, false>, S3, a);
-            return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, true>, S3, a)
-                            : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, false>, S3, a);
+                return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, true>, NT, S3, a)
+                                : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, +1, false>, NT, S3, a);
+            return a.a.hilo ? launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, true>, NT, S3, a)
+                            : launch_pipe_kernel(k_pipe_strided<N, P_S_FFT, -1, false>, NT, S3, a);
         case P_H_NLKIN:
-            return (a.a.nl.flags & 1) ? launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, true>, S2H, a)
-                                      : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, S2H, a);
-        case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, S2H, a);
+            return (a.a.nl.flags & 1) ? launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, true>, NT, S2H, a)
+                                      : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, NT, S2H, a);
+        case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, NT, S2H, a);
         default: break;
         }
     }
