@@ -73,6 +73,8 @@ typedef struct snref_ctx {
      * w ln(rho) / (n w/(n-1)) rho^(n-1), and a fixed external potential phi_C(r) (eq. (11)) */
     double g_log, rho_floor, g_pow, p_pow;
     double *vext; /* NULL or cells doubles */
+    /* modified Poisson source of eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho) */
+    double *beta, *gamma; /* both NULL (plain eq. (2)) or both cells doubles */
     cplx *psi;   /* state */
     cplx *work;  /* rho^ / phi^ scratch */
     int has_state;
@@ -316,9 +318,28 @@ int snref_set_external_potential(snref_ctx *c, const double *v)
     return SNREF_OK;
 }
 
+/* position-dependent source of eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); tables are copied;
+ * two NULLs restore eq. (2) (equivalent to gamma = 1, beta = 0) */
+int snref_set_source_tables(snref_ctx *c, const double *beta, const double *gamma)
+{
+    if (!c) return SNREF_ERR_NULL;
+    if ((beta == NULL) != (gamma == NULL)) return SNREF_ERR_NULL;
+    free(c->beta); free(c->gamma);
+    c->beta = c->gamma = NULL;
+    if (!beta) return SNREF_OK;
+    c->beta = (double *)malloc(sizeof(double) * (size_t)c->cells);
+    c->gamma = (double *)malloc(sizeof(double) * (size_t)c->cells);
+    if (!c->beta || !c->gamma) { free(c->beta); free(c->gamma); c->beta = c->gamma = NULL; return SNREF_ERR_NOMEM; }
+    memcpy(c->beta, beta, sizeof(double) * (size_t)c->cells);
+    memcpy(c->gamma, gamma, sizeof(double) * (size_t)c->cells);
+    return SNREF_OK;
+}
+
 int snref_destroy(snref_ctx *c)
 {
     if (!c) return SNREF_ERR_NULL;
+    free(c->beta);
+    free(c->gamma);
     free(c->vext);
     free(c->psi);
     free(c->work);
@@ -374,7 +395,20 @@ static int potential(snref_ctx *c)
         double re = creal(c->psi[i]), im = cimag(c->psi[i]);
         c->work[i] = re * re + im * im;
     }
-    int rc = fftn(c->work, c->ndim, c->n, +1);
+    int rc;
+    if (c->beta) {
+        /* source s = gamma rho + beta lap rho, lap rho spectrally: F^-1[-k^2 F[rho]]   (eq. (12)) */
+        if ((rc = fftn(c->work, c->ndim, c->n, +1))) return rc;
+#pragma omp parallel for schedule(static)
+        for (int64_t i = 0; i < c->cells; i++) c->work[i] *= -ksq_at(c, i);
+        if ((rc = fftn(c->work, c->ndim, c->n, -1))) return rc;
+#pragma omp parallel for schedule(static)
+        for (int64_t i = 0; i < c->cells; i++) {
+            double re = creal(c->psi[i]), im = cimag(c->psi[i]);
+            c->work[i] = c->gamma[i] * (re * re + im * im) + c->beta[i] * creal(c->work[i]);
+        }
+    }
+    rc = fftn(c->work, c->ndim, c->n, +1);
     if (rc) return rc;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < c->cells; i++) {

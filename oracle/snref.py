@@ -50,6 +50,7 @@ def lib() -> ctypes.CDLL:
         L.snref_diagnostics.argtypes = [vp, ctypes.POINTER(SnrefDiag)]
         L.snref_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
         L.snref_set_external_potential.argtypes = [vp, vp]
+        L.snref_set_source_tables.argtypes = [vp, vp, vp]
         L.snref_num_threads.restype = ctypes.c_int
         L.snref_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -149,6 +150,16 @@ class Oracle:
         a = np.ascontiguousarray(v, dtype=np.float64)
         assert a.shape == self.dims, (a.shape, self.dims)
         _chk(lib().snref_set_external_potential(self._h, a.ctypes.data), "snref_set_external_potential")
+
+    def set_source_tables(self, beta, gamma) -> None:
+        """eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); (None, None) restores eq. (2)."""
+        if beta is None and gamma is None:
+            _chk(lib().snref_set_source_tables(self._h, None, None), "snref_set_source_tables")
+            return
+        b = np.ascontiguousarray(beta, dtype=np.float64)
+        g = np.ascontiguousarray(gamma, dtype=np.float64)
+        assert b.shape == self.dims and g.shape == self.dims
+        _chk(lib().snref_set_source_tables(self._h, b.ctypes.data, g.ctypes.data), "snref_set_source_tables")
 
     def potential(self) -> np.ndarray:
         out = np.empty(self.dims, dtype=np.float64)

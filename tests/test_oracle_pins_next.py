@@ -133,3 +133,44 @@ def test_w4_energy_closed_forms_and_conservation():
     assert abs(d1["e_total"] - d0["e_total"]) < 2e-6 * abs(d0["e_total"])   # O(dtau^2), bounded
     assert abs(d1["norm"] - d0["norm"]) < 1e-12 * d0["norm"]
     o.close()
+
+
+# ------------------------------------------------------------------ W5 modified Poisson source, eq. (12)
+
+@pytest.mark.parametrize("dims,C", [((32, 48), 0.0), ((16, 24, 32), -0.8)])
+def test_w5_position_dependent_source_closed_form(dims, C):
+    """rho = rb + e cos(q.x), beta = b0 + b1 cos(p.x), gamma = g0 + g1 cos(p.x):
+    s = gamma rho + beta lap rho has modes 0, p, q, p+q, p-q with amplitudes from cos a cos b = (cos(a+b) + cos(a-b))/2;
+    each mode k gives phi_k = D s_k/(C - |k|^2) (mode 0: dropped if C = 0, else D s_0/C)."""
+    L, D = 9.0, 1.7
+    nd = len(dims)
+    X = grid(dims, L)
+    k0 = 2 * np.pi / L
+    q = np.array([2, 1, -1][:nd]) * k0
+    p = np.array([1, -2, 2][:nd]) * k0
+    rb, e, b0, b1, g0, g1 = 1.3, 0.4, 0.25, 0.1, 0.6, -0.2
+    ph = lambda k: sum(ka * xa for ka, xa in zip(k, X))
+    rho = rb + e * np.cos(ph(q))
+    beta = b0 + b1 * np.cos(ph(p))
+    gamma = g0 + g1 * np.cos(ph(p))
+    q2 = float(q @ q)
+    # s = g0 rb + g0 e cos q + g1 rb cos p + g1 e cos p cos q - q2 e (b0 cos q + b1 cos p cos q)
+    modes = [(np.zeros(nd), g0 * rb), (q, g0 * e - q2 * e * b0), (p, g1 * rb),
+             (p + q, 0.5 * (g1 * e - q2 * e * b1)), (p - q, 0.5 * (g1 * e - q2 * e * b1))]
+    want = np.zeros(dims)
+    for k, amp in modes:
+        k2 = float(k @ k)
+        if k2 == 0.0:
+            want += 0.0 if C == 0.0 else D * amp / C
+        else:
+            want += D * amp / (C - k2) * np.cos(ph(k))
+    o = Oracle(dims, L, -0.5, 1.0, C, D, (), 1e-3)
+    o.set_source_tables(beta, gamma)
+    o.set_state(np.sqrt(rho).astype(complex))
+    assert np.abs(o.potential() - want).max() < 1e-12 * max(1.0, np.abs(want).max())
+    # gamma = 1, beta = 0 is eq. (2) itself
+    o.set_source_tables(np.zeros(dims), np.ones(dims))
+    a = o.potential()
+    o.set_source_tables(None, None)
+    assert np.abs(a - o.potential()).max() < 1e-13
+    o.close()
