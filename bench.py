@@ -46,6 +46,7 @@ PASS_BYTES_PER_CELL = {
     "H_R2C": 12.0,     # read psi (8) + write rho^ (4)
     "S_FFT": 8.0,      # read + write half spectrum
     "X_POISSON": 8.0,
+    "H_SRC": 24.0,     # eq. (12): read F[lap rho] (4) + psi (8) + beta, gamma (8), write F[s] (4)
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
 B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update

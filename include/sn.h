@@ -94,7 +94,13 @@ int sn_set_dtau(sn_ctx *ctx, double dtau);
  *   device pointer, copied into the workspace) enters the N sub-step as exp(-i s (B phi + G(rho) + V)) -- phi_C
  *   of eq. (11),(15).  NULL removes it.  With V set the axis-0 nonlinear pass runs the first-path kernel.
  * Both rebuild the nonlinear-phase coefficients; e_local of sn_diagnostics then includes sum (F(rho) + V rho) dV. */
+/* sn_set_source_tables: eq. (12), PAPER.md:92 -- lap phi + C phi = D (gamma(x) rho + beta(x) lap rho) instead of
+ *   eq. (2).  beta, gamma: float32, prod(dims) values each, layout of psi, host or device (copied into the
+ *   workspace); two NULLs restore eq. (2) (= gamma 1, beta 0).  Costs one more half-spectrum chain and one more
+ *   axis-0 pass per step.  e_nonlocal of sn_diagnostics stays (B/2) sum phi rho dV (no longer a conserved energy
+ *   when beta, gamma vary in space: the kernel of phi[rho] is not symmetric). */
 int sn_set_local_terms(sn_ctx *ctx, double g_log, double rho_floor, double g_pow, double p_pow);
+int sn_set_source_tables(sn_ctx *ctx, const float *beta, const float *gamma, int src_on_device);
 int sn_set_external_potential(sn_ctx *ctx, const float *v, int src_on_device);
 
 int sn_destroy(sn_ctx *ctx);
@@ -114,8 +120,8 @@ int64_t sn_launch_count(const sn_ctx *ctx);
  *   4 H_R2C  axis-0 density + packed r2c           5 H_POT  axis-0 c2r -> phi (test hook)
  *   6 H_DIAG axis-0 c2r + energy sums              7 X_FFT  contiguous-axis plain transform
  *   8 X_KIN  contiguous-axis forward-phase-inverse 9 X_POISSON contiguous-axis forward-D/(C-k^2)-inverse
- *  10 X_KDIAG contiguous-axis kinetic-energy sum */
-#define SN_NUM_PASS_KINDS 11
+ *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12)) */
+#define SN_NUM_PASS_KINDS 12
 int sn_profile(sn_ctx *ctx, int enable);
 int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 11 */, int64_t *launches_by_kind /* host, 11 */,
                     int reset);

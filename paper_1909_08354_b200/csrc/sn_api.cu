@@ -50,7 +50,7 @@ struct Layout {
     int ndim;
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
-    size_t off_psi, off_hs, off_phi, off_vext, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
+    size_t off_psi, off_hs, off_phi, off_vext, off_beta, off_gamma, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
 };
 
 bool make_layout(int ndim, const int64_t *dims, Layout &L)
@@ -73,6 +73,8 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L)
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
     L.off_phi = o; o = align256(o + (size_t)L.cells * 4);
     L.off_vext = o; o = align256(o + (size_t)L.cells * 4);
+    L.off_beta = o; o = align256(o + (size_t)L.cells * 4);
+    L.off_gamma = o; o = align256(o + (size_t)L.cells * 4);
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
         L.off_ph_full[d] = o; o = align256(o + (size_t)L.n[d] * 16);
@@ -112,6 +114,8 @@ struct sn_ctx {
     bool has_vext;                          // external potential set (eq. (15) phi_C)
     bool v_in_xkin;                         // its phase is applied by the pipelined contiguous-axis kinetic pass
     float *vext;
+    bool has_src;                           // position-dependent Poisson source of eq. (12) set
+    float *beta, *gamma;
     int n_g;
     char *ws;
     cudaStream_t stream;
@@ -457,17 +461,12 @@ int kinetic_sweep(sn_ctx *c, bool half, bool with_nl, bool before_n)
     return SN_OK;
 }
 
-// phi^ (half spectrum, all scales folded in, ready for the axis-0 c2r) from the current psi
-int potential_spectrum(sn_ctx *c)
+// half-spectrum passes along the non-zero axes: forward (axis 1 in 3D) -> fused forward-multiply-inverse along
+// the contiguous axis -> inverse (axis 1).  lap: multiply by -k^2/prod(N) (Laplacian) instead of D/(C - k^2)/prod(N).
+int spectrum_chain(sn_ctx *c, bool lap)
 {
     const Layout &l = c->lay;
     int rc;
-    {
-        PassArgs a = base_args(c);
-        a.kind = snk::P_H_R2C; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
-        set_axis_geometry(c, a, 0, l.n[0]);
-        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
-    }
     if (l.ndim == 3) {
         PassArgs a = base_args(c);
         a.kind = snk::P_S_FFT; a.dir = +1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1];
@@ -479,7 +478,8 @@ int potential_spectrum(sn_ctx *c)
         PassArgs a = base_args(c);
         a.kind = snk::P_X_POISSON; a.data = c->hs; a.tw = c->tw[dx]; a.ksq = c->ksq[dx]; a.kother2 = c->kother;
         a.nlines = (int)l.hs_lines;
-        a.pscale = (float)(c->D * 0.5 / (double)l.cells);
+        a.lap = lap ? 1 : 0;
+        a.pscale = (float)((lap ? 1.0 : c->D) * 0.5 / (double)l.cells); // 0.5: the packed r2c carries a factor 2
         if ((rc = run_pass(c, (int)l.n[dx], a))) return rc;
     }
     if (l.ndim == 3) {
@@ -489,6 +489,29 @@ int potential_spectrum(sn_ctx *c)
         if ((rc = run_pass(c, (int)l.n[1], a))) return rc;
     }
     return SN_OK;
+}
+
+// phi^ (half spectrum, all scales folded in, ready for the axis-0 c2r) from the current psi.
+// With source tables (eq. (12)): rho -> F[rho] -> -k^2 -> lap rho -> s = gamma rho + beta lap rho -> F[s] -> phi^.
+int potential_spectrum(sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    int rc;
+    {
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_R2C; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+        set_axis_geometry(c, a, 0, l.n[0]);
+        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    }
+    if (c->has_src) {
+        if ((rc = spectrum_chain(c, /*lap=*/true))) return rc;
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_SRC; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+        a.beta = c->beta; a.gamma = c->gamma;
+        set_axis_geometry(c, a, 0, l.n[0]);
+        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    }
+    return spectrum_chain(c, /*lap=*/false);
 }
 
 // capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
@@ -579,6 +602,8 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
     c->hs = reinterpret_cast<float2 *>(c->ws + l.off_hs);
     c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
     c->vext = reinterpret_cast<float *>(c->ws + l.off_vext);
+    c->beta = reinterpret_cast<float *>(c->ws + l.off_beta);
+    c->gamma = reinterpret_cast<float *>(c->ws + l.off_gamma);
     c->rho_floor = 1e-30; c->p_pow = 1.0;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
@@ -663,6 +688,22 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
     c->has_vext = v != nullptr;
     c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0; // the pipelined contiguous pass serves 2^n only
     return upload_phase_tables(c);
+}
+
+int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int src_on_device)
+{
+    if (!c) return SN_ERR_NULL;
+    if ((beta == nullptr) != (gamma == nullptr)) return SN_ERR_NULL;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c);
+    if (beta) {
+        const cudaMemcpyKind k = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+        SN_CUDA(cudaMemcpyAsync(c->beta, beta, (size_t)c->lay.cells * 4, k, c->stream));
+        SN_CUDA(cudaMemcpyAsync(c->gamma, gamma, (size_t)c->lay.cells * 4, k, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream));
+    }
+    c->has_src = beta != nullptr;
+    return SN_OK;
 }
 
 int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)

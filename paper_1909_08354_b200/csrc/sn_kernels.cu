@@ -149,14 +149,30 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
     float4 *hs4 = reinterpret_cast<float4 *>(p.hs) + col4;
     SmemTile<CP> sm{smem, t};
 
-    if (MODE == P_H_R2C) {
+    if (MODE == P_H_R2C || MODE == P_H_SRC) {
         float2 a[P], b[P];
+        if (MODE == P_H_SRC) {
+            // eq. (12): the half spectrum holds F[lap rho]; bring it back along axis 0 and form the source
+            // s = gamma(x) rho + beta(x) lap rho for the thread's four real columns, then transform s like rho
+            c2r_potential<N, CP>(p, hs4, rs4, t, j, a, b, sm);
+            const float2 *be2 = reinterpret_cast<const float2 *>(p.beta) + col4, *ga2 = reinterpret_cast<const float2 *>(p.gamma) + col4;
 #pragma unroll
-        for (int m = 0; m < P; m++) {
-            const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
-            const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
-            a[m] = make_float2(abs2(lo2(u)), abs2(hi2(u)));
-            b[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+            for (int m = 0; m < P; m++) {
+                const long long row = (long long)(j + T * m) * rs4;
+                const float4 u = psi4[row + t], v = psi4[row + CP + t];
+                const float2 b0 = __ldg(be2 + row + t), b1 = __ldg(be2 + row + CP + t);
+                const float2 g0 = __ldg(ga2 + row + t), g1 = __ldg(ga2 + row + CP + t);
+                a[m] = make_float2(fmaf(g0.x, abs2(lo2(u)), b0.x * a[m].x), fmaf(g0.y, abs2(hi2(u)), b0.y * a[m].y));
+                b[m] = make_float2(fmaf(g1.x, abs2(lo2(v)), b1.x * b[m].x), fmaf(g1.y, abs2(hi2(v)), b1.y * b[m].y));
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < P; m++) {
+                const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
+                const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
+                a[m] = make_float2(abs2(lo2(u)), abs2(hi2(u)));
+                b[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+            }
         }
         fft_pair<N, +1, false>(a, b, j, p.tw, sm);
         sm.sync();
@@ -309,8 +325,9 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         for (int m = 0; m < P; m++) {
             const float kx2 = __ldg(p.ksq + j + T * m);
             const float da = p.C - kx2 - ka, db = p.C - kx2 - kb;
-            const float ga = da == 0.f ? 0.f : p.pscale / da;
-            const float gb = db == 0.f ? 0.f : p.pscale / db;
+            // lap != 0: multiply by -k^2 instead (Laplacian of the density, eq. (12))
+            const float ga = p.lap ? -(kx2 + ka) * p.pscale : (da == 0.f ? 0.f : p.pscale / da);
+            const float gb = p.lap ? -(kx2 + kb) * p.pscale : (db == 0.f ? 0.f : p.pscale / db);
             a[m].x *= ga; a[m].y *= ga; b[m].x *= gb; b[m].y *= gb;
         }
         fft_pair<N, -1, false>(a, b, j, p.tw, sm);
@@ -366,11 +383,13 @@ int launch_pass(const PassArgs &a)
     case P_H_NLKIN:
     case P_H_R2C:
     case P_H_POT:
+    case P_H_SRC:
     case P_H_DIAG: {
         const unsigned grid = (unsigned)(a.ncols / (4 * CP));
         if (a.kind == P_H_NLKIN) return launch_kernel(k_haxis<N, CP, P_H_NLKIN>, grid, ST, SSMEM, a);
         if (a.kind == P_H_R2C) return launch_kernel(k_haxis<N, CP, P_H_R2C>, grid, ST, SSMEM, a);
         if (a.kind == P_H_POT) return launch_kernel(k_haxis<N, CP, P_H_POT>, grid, ST, SSMEM, a);
+        if (a.kind == P_H_SRC) return launch_kernel(k_haxis<N, CP, P_H_SRC>, grid, ST, SSMEM, a);
         return launch_kernel(k_haxis<N, CP, P_H_DIAG>, grid, ST, SSMEM, a);
     }
     case P_X_FFT:

@@ -17,7 +17,8 @@ enum PassKind {
     P_X_FFT,       // contiguous axis: plain c2c transform
     P_X_KIN,       // contiguous axis: forward -> kinetic phase -> inverse
     P_X_POISSON,   // contiguous axis of the half spectrum: forward -> D/(C-k^2) -> inverse (S5-S7)
-    P_X_KDIAG      // contiguous axis: forward, accumulate sum k_x^2 |psi^|^2
+    P_X_KDIAG,     // contiguous axis: forward, accumulate sum k_x^2 |psi^|^2
+    P_H_SRC        // axis 0: c2r of F[lap rho] -> s = gamma rho + beta lap rho -> packed r2c   (eq. (12), NEXT-1)
 };
 
 // Nonlinear phase psi *= exp(-i dtau (B phi + sum_j g_j rho^j)), stored as HALF-angle
@@ -56,6 +57,8 @@ struct PassArgs {
     NLParams nl;
     float *phi_out;         // DEVICE: P_H_POT
     const float *vext;      // DEVICE: external potential (same layout as psi, float) or nullptr
+    const float *beta, *gamma; // DEVICE: P_H_SRC source tables of eq. (12) (layout of psi, float)
+    int lap;                // P_X_POISSON: multiply by -k^2 * pscale instead of pscale/(C - k^2)
     double *diag;           // DEVICE: accumulators
     cudaStream_t stream;
 };

@@ -574,8 +574,9 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
                 for (int m = 0; m < P; m++) {
                     const float kx2 = __ldg(p.a.ksq + jf + T * m);
                     const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
-                    const float ga = da == 0.f ? 0.f : __fdividef(p.a.pscale, da);
-                    const float gb = db == 0.f ? 0.f : __fdividef(p.a.pscale, db);
+                    // lap != 0: multiply by -k^2 instead (Laplacian of the density, eq. (12))
+                    const float ga = p.a.lap ? -(kx2 + ka) * p.a.pscale : (da == 0.f ? 0.f : __fdividef(p.a.pscale, da));
+                    const float gb = p.a.lap ? -(kx2 + kb) * p.a.pscale : (db == 0.f ? 0.f : __fdividef(p.a.pscale, db));
                     a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
                 }
                 fft_pair<N, -1, false>(a, c, ji, p.a.tw, sm);

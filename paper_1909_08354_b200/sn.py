@@ -23,10 +23,10 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
-              "X_KDIAG")
+              "X_KDIAG", "H_SRC")
 
 
 class SnDiag(ctypes.Structure):
@@ -73,6 +73,7 @@ def lib() -> ctypes.CDLL:
         L.sn_debug_potential.argtypes = [vp, vp, ctypes.c_int]
         L.sn_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
         L.sn_set_external_potential.argtypes = [vp, vp, ctypes.c_int]
+        L.sn_set_source_tables.argtypes = [vp, vp, vp, ctypes.c_int]
         _lib = L
     return _lib
 
@@ -191,6 +192,23 @@ class Simulation:
             assert v.dtype == torch.float32 and v.is_contiguous() and tuple(v.shape) == self.dims
             _chk(lib().sn_set_external_potential(self._h, ctypes.c_void_p(v.data_ptr()), 1 if v.is_cuda else 0),
                  "sn_set_external_potential")
+
+    def set_source_tables(self, beta, gamma) -> None:
+        """eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); numpy float32 arrays or CUDA float32
+        tensors of shape dims; (None, None) restores eq. (2)."""
+        if beta is None and gamma is None:
+            _chk(lib().sn_set_source_tables(self._h, None, None, 0), "sn_set_source_tables")
+        elif isinstance(beta, np.ndarray):
+            b = np.ascontiguousarray(beta, dtype=np.float32)
+            g = np.ascontiguousarray(gamma, dtype=np.float32)
+            assert b.shape == self.dims and g.shape == self.dims
+            _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
+                 "sn_set_source_tables")
+        else:
+            assert beta.is_cuda and gamma.is_cuda and beta.is_contiguous() and gamma.is_contiguous()
+            assert tuple(beta.shape) == self.dims and tuple(gamma.shape) == self.dims
+            _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(beta.data_ptr()),
+                                            ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables")
 
     def diagnostics(self) -> dict:
         d = SnDiag()

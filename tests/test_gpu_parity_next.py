@@ -102,3 +102,66 @@ def test_parameter_validation(mods):
             sim.set_local_terms(*bad)
         assert e.value.code == -3
     sim.close()
+
+
+# ------------------------------------------------------------------ eq. (12): position-dependent Poisson source
+
+def nmc_tables(dims, L, lam=1.0, r0=2.0):
+    """gamma = (1/2)[1 - (r0/(r+r0))^lambda] (eq. (9)), beta = lambda (r0/(r+r0))^lambda /(r+r0) (eq. (10)), radius
+    softened to sqrt(r^2 + 1) as for phi_C."""
+    from paper_1909_08354_b200 import inputs
+    X = np.meshgrid(*[inputs.coords(n, L) for n in dims], indexing="ij")
+    r = np.sqrt(sum(x * x for x in X) + 1.0)
+    f = (r0 / (r + r0)) ** lam
+    return (lam * f / (r + r0)).astype(np.float32), (0.5 * (1.0 - f)).astype(np.float32)
+
+
+@pytest.mark.parametrize("dims,C", [((128, 64), 0.0), ((64, 256), -1.0), ((64, 64, 128), 0.0), ((96, 64, 64), -0.7)])
+def test_source_tables_potential_matches_oracle(mods, dims, C):
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C2" if len(dims) == 2 else "C4"], dims, L=16.0)
+    psi0 = cfg.initial_state()
+    beta, gamma = nmc_tables(dims, 16.0)
+    sim = sn.Simulation(dims, 16.0, -0.5, 1.0, C, 0.9, (0.1,), 1e-3)
+    sim.set_source_tables(beta, gamma)
+    sim.set_state(psi0)
+    orc = Oracle(dims, 16.0, -0.5, 1.0, C, 0.9, (0.1,), 1e-3)
+    orc.set_source_tables(beta.astype(np.float64), gamma.astype(np.float64))
+    orc.set_state(psi0.astype(np.complex128))
+    want = orc.potential()
+    assert rel(sim.debug_potential(), want) < 5e-6
+    sim.set_source_tables(None, None)                      # back to eq. (2)
+    orc.set_source_tables(None, None)
+    assert rel(sim.debug_potential(), orc.potential()) < 2e-6
+    sim.close()
+    orc.close()
+
+
+@pytest.mark.parametrize("name,dims,L,steps", [("C2", (256, 256), 25.0, 150), ("C4", (64, 128, 64), 16.0, 60),
+                                               ("C5_256", (128, 128, 128), 128.0, 10)])
+def test_source_tables_steps_match_oracle(mods, name, dims, L, steps):
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=steps)
+    psi0 = cfg.initial_state()
+    beta, gamma = nmc_tables(dims, L)
+    sim = sn.Simulation.from_config(cfg)
+    sim.set_source_tables(beta, gamma)
+    sim.set_external_potential(nmc_potential(dims, L).astype(np.float32))   # the full NMC model of eq. (15): phi_N + phi_C
+    sim.set_state(psi0)
+    d0 = sim.diagnostics()
+    sim.step(steps)
+    got = sim.get_state()
+    d1 = sim.diagnostics()
+    sim.close()
+    orc = Oracle.from_config(cfg)
+    orc.set_source_tables(beta.astype(np.float64), gamma.astype(np.float64))
+    orc.set_external_potential(nmc_potential(dims, L).astype(np.float32).astype(np.float64))
+    orc.set_state(psi0.astype(np.complex128))
+    orc.step(steps)
+    want = orc.get_state()
+    r1 = orc.diagnostics()
+    orc.close()
+    assert rel(got, want) < TOL_STATE
+    assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
+    for k in ("e_kin", "e_nonlocal", "e_local"):
+        assert abs(d1[k] - r1[k]) < 2e-5 * max(abs(r1["e_total"]), abs(r1[k])), (k, d1[k], r1[k])

@@ -32,8 +32,9 @@ def test_workspace_bytes(lib):
     assert sn.workspace_bytes((64, 64)) > 64 * 64 * 8
     w = sn.workspace_bytes((512, 512, 512))
     cells = 512 ** 3
-    # psi (8 B) + half spectrum (~4 B) + phi scratch for the test hook (4 B) + external potential (4 B) + tables
-    assert cells * 20 < w < cells * 20.2
+    # psi (8 B) + half spectrum (~4 B) + phi scratch for the test hook (4 B) + external potential (4 B)
+    # + beta, gamma tables of eq. (12) (4 B each) + FFT tables
+    assert cells * 28 < w < cells * 28.2
     assert w % 256 == 0
     for bad in [(64,), (64, 64, 64, 64), (48, 64), (32, 64), (8192, 64), (64, 100), (0, 64), (192, 64)]:
         assert sn.workspace_bytes(bad) == 0
