@@ -179,7 +179,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--extras", action="store_true",
                     help="NEXT-1 row: also run with the pressure potential 0.02 ln(rho) (eq. (16)) and the "
-                         "phi_C table of eq. (11) as external potential (DESIGN.md section 9)")
+                         "phi_C table of eq. (11) as external potential and the beta, gamma tables of eq. (12) "
+                         "(DESIGN.md section 8)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
 
@@ -222,10 +223,13 @@ def main():
         # r0 = 2, radius softened to sqrt(r^2 + 1) (the grid has a point at r = 0)
         ax = [inputs.coords(n, cfg.L) for n in cfg.dims]
         r2 = sum(np.square(a).reshape([-1 if i == k else 1 for i in range(nd)]) for k, a in enumerate(ax))
-        V = np.log(1.0 - 2.0 / (np.sqrt(r2 + 1.0) + 2.0)).astype(np.float32)
+        rs = np.sqrt(r2 + 1.0)
+        f = 2.0 / (rs + 2.0)
         sim.set_local_terms(0.02, 1e-12, 0.0, 1.0)
-        sim.set_external_potential(V)
-        del V, r2
+        sim.set_external_potential(np.log(1.0 - f).astype(np.float32))
+        # eq. (12) with eq. (9),(10): gamma = (1 - f)/2, beta = lambda f/(r + r0)
+        sim.set_source_tables((f / (rs + 2.0)).astype(np.float32), (0.5 * (1.0 - f)).astype(np.float32))
+        del rs, f, r2
     sim.set_state(dev_in)
     sim.step(W)                                         # untimed warm-up steps
     barrier()
@@ -283,7 +287,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
-            "config": {"workload": f"{cfg.name}{'+next1(0.02 ln rho, phi_C table)' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
+            "config": {"workload": f"{cfg.name}{'+next1(0.02 ln rho, phi_C, beta/gamma tables of eq. (12))' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
                                    f"B={cfg.B}, C={cfg.C}, D={cfg.D:.6g}, g={list(cfg.g)}, dtau={cfg.dtau}",
                        "dims": list(cfg.dims), "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
