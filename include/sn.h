@@ -77,6 +77,11 @@ int sn_set_state(sn_ctx *ctx, const void *psi, int src_on_device);
  * synchronising.  Adjacent kinetic half steps are merged inside one call (mathematically identical). */
 int sn_step(sn_ctx *ctx, int64_t nsteps);
 
+/* Fourth-order variant (not in the paper, which uses the second-order symmetric scheme of
+ * PAPER.md:113): one step is the Yoshida composition S2(w1 dtau) S2(w0 dtau) S2(w1 dtau) of three Strang steps,
+ * w1 = 1/(2 - 2^(1/3)), w0 = 1 - 2 w1 (< 0), adjacent kinetic half steps merged.  Three N sub-steps per step. */
+int sn_step_order4(sn_ctx *ctx, int64_t nsteps);
+
 /* Copy the state out.  A host destination synchronises the stream. */
 int sn_get_state(sn_ctx *ctx, void *psi_out, int dst_on_device);
 

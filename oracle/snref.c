@@ -452,6 +452,26 @@ int snref_step(snref_ctx *c, int64_t nsteps)
     return SNREF_OK;
 }
 
+/* n fourth-order steps: each is the composition S2(w1 dtau) S2(w0 dtau) S2(w1 dtau) of three Strang steps
+ * (Yoshida 1990 triple jump), w1 = 1/(2 - 2^(1/3)), w0 = 1 - 2 w1; written out as three plain Strang steps,
+ * nothing merged.  Not in the paper (its scheme is the second-order one); SURVEY.md 8(f) item 4. */
+int snref_step_order4(snref_ctx *c, int64_t nsteps)
+{
+    if (!c) return SNREF_ERR_NULL;
+    if (!c->has_state) return SNREF_ERR_STATE;
+    if (nsteps < 0) return SNREF_ERR_PARAM;
+    const double w1 = 1.0 / (2.0 - cbrt(2.0)), w0 = 1.0 - 2.0 * w1, h = c->dtau;
+    const double w[3] = {w1, w0, w1};
+    int rc = SNREF_OK;
+    for (int64_t s = 0; s < nsteps && !rc; s++)
+        for (int i = 0; i < 3 && !rc; i++) {
+            c->dtau = w[i] * h;
+            rc = snref_step(c, 1);
+        }
+    c->dtau = h;
+    return rc;
+}
+
 /* phi (real, cells doubles) from the current state; state unchanged */
 int snref_potential(snref_ctx *c, double *phi_out)
 {

@@ -46,6 +46,7 @@ def lib() -> ctypes.CDLL:
         L.snref_set_state.argtypes = [vp, vp]
         L.snref_get_state.argtypes = [vp, vp]
         L.snref_step.argtypes = [vp, ctypes.c_int64]
+        L.snref_step_order4.argtypes = [vp, ctypes.c_int64]
         L.snref_potential.argtypes = [vp, vp]
         L.snref_diagnostics.argtypes = [vp, ctypes.POINTER(SnrefDiag)]
         L.snref_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
@@ -133,6 +134,9 @@ class Oracle:
 
     def step(self, n: int) -> None:
         _chk(lib().snref_step(self._h, int(n)), "snref_step")
+
+    def step_order4(self, n: int) -> None:
+        _chk(lib().snref_step_order4(self._h, int(n)), "snref_step_order4")
 
     def set_dtau(self, dtau: float) -> None:
         _chk(lib().snref_set_dtau(self._h, float(dtau)), "snref_set_dtau")

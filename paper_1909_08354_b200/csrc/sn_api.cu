@@ -17,6 +17,15 @@ namespace {
 
 using snk::PassArgs;
 
+// kinetic sub-step lengths (in units of dtau) and nonlinear sub-step lengths of the two integrators:
+// Strang: K(1/2) N(1) K(1/2), merged K(1) between steps.  Order 4 (Yoshida composition of three
+// Strang steps of lengths w1, w0, w1): w1 = 1/(2 - 2^(1/3)), w0 = 1 - 2 w1.
+constexpr double YW1 = 1.3512071919596576340476878089715, YW0 = 1.0 - 2.0 * YW1;
+enum { PH_FULL = 0, PH_HALF, PH_Y_END, PH_Y_MID, PH_Y_JOIN, PH_SLOTS };
+const double PH_LEN[PH_SLOTS] = {1.0, 0.5, 0.5 * YW1, 0.5 * (YW1 + YW0), YW1};
+enum { NL_MAIN = 0, NL_Y1, NL_Y0, NL_SLOTS };
+const double NL_LEN[NL_SLOTS] = {1.0, YW1, YW0};
+
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
 // supported line lengths: 2^n in [64, 4096] and 6*4^a (96, 384, 1536); keep in step with build.py LENGTHS
@@ -50,7 +59,7 @@ struct Layout {
     int ndim;
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
-    size_t off_psi, off_hs, off_phi, off_vext, off_beta, off_gamma, off_tw[3], off_ph_full[3], off_ph_half[3], off_ksq[3], off_kother, off_diag, total;
+    size_t off_psi, off_hs, off_phi, off_vext, off_beta, off_gamma, off_tw[3], off_ph[5][3], off_ksq[3], off_kother, off_diag, total;
 };
 
 bool make_layout(int ndim, const int64_t *dims, Layout &L)
@@ -77,8 +86,7 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L)
     L.off_gamma = o; o = align256(o + (size_t)L.cells * 4);
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
-        L.off_ph_full[d] = o; o = align256(o + (size_t)L.n[d] * 16);
-        L.off_ph_half[d] = o; o = align256(o + (size_t)L.n[d] * 16);
+        for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
         L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
     }
     L.off_kother = o; o = align256(o + (size_t)L.hs_lines * 4);
@@ -124,7 +132,8 @@ struct sn_ctx {
     snk::NLParams nl;
     float2 *psi, *hs;
     float *phi;
-    const float4 *tw[3], *ph_full[3], *ph_half[3];
+    const float4 *tw[3], *ph[5][3]; // kinetic phase tables per slot (PH_*) and axis
+    snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
     const float *ksq[3], *kother;
     double *diag;
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
@@ -332,30 +341,35 @@ int upload_phase_tables(sn_ctx *c)
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
         const int64_t n = l.n[d];
-        std::vector<f4> full(n), half(n);
-        for (int64_t k = 0; k < n; k++) {
-            const double kk = kval(k, n, c->L[d]);
-            const double th = c->A * kk * kk * c->dtau;
-            full[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
-            half[k] = split_hilo(std::cos(0.5 * th) / (double)n, std::sin(0.5 * th) / (double)n);
+        std::vector<f4> tab(n);
+        for (int sl = 0; sl < PH_SLOTS; sl++) {
+            for (int64_t k = 0; k < n; k++) {
+                const double kk = kval(k, n, c->L[d]);
+                const double th = c->A * kk * kk * c->dtau * PH_LEN[sl];
+                tab[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
+            }
+            SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph[sl][d], tab.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
+            SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vector is rewritten in the next iteration
         }
-        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph_full[d], full.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
-        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph_half[d], half.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
-        SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vectors die at the end of this iteration
     }
-    c->nl.hb = (float)(-0.5 * c->dtau * c->B);
-    c->nl.flags = ((c->g_log != 0.0 || c->g_pow != 0.0) ? 1 : 0) | (c->has_vext ? 2 : 0);
-    c->nl.hlog = (float)(-0.5 * c->dtau * c->g_log);
-    c->nl.hpow = (float)(-0.5 * c->dtau * c->g_pow);
-    c->nl.floor_ = (float)c->rho_floor;
-    c->nl.ppow = (float)c->p_pow;
-    c->nl.hv = (float)(-0.5 * c->dtau);
-    c->nl.flog = (float)c->g_log;
-    c->nl.fpow = (float)(c->g_pow / (c->p_pow + 1.0));
-    for (int j = 0; j < 4; j++) {
-        c->nl.hg[j] = j < c->n_g ? (float)(-0.5 * c->dtau * c->g[j]) : 0.f;
-        c->nl.fg[j] = j < c->n_g ? (float)(c->g[j] / (double)(j + 2)) : 0.f;
+    for (int sl = 0; sl < NL_SLOTS; sl++) {
+        snk::NLParams &nl = c->nlv[sl];
+        const double h = -0.5 * c->dtau * NL_LEN[sl]; // half-angle factor of this sub-step
+        nl.hb = (float)(h * c->B);
+        nl.flags = ((c->g_log != 0.0 || c->g_pow != 0.0) ? 1 : 0) | (c->has_vext ? 2 : 0);
+        nl.hlog = (float)(h * c->g_log);
+        nl.hpow = (float)(h * c->g_pow);
+        nl.floor_ = (float)c->rho_floor;
+        nl.ppow = (float)c->p_pow;
+        nl.hv = (float)h;
+        nl.flog = (float)c->g_log;
+        nl.fpow = (float)(c->g_pow / (c->p_pow + 1.0));
+        for (int j = 0; j < 4; j++) {
+            nl.hg[j] = j < c->n_g ? (float)(h * c->g[j]) : 0.f;
+            nl.fg[j] = j < c->n_g ? (float)(c->g[j] / (double)(j + 2)) : 0.f;
+        }
     }
+    c->nl = c->nlv[NL_MAIN];
     return SN_OK;
 }
 
@@ -434,8 +448,10 @@ void set_axis_geometry(const sn_ctx *c, PassArgs &a, int axis, int64_t n0)
 }
 
 // one kinetic sweep over all axes; with_nl fuses the nonlinear phase (and the c2r of phi^) into axis 0
-// before_n: the sweep is followed by an N sub-step (the external-potential phase may ride on its last pass)
-int kinetic_sweep(sn_ctx *c, bool half, bool with_nl, bool before_n)
+// ph_slot: which kinetic phase table (PH_*); with_nl: the axis-0 pass first applies the nonlinear phase of the N
+// sub-step just solved, with the coefficients of nl_slot; before_n / next_nl_slot: the sweep is followed by an N
+// sub-step of that slot (the external-potential phase of THAT sub-step may ride on the sweep's last pass)
+int kinetic_sweep(sn_ctx *c, int ph_slot, bool with_nl, bool before_n, int nl_slot = NL_MAIN, int next_nl_slot = NL_MAIN)
 {
     const Layout &l = c->lay;
     int rc;
@@ -444,13 +460,17 @@ int kinetic_sweep(sn_ctx *c, bool half, bool with_nl, bool before_n)
         a.data = c->psi;
         a.hs = c->hs;
         a.tw = c->tw[d];
-        a.phase = half ? c->ph_half[d] : c->ph_full[d];
+        a.phase = c->ph[ph_slot][d];
+        a.nl = c->nlv[nl_slot];
         if (c->v_in_xkin) a.nl.flags &= ~2; // the axis-0 pass leaves V to the contiguous pass
         a.vext = nullptr;
         if (d == l.ndim - 1) {
             a.kind = snk::P_X_KIN;
             a.nlines = (int)(l.cells / l.nx);
-            if (c->v_in_xkin && before_n) a.vext = c->vext;
+            if (c->v_in_xkin && before_n) {
+                a.vext = c->vext;
+                a.nl.hv = c->nlv[next_nl_slot].hv;
+            }
         } else {
             a.kind = (d == 0 && with_nl) ? snk::P_H_NLKIN : snk::P_S_KIN;
             if (a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin) a.vext = c->vext;
@@ -523,7 +543,7 @@ int build_step_graph(sn_ctx *c)
     SN_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->cap_stream;
     int rc = potential_spectrum(c);
-    if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/false, /*with_nl=*/true, /*before_n=*/true);
+    if (rc == SN_OK) rc = kinetic_sweep(c, PH_FULL, /*with_nl=*/true, /*before_n=*/true);
     c->stream = user;
     cudaGraph_t g = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
@@ -607,8 +627,7 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
     c->rho_floor = 1e-30; c->p_pow = 1.0;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
-        c->ph_full[d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph_full[d]);
-        c->ph_half[d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph_half[d]);
+        for (int sl = 0; sl < PH_SLOTS; sl++) c->ph[sl][d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph[sl][d]);
         c->ksq[d] = reinterpret_cast<const float *>(c->ws + l.off_ksq[d]);
     }
     c->kother = reinterpret_cast<const float *>(c->ws + l.off_kother);
@@ -733,7 +752,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
     // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
-    int rc = kinetic_sweep(c, /*half=*/true, /*with_nl=*/false, /*before_n=*/true);
+    int rc = kinetic_sweep(c, PH_HALF, /*with_nl=*/false, /*before_n=*/true);
     int64_t i = 1;
     if (rc == SN_OK && c->use_graph && !c->profiling && nsteps >= 4) {
         if (!c->step_graph) rc = build_step_graph(c);
@@ -744,7 +763,27 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     }
     for (; rc == SN_OK && i <= nsteps; i++) {
         rc = potential_spectrum(c);
-        if (rc == SN_OK) rc = kinetic_sweep(c, /*half=*/i == nsteps, /*with_nl=*/true, /*before_n=*/i < nsteps);
+        if (rc == SN_OK) rc = kinetic_sweep(c, i == nsteps ? PH_HALF : PH_FULL, /*with_nl=*/true, /*before_n=*/i < nsteps);
+    }
+    return rc;
+}
+
+int sn_step_order4(sn_ctx *c, int64_t nsteps)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    if (nsteps < 0) return SN_ERR_PARAM;
+    if (nsteps == 0) return SN_OK;
+    // one step = S2(w1 h) S2(w0 h) S2(w1 h) with S2 the Strang step; adjacent kinetic halves merged:
+    // K(w1/2) [N(w1) K((w1+w0)/2) N(w0) K((w0+w1)/2) N(w1) K(w1 or w1/2)]^n
+    int rc = kinetic_sweep(c, PH_Y_END, /*with_nl=*/false, /*before_n=*/true, NL_MAIN, NL_Y1);
+    for (int64_t i = 1; rc == SN_OK && i <= nsteps; i++) {
+        rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = kinetic_sweep(c, PH_Y_MID, true, true, NL_Y1, NL_Y0);
+        if (rc == SN_OK) rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = kinetic_sweep(c, PH_Y_MID, true, true, NL_Y0, NL_Y1);
+        if (rc == SN_OK) rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = kinetic_sweep(c, i == nsteps ? PH_Y_END : PH_Y_JOIN, true, /*before_n=*/i < nsteps, NL_Y1, NL_Y1);
     }
     return rc;
 }

@@ -23,7 +23,7 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG", "H_SRC")
@@ -59,6 +59,7 @@ def lib() -> ctypes.CDLL:
                                 ctypes.c_size_t, vp]
         L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_step.argtypes = [vp, ctypes.c_int64]
+        L.sn_step_order4.argtypes = [vp, ctypes.c_int64]
         L.sn_get_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_diagnostics.argtypes = [vp, ctypes.POINTER(SnDiag)]
         L.sn_set_dtau.argtypes = [vp, ctypes.c_double]
@@ -169,6 +170,10 @@ class Simulation:
     def step(self, n: int) -> None:
         _chk(lib().sn_step(self._h, int(n)), "sn_step")
 
+    def step_order4(self, n: int) -> None:
+        """n fourth-order steps (Yoshida composition of three Strang steps each)."""
+        _chk(lib().sn_step_order4(self._h, int(n)), "sn_step_order4")
+
     def set_dtau(self, dtau: float) -> None:
         _chk(lib().sn_set_dtau(self._h, float(dtau)), "sn_set_dtau")
 
@@ -197,18 +202,18 @@ class Simulation:
         """eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); numpy float32 arrays or CUDA float32
         tensors of shape dims; (None, None) restores eq. (2)."""
         if beta is None and gamma is None:
-            _chk(lib().sn_set_source_tables(self._h, None, None, 0), "sn_set_source_tables")
+            _chk(lib().sn_set_source_tables(self._h, None, None, 0), "sn_set_source_tables", "sn_step_order4")
         elif isinstance(beta, np.ndarray):
             b = np.ascontiguousarray(beta, dtype=np.float32)
             g = np.ascontiguousarray(gamma, dtype=np.float32)
             assert b.shape == self.dims and g.shape == self.dims
             _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
-                 "sn_set_source_tables")
+                 "sn_set_source_tables", "sn_step_order4")
         else:
             assert beta.is_cuda and gamma.is_cuda and beta.is_contiguous() and gamma.is_contiguous()
             assert tuple(beta.shape) == self.dims and tuple(gamma.shape) == self.dims
             _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(beta.data_ptr()),
-                                            ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables")
+                                            ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables", "sn_step_order4")
 
     def diagnostics(self) -> dict:
         d = SnDiag()

@@ -174,3 +174,51 @@ def test_w5_position_dependent_source_closed_form(dims, C):
     o.set_source_tables(None, None)
     assert np.abs(a - o.potential()).max() < 1e-13
     o.close()
+
+
+# ------------------------------------------------------------------ W6 fourth-order composition
+
+def test_w6_order4_self_convergence_and_invariants():
+    """Halving dtau must reduce the error 16-fold (order 4), against 4-fold for the Strang step; the composition is
+    still unitary (norm), time-reversible, and exact on a plane wave."""
+    dims, L = (64, 64), 20.0
+    cfg = inputs.scaled(inputs.CONFIGS["C1"], dims, L=L)
+    psi0 = cfg.initial_state().astype(np.complex128) * 6.0        # strong self-gravity: splitting error well above roundoff
+    T = 0.4
+
+    def run(order, dtau):
+        o = Oracle(dims, L, -0.5, 1.0, 0.0, 1.0, (0.05,), dtau)
+        o.set_state(psi0)
+        n = int(round(T / dtau))
+        (o.step_order4 if order == 4 else o.step)(n)
+        out, d = o.get_state(), o.diagnostics()
+        o.close()
+        return out, d
+
+    ref, _ = run(4, T / 640)
+    e4 = [rel(run(4, T / n)[0], ref) for n in (10, 20, 40)]
+    e2 = [rel(run(2, T / n)[0], ref) for n in (10, 20, 40)]
+    assert 13.0 < e4[0] / e4[1] < 19.0 and 13.0 < e4[1] / e4[2] < 19.0, e4
+    assert 3.6 < e2[1] / e2[2] < 4.4, e2
+    assert e4[2] < 0.01 * e2[2]
+    out, d = run(4, T / 20)
+    n0 = float((np.abs(psi0) ** 2).sum() * (L / 64) ** 2)
+    assert abs(d["norm"] - n0) < 1e-11 * n0
+    # time reversal
+    o = Oracle(dims, L, -0.5, 1.0, 0.0, 1.0, (0.05,), T / 20)
+    o.set_state(psi0)
+    o.step_order4(7)
+    o.set_dtau(-T / 20)
+    o.step_order4(7)
+    assert rel(o.get_state(), psi0) < 1e-11
+    o.close()
+    # plane wave: exact for any composition of exact sub-flows (w1 + w0 + w1 = 1)
+    X, Y = grid(dims, L)
+    q = 2 * np.pi / L * np.array([3, -2])
+    pw = 0.7 * np.exp(1j * (q[0] * X + q[1] * Y))
+    o = Oracle(dims, L, -0.5, 1.0, -1.0, 0.9, (0.2,), 3e-2)
+    o.set_state(pw)
+    o.step_order4(5)
+    rate = -0.5 * float(q @ q) - 1.0 * 0.9 * 0.49 / (-1.0) - 0.2 * 0.49
+    assert rel(o.get_state(), pw * np.exp(1j * rate * 5 * 3e-2)) < 1e-12
+    o.close()
