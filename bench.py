@@ -177,6 +177,8 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--order4", action="store_true",
+                    help="time sn_step_order4 (Yoshida composition of three Strang steps per step) instead of sn_step")
     ap.add_argument("--extras", action="store_true",
                     help="NEXT-1 row: also run with the pressure potential 0.02 ln(rho) (eq. (16)) and the "
                          "phi_C table of eq. (11) as external potential and the beta, gamma tables of eq. (12) "
@@ -230,8 +232,9 @@ def main():
         # eq. (12) with eq. (9),(10): gamma = (1 - f)/2, beta = lambda f/(r + r0)
         sim.set_source_tables((f / (rs + 2.0)).astype(np.float32), (0.5 * (1.0 - f)).astype(np.float32))
         del rs, f, r2
+    step = sim.step_order4 if args.order4 else sim.step
     sim.set_state(dev_in)
-    sim.step(W)                                         # untimed warm-up steps
+    step(W)                                             # untimed warm-up steps
     barrier()
 
     # ---- timed region: exactly K Strang steps, state resident in HBM ----
@@ -240,7 +243,7 @@ def main():
     with ClockSampler(local) as clk:
         barrier()
         e0.record(stream)
-        sim.step(K)
+        step(K)
         e1.record(stream)
         barrier()
     launches = sim.launch_count() - n0
@@ -248,7 +251,7 @@ def main():
 
     # ---- per-launch CUDA events over the same K steps (roofline of the dominant kernel) ----
     sim.profile(True)
-    sim.step(K)
+    step(K)
     prof = sim.profile_read(reset=True)
     sim.profile(False)
     norm_after = sim.diagnostics()["norm"]
@@ -257,7 +260,7 @@ def main():
     barrier()
     t0 = time.perf_counter()
     sim.set_state(host_in)
-    sim.step(K)
+    step(K)
     sim.get_state(host_out)
     d = sim.diagnostics()
     torch.cuda.synchronize()
@@ -293,7 +296,7 @@ def main():
                        "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
                            cells, cells * 8 / 2 ** 20) if cells * 8 > 126e6 else
                        "state fits L2: launch/L2-bound regime, HBM fraction is an effective figure only",
-                       "timed_call": f"one sn_step({K}) (merged half kinetics)"},
+                       "timed_call": f"one {'sn_step_order4' if args.order4 else 'sn_step'}({K}) (merged half kinetics)"},
             "gpu_launches": launches,
             "clocks": clk.summary(),
             "roofline": {

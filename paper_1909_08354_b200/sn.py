@@ -202,18 +202,18 @@ class Simulation:
         """eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); numpy float32 arrays or CUDA float32
         tensors of shape dims; (None, None) restores eq. (2)."""
         if beta is None and gamma is None:
-            _chk(lib().sn_set_source_tables(self._h, None, None, 0), "sn_set_source_tables", "sn_step_order4")
+            _chk(lib().sn_set_source_tables(self._h, None, None, 0), "sn_set_source_tables")
         elif isinstance(beta, np.ndarray):
             b = np.ascontiguousarray(beta, dtype=np.float32)
             g = np.ascontiguousarray(gamma, dtype=np.float32)
             assert b.shape == self.dims and g.shape == self.dims
             _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
-                 "sn_set_source_tables", "sn_step_order4")
+                 "sn_set_source_tables")
         else:
             assert beta.is_cuda and gamma.is_cuda and beta.is_contiguous() and gamma.is_contiguous()
             assert tuple(beta.shape) == self.dims and tuple(gamma.shape) == self.dims
             _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(beta.data_ptr()),
-                                            ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables", "sn_step_order4")
+                                            ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables")
 
     def diagnostics(self) -> dict:
         d = SnDiag()

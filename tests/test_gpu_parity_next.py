@@ -165,3 +165,56 @@ def test_source_tables_steps_match_oracle(mods, name, dims, L, steps):
     assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
     for k in ("e_kin", "e_nonlocal", "e_local"):
         assert abs(d1[k] - r1[k]) < 2e-5 * max(abs(r1["e_total"]), abs(r1[k])), (k, d1[k], r1[k])
+
+
+# ------------------------------------------------------------------ fourth-order composition
+
+@pytest.mark.parametrize("name,dims,L,steps,extras", [
+    ("C2", (256, 256), 25.0, 100, False),
+    ("C4", (64, 128, 64), 16.0, 40, False),
+    ("C5_384", (96, 64, 128), 128.0, 10, False),
+    ("C2", (128, 256), 25.0, 60, True),            # with the full NMC model: external potential rides on the right sub-step
+])
+def test_order4_steps_match_oracle(mods, name, dims, L, steps, extras):
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=steps)
+    psi0 = cfg.initial_state()
+    sim = sn.Simulation.from_config(cfg)
+    orc = Oracle.from_config(cfg)
+    if extras:
+        beta, gamma = nmc_tables(dims, L)
+        V = nmc_potential(dims, L).astype(np.float32)
+        sim.set_local_terms(0.05, 1e-12, 0.03, 0.5)
+        sim.set_external_potential(V)
+        sim.set_source_tables(beta, gamma)
+        orc.set_local_terms(0.05, 1e-12, 0.03, 0.5)
+        orc.set_external_potential(V.astype(np.float64))
+        orc.set_source_tables(beta.astype(np.float64), gamma.astype(np.float64))
+    sim.set_state(psi0)
+    d0 = sim.diagnostics()
+    sim.step_order4(steps // 2)
+    sim.step_order4(steps - steps // 2)                       # split calls: the end sweeps are half sweeps
+    got = sim.get_state()
+    d1 = sim.diagnostics()
+    sim.close()
+    orc.set_state(psi0.astype(np.complex128))
+    orc.step_order4(steps)
+    want = orc.get_state()
+    orc.close()
+    assert rel(got, want) < TOL_STATE
+    assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
+
+
+def test_order4_differs_from_order2_by_the_splitting_error(mods):
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C2"], (128, 128), L=25.0, steps=40)
+    psi0 = cfg.initial_state()
+    sim = sn.Simulation(cfg.dims, cfg.L, cfg.A, cfg.B, cfg.C, cfg.D, cfg.g, 2e-2)
+    sim.set_state(psi0)
+    sim.step(40)
+    a = sim.get_state()
+    sim.set_state(psi0)
+    sim.step_order4(40)
+    b = sim.get_state()
+    sim.close()
+    assert 1e-6 < rel(a, b) < 1e-2
