@@ -10,7 +10,10 @@
 #include <cstdlib>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <set>
+#include <utility>
 #include <vector>
 
 namespace {
@@ -113,6 +116,26 @@ inline double kval(int64_t j, int64_t n, double L)
 }
 
 } // namespace
+
+namespace snk {
+// kernels whose dynamic-shared-memory limit has been raised, per device (key = device id, kernel address)
+static std::mutex g_attr_mu;
+static std::set<std::pair<int, const void *>> g_attr_set;
+bool smem_attr_done(const void *kernel)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lk(g_attr_mu);
+    return g_attr_set.count({dev, kernel}) != 0;
+}
+void smem_attr_mark(const void *kernel)
+{
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lk(g_attr_mu);
+    g_attr_set.insert({dev, kernel});
+}
+} // namespace snk
 
 struct sn_ctx {
     Layout lay;

@@ -351,9 +351,11 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
 template <class K>
 static int launch_kernel(K kern, unsigned grid, int threads, size_t smem_bytes, const PassArgs &a)
 {
-    if (smem_bytes > 40 * 1024) { // static shared memory (block_accumulate) counts against the 48 KB default too
+    // static shared memory (block_accumulate) counts against the 48 KB default too
+    if (smem_bytes > 40 * 1024 && !smem_attr_done(reinterpret_cast<const void *>(kern))) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
         if (e != cudaSuccess) return (int)e;
+        smem_attr_mark(reinterpret_cast<const void *>(kern));
     }
     kern<<<grid, threads, smem_bytes, a.stream>>>(a);
     return (int)cudaGetLastError();

@@ -63,6 +63,11 @@ struct PassArgs {
     cudaStream_t stream;
 };
 
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is needed once per kernel and device, not per launch
+// (it costs ~1 us of host time per call); the set of kernels already configured lives in sn_api.cu.
+bool smem_attr_done(const void *kernel);
+void smem_attr_mark(const void *kernel);
+
 // Returns cudaError_t as int.  Explicitly instantiated for N in {64,...,4096}.
 template <int N>
 int launch_pass(const PassArgs &a);

@@ -609,8 +609,11 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
 template <class K>
 static int launch_pipe_kernel(K kern, int threads, size_t smem_bytes, const PipeArgs &a)
 {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
-    if (e != cudaSuccess) return (int)e;
+    if (!smem_attr_done(reinterpret_cast<const void *>(kern))) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes);
+        if (e != cudaSuccess) return (int)e;
+        smem_attr_mark(reinterpret_cast<const void *>(kern));
+    }
     kern<<<a.grid, threads, smem_bytes, a.a.stream>>>(a);
     return (int)cudaGetLastError();
 }
