@@ -161,6 +161,7 @@ struct sn_ctx {
     double *diag;
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
     bool use_pipe;
+    bool pipe_all;  // SN_PIPE_ALL=1: pipelined kernels wherever they are instantiated (tests, A/B runs)
     int sm_count;
     CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row;
     bool m_ok[2];
@@ -303,7 +304,11 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         const int axis = strided ? a.axis : 0;
         const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
                           !(a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin); // then the first-path kernel reads V
-        if (maps && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
+        // which kinds gain from the pipeline depends on the line length (measured): the heavy axis-0
+        // pass always; the others at N = 512 and N >= 2048 (N <= 256 and N = 1024: two first-path CTAs per SM win)
+        const bool worth = a.kind == snk::P_H_NLKIN || c->pipe_all || N == 512 || N >= 2048 ||
+                           (a.kind == snk::P_X_KIN && a.vext != nullptr); // V rides on the pipelined contiguous pass
+        if (maps && worth && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
             pa.a = a;
@@ -661,6 +666,8 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
         int dev = 0;
         const char *ng = std::getenv("SN_NO_GRAPH"); // SN_NO_GRAPH=1: plain stream launches for every grid
         c->use_graph = l.cells <= ((int64_t)1 << 24) && !(ng && ng[0] == '1');
+        const char *pa = std::getenv("SN_PIPE_ALL");
+        c->pipe_all = pa && pa[0] == '1';
         const char *np = std::getenv("SN_NO_PIPE"); // SN_NO_PIPE=1: first-path kernels only (A/B runs, tests)
         c->use_pipe = !(np && np[0] == '1');
         if (cudaGetDevice(&dev) != cudaSuccess ||

@@ -327,6 +327,7 @@ def test_first_path_and_pipelined_kernels_agree(mods, dims, L, name, monkeypatch
     cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=6)
     psi0 = cfg.initial_state()
     out = {}
+    monkeypatch.setenv("SN_PIPE_ALL", "1")               # mode "0": every kind on the pipelined kernels
     for mode in ("0", "1"):
         monkeypatch.setenv("SN_NO_PIPE", mode)
         sim = sn.Simulation.from_config(cfg)
@@ -341,3 +342,16 @@ def test_first_path_and_pipelined_kernels_agree(mods, dims, L, name, monkeypatch
     orc.close()
     assert rel(out["0"], want) < TOL_STATE and rel(out["1"], want) < TOL_STATE
     assert rel(out["0"], out["1"]) < 5e-6
+
+
+@pytest.mark.parametrize("name,dims,L,steps", [("C2", (256, 128), 25.0, 50), ("C4", (64, 128, 256), 32.0, 10),
+                                               ("C5_64", (64, 64, 64), 128.0, 20), ("C2", (1024, 64), 25.0, 10)])
+def test_steps_match_oracle_all_pipelined(mods, name, dims, L, steps, monkeypatch):
+    """The default dispatch uses the pipelined kernels only where they are faster (axis-0 nonlinear pass always,
+    the others at N = 512 and N >= 2048); SN_PIPE_ALL=1 forces them for every kind and length."""
+    monkeypatch.setenv("SN_PIPE_ALL", "1")
+    snref, Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=steps)
+    got, want, sim = run_pair(mods, cfg, steps)
+    sim.close()
+    assert rel(got, want) < TOL_STATE
