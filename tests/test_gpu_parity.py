@@ -355,3 +355,26 @@ def test_steps_match_oracle_all_pipelined(mods, name, dims, L, steps, monkeypatc
     got, want, sim = run_pair(mods, cfg, steps)
     sim.close()
     assert rel(got, want) < TOL_STATE
+
+
+def test_graph_replay_is_bitwise_the_stream_launch_path(mods, monkeypatch):
+    """sn_step(n >= 4) on grids of <= 2^24 cells replays a captured CUDA graph of the interior step; the kernels and
+    their order are the same as with plain stream launches (SN_NO_GRAPH=1), so the states must agree bit for bit, also
+    after sn_set_dtau (which drops the graph) and across split calls."""
+    snref, Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C4"], (64, 64, 128), L=16.0, steps=12)
+    psi0 = cfg.initial_state()
+    out = {}
+    for mode in ("0", "1"):
+        monkeypatch.setenv("SN_NO_GRAPH", mode)
+        sim = sn.Simulation.from_config(cfg)
+        sim.set_state(psi0)
+        n0 = sim.launch_count()
+        sim.step(7)
+        sim.set_dtau(0.5 * cfg.dtau)
+        sim.step(5)
+        sim.step(2)                                   # below the graph threshold: plain launches in both modes
+        out[mode] = (sim.get_state(), sim.launch_count() - n0)
+        sim.close()
+    assert np.array_equal(out["0"][0], out["1"][0])
+    assert out["0"][1] == out["1"][1]                 # the launch counter counts the kernels inside the graph too
