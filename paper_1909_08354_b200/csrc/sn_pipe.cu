@@ -10,13 +10,17 @@
 // lines), completion is tracked with mbarriers, and the butterflies of tile k run while tile
 // k+1/k+2 are landing and tile k-1 is draining.  No register is spent on global addresses.
 //
-// Tile geometry (strided kinds): T = N/8 threads carry one PAIR of adjacent columns (a "line
-// pair", one float4 = 2 complex per row); G = 512/T groups per CTA; a tile is N rows x 2G
-// columns, stored as G/8 sub-tiles of [N rows][128 B].  In a sub-tile the TMA 128B swizzle puts
-// the 16-byte chunk c of row r at chunk c ^ (r & 7): the 8 lanes of a quarter-warp (consecutive
-// rows, same column pair) hit 8 different bank groups, so every 128-bit access is conflict-free.
-// A group only ever touches its own N slots (one per row), so the Stockham exchanges of its FFT
-// run IN PLACE in the tile, position pos living in the slot of row pos ^ ((pos >> 3) & 7).
+// Tile geometry (strided kinds): T = N/P threads carry one PAIR of adjacent columns (a "line pair", one float4 =
+// 2 complex per row; P = 8 points per thread, 12 for N = 6*4^a); G = threads/T groups per CTA; a tile is N rows x
+// 2G columns, stored as sub-tiles of [N rows][16*CPW bytes], CPW = min(G, 8) column pairs per row.  The TMA
+// swizzle of that width (128B / 64B / 32B / none) puts the 16-byte chunk c of row r at chunk c ^ swz(r), and in
+// every case the bank unit is a bijection of (r & 7): the 8 lanes of a quarter-warp (consecutive rows, same
+// column pair) hit 8 different bank groups, so every 128-bit access is conflict-free.  A group only ever touches
+// its own N slots (one per row), so the Stockham exchanges of its FFT run IN PLACE in the tile, position pos
+// living in the slot of row pos ^ ((pos >> 3) & 7).
+//
+// Which passes actually run these kernels is decided per line length in sn_api.cu (run_pass_raw): measured, the
+// axis-0 nonlinear pass always, the other kinds at N = 512 and N >= 2048.
 #include "sn_fft_core.cuh"
 #include "sn_launch.h"
 #include "sn_pointwise.cuh"
