@@ -177,6 +177,9 @@ def main():
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--batch", type=int, default=0,
+                    help="2D workloads only: an ensemble of this many independent systems in one context "
+                         "(sn_create_batch2d; every member a shifted, rescaled copy of the workload's state)")
     ap.add_argument("--order4", action="store_true",
                     help="time sn_step_order4 (Yoshida composition of three Strang steps per step) instead of sn_step")
     ap.add_argument("--extras", action="store_true",
@@ -214,12 +217,19 @@ def main():
     nd = len(cfg.dims)
     K, W = args.steps, args.warmup
     psi0 = cfg.initial_state()                          # seeded synthetic state, complex64
+    if args.batch:
+        assert nd == 2, "--batch needs a 2D workload"
+        rng = np.random.default_rng(1)
+        mem = [np.roll(psi0, (int(rng.integers(cfg.dims[0])), int(rng.integers(cfg.dims[1]))), axis=(0, 1)) *
+               np.complex64(0.8 + 0.4 * b / args.batch) for b in range(args.batch)]
+        psi0 = np.ascontiguousarray(np.stack(mem, axis=1).astype(np.complex64))   # storage layout [n0][batch][n1]
+        del mem
     host_in = torch.from_numpy(psi0).pin_memory()
     host_out = torch.empty_like(host_in).pin_memory()
     dev_in = host_in.to(dev, non_blocking=True)
 
     stream = torch.cuda.current_stream()
-    sim = sn.Simulation.from_config(cfg, device=dev, stream=stream)
+    sim = sn.Simulation.from_config(cfg, device=dev, stream=stream, batch=args.batch or None)
     if args.extras:
         # eq. (16) n = 1: V_pressure = w ln(rho), w = 0.02; eq. (11): phi_C = ln[1 - (r0/(r + r0))^lambda], lambda = 1,
         # r0 = 2, radius softened to sqrt(r^2 + 1) (the grid has a point at r = 0)
@@ -271,7 +281,7 @@ def main():
     ms, e2e_ms = replicas.max_over_ranks([ms, e2e_s * 1e3], device=dev)
 
     if rank == 0:
-        cells = cfg.cells
+        cells = cfg.cells * max(1, args.batch)
         value = replicas.whole_job_rate(cells, K, world, ms)
         peak, peak_src = load_peaks()
         tot = sum(v[0] for v in prof.values()) or 1.0
@@ -290,7 +300,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
-            "config": {"workload": f"{cfg.name}{'+next1(0.02 ln rho, phi_C, beta/gamma tables of eq. (12))' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
+            "config": {"workload": f"{cfg.name}{' x%d ensemble' % args.batch if args.batch else ''}{'+next1(0.02 ln rho, phi_C, beta/gamma tables of eq. (12))' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
                                    f"B={cfg.B}, C={cfg.C}, D={cfg.D:.6g}, g={list(cfg.g)}, dtau={cfg.dtau}",
                        "dims": list(cfg.dims), "parallelism": "replicas only" if world > 1 else "single GPU",
                        "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (

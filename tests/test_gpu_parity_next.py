@@ -218,3 +218,52 @@ def test_order4_differs_from_order2_by_the_splitting_error(mods):
     b = sim.get_state()
     sim.close()
     assert 1e-6 < rel(a, b) < 1e-2
+
+
+# ------------------------------------------------------------------ ensembles of 2D systems
+
+@pytest.mark.parametrize("dims,batch,steps", [((128, 128), 8, 60), ((64, 256), 3, 40), ((512, 64), 4, 12), ((96, 128), 5, 20)])
+def test_batch2d_members_match_single_system_oracle(mods, dims, batch, steps):
+    """An ensemble context advances every member exactly like a single-system run: compare each member with the
+    float64 oracle run on that member alone, and the ensemble diagnostics with the sum of the members'."""
+    Oracle, inputs, sn = mods
+    L = 25.0
+    base = inputs.scaled(inputs.CONFIGS["C2"], dims, L=L, steps=steps)
+    rng = np.random.default_rng(11)
+    members = []
+    for b in range(batch):                                # same recipe, each member rotated/scaled differently
+        psi = np.roll(base.initial_state(), (int(rng.integers(dims[0])), int(rng.integers(dims[1]))), axis=(0, 1))
+        members.append((psi * np.complex64(0.6 + 0.1 * b)).astype(np.complex64))
+    store = np.ascontiguousarray(np.stack(members, axis=1))          # storage layout [n0][batch][n1]
+    sim = sn.Simulation(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau, batch=batch)
+    assert sim.dims == (dims[0], batch, dims[1])
+    sim.set_state(store)
+    d0 = sim.diagnostics()
+    sim.step(steps)
+    got = sim.get_state()
+    d1 = sim.diagnostics()
+    sim.close()
+    tot = {k: 0.0 for k in d1}
+    for b in range(batch):
+        orc = Oracle(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau)
+        orc.set_state(members[b].astype(np.complex128))
+        orc.step(steps)
+        assert rel(got[:, b, :], orc.get_state()) < TOL_STATE, b
+        r = orc.diagnostics()
+        for k in tot:
+            tot[k] += r[k]
+        orc.close()
+    assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
+    for k in tot:
+        assert abs(d1[k] - tot[k]) < 2e-5 * max(abs(tot["e_total"]), abs(tot[k])), (k, d1[k], tot[k])
+
+
+def test_batch2d_validation(mods):
+    Oracle, inputs, sn = mods
+    from paper_1909_08354_b200.sn import lib
+    import ctypes
+    d = (ctypes.c_int64 * 2)(128, 128)
+    assert lib().sn_workspace_bytes_batch2d(d, 0) == 0
+    assert lib().sn_workspace_bytes_batch2d(d, 7) > 7 * 128 * 128 * 8
+    bad = (ctypes.c_int64 * 2)(100, 128)
+    assert lib().sn_workspace_bytes_batch2d(bad, 4) == 0
