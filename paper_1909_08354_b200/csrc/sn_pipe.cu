@@ -561,6 +561,10 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
             }
             if (MODE == P_X_KIN) {
                 fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+                if (NST == 2 && tid == 0 && k >= 1 && k + 1 < nk) { // reload the stage tile k-1 was stored from
+                    bulk_wait_read<0>();
+                    issue_load(k + 1);
+                }
                 apply_phase<T, P>(a, c, jf, p.a.phase);
                 fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
                 if (VEXT) {
@@ -598,11 +602,12 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
             mbar_wait(done + b, par);
             bulk_store_1d(p.a.data + line0 * N, base + b * STAGE_BYTES, (uint32_t)nl * N * 8);
             bulk_commit();
-            if (k + 2 < nk) {
-                if (NST == 3) bulk_wait_read<1>(); // tile k+2 goes where tile k-1 was stored from
-                else bulk_wait_read<0>();          // two stages: tile k+2 reuses this stage
+            if (NST == 3 && k + 2 < nk) {
+                bulk_wait_read<1>(); // tile k+2 goes where tile k-1 was stored from
                 issue_load(k + 2);
             }
+            // two stages (VEXT): tile k+2 reuses THIS stage; it is reloaded from inside tile k+1's compute (below),
+            // when this store has long drained, so the issuer never waits for it
         }
     }
     if (tid == 0) bulk_wait<0>();
