@@ -100,7 +100,7 @@ int sn_get_state(sn_ctx *ctx, void *psi_out, int dst_on_device);
 /* Norm and energy of the current state (host struct).  Synchronises; the state is unchanged. */
 int sn_diagnostics(sn_ctx *ctx, sn_diag *out);
 
-/* Replace dtau (rebuilds the kinetic phase tables). */
+/* Replace dtau (rebuilds the kinetic phase tables and the nonlinear coefficients; synchronises the stream). */
 int sn_set_dtau(sn_ctx *ctx, double dtau);
 
 /* ---- NEXT-1 terms of the local potential (eq. (15),(16)) ----
@@ -109,7 +109,8 @@ int sn_set_dtau(sn_ctx *ctx, double dtau);
  *   the paper does not say how ln(0) is avoided), p_pow != -1.  g_log = g_pow = 0 switches the terms off.
  * sn_set_external_potential: a fixed real potential V(x) (float32, prod(dims) values, layout of psi; host or
  *   device pointer, copied into the workspace) enters the N sub-step as exp(-i s (B phi + G(rho) + V)) -- phi_C
- *   of eq. (11),(15).  NULL removes it.  With V set the axis-0 nonlinear pass runs the first-path kernel.
+ *   of eq. (11),(15).  NULL removes it.  exp(-i s V) commutes with the rest of the N phase, so it is applied by the
+ *   contiguous-axis kinetic pass that precedes each N sub-step (by the axis-0 pass when that one is first-path).
  * Both rebuild the nonlinear-phase coefficients; e_local of sn_diagnostics then includes sum (F(rho) + V rho) dV. */
 /* sn_set_source_tables: eq. (12), PAPER.md:92 -- lap phi + C phi = D (gamma(x) rho + beta(x) lap rho) instead of
  *   eq. (2).  beta, gamma: float32, prod(dims) values each, layout of psi, host or device (copied into the
@@ -140,7 +141,7 @@ int64_t sn_launch_count(const sn_ctx *ctx);
  *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12)) */
 #define SN_NUM_PASS_KINDS 12
 int sn_profile(sn_ctx *ctx, int enable);
-int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 11 */, int64_t *launches_by_kind /* host, 11 */,
+int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 12 */, int64_t *launches_by_kind /* host, 12 */,
                     int reset);
 
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */
