@@ -267,3 +267,33 @@ def test_batch2d_validation(mods):
     assert lib().sn_workspace_bytes_batch2d(d, 7) > 7 * 128 * 128 * 8
     bad = (ctypes.c_int64 * 2)(100, 128)
     assert lib().sn_workspace_bytes_batch2d(bad, 4) == 0
+
+
+def test_batch2d_with_nmc_terms_and_order4(mods):
+    """Ensemble + every NEXT-1 term + the fourth-order step at once: the tables are per member, stored in the same
+    [n0][batch][n1] layout as the state."""
+    Oracle, inputs, sn = mods
+    dims, batch, L, steps = (128, 64), 3, 25.0, 16
+    base = inputs.scaled(inputs.CONFIGS["C2"], dims, L=L, steps=steps)
+    beta, gamma = nmc_tables(dims, L)
+    V = nmc_potential(dims, L).astype(np.float32)
+    members = [np.roll(base.initial_state(), 7 * b, axis=1) * np.complex64(0.7 + 0.1 * b) for b in range(batch)]
+    tabs = [(np.roll(beta, 3 * b, axis=0) * (1.0 + 0.2 * b), gamma * (1.0 - 0.1 * b), V * (1.0 + 0.5 * b)) for b in range(batch)]
+    st = lambda arrs, dt: np.ascontiguousarray(np.stack(arrs, axis=1).astype(dt))
+    sim = sn.Simulation(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau, batch=batch)
+    sim.set_local_terms(0.04, 1e-12, 0.03, 0.5)
+    sim.set_source_tables(st([t[0] for t in tabs], np.float32), st([t[1] for t in tabs], np.float32))
+    sim.set_external_potential(st([t[2] for t in tabs], np.float32))
+    sim.set_state(st(members, np.complex64))
+    sim.step_order4(steps)
+    got = sim.get_state()
+    sim.close()
+    for b in range(batch):
+        orc = Oracle(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau)
+        orc.set_local_terms(0.04, 1e-12, 0.03, 0.5)
+        orc.set_source_tables(tabs[b][0].astype(np.float32).astype(np.float64), tabs[b][1].astype(np.float32).astype(np.float64))
+        orc.set_external_potential(tabs[b][2].astype(np.float32).astype(np.float64))
+        orc.set_state(members[b].astype(np.complex64).astype(np.complex128))
+        orc.step_order4(steps)
+        assert rel(got[:, b, :], orc.get_state()) < TOL_STATE, b
+        orc.close()
