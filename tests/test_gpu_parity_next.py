@@ -297,3 +297,42 @@ def test_batch2d_with_nmc_terms_and_order4(mods):
         orc.step_order4(steps)
         assert rel(got[:, b, :], orc.get_state()) < TOL_STATE, b
         orc.close()
+
+
+# ------------------------------------------------------------------ full size, all terms: exact plane-wave solution
+
+@pytest.mark.parametrize("dims,C,order4", [((512, 512, 512), -1.0, False), ((256, 256, 256), -0.6, True),
+                                           ((4096, 2048), -1.0, False)])
+def test_plane_wave_full_size_with_next_terms(mods, dims, C, order4):
+    """At BASELINE.json's full sizes, in the launch configuration bench.py --extras times: a plane wave a e^{iq.x}
+    stays an exact solution with the logarithmic/power-law terms, a uniform external potential v0 and CONSTANT source
+    tables gamma = g0, beta = b0 (rho is uniform, so lap rho = 0 and phi0 = D g0 a^2/C):
+    psi(tau) = psi0 exp(i (A|q|^2 - B phi0 - G(a^2) - v0) tau), for the Strang and the order-4 step alike."""
+    Oracle, inputs, sn = mods
+    L, A, B, D, g, dtau, steps, amp = 32.0, -0.5, 1.3, 0.9, (0.2,), 5e-3, 12, 0.8
+    g_log, g_pow, p, v0, g0, b0 = 0.31, -0.45, 2.0 / 3.0, 0.37, 0.6, 0.25
+    nd = len(dims)
+    mode = (3, -2, 5)[:nd]
+    ax = [inputs.coords(n, L) for n in dims]
+    ph = sum((2 * np.pi / L * m) * a.reshape([-1 if i == k else 1 for i in range(nd)]) for k, (m, a) in enumerate(zip(mode, ax)))
+    psi0 = (amp * np.exp(1j * ph)).astype(np.complex64)
+    del ph
+    q2 = sum((2 * np.pi / L * m) ** 2 for m in mode)
+    sim = sn.Simulation(dims, L, A, B, C, D, g, dtau)
+    sim.set_local_terms(g_log, 1e-12, g_pow, p)
+    sim.set_external_potential(np.full(dims, v0, dtype=np.float32))
+    sim.set_source_tables(np.full(dims, b0, dtype=np.float32), np.full(dims, g0, dtype=np.float32))
+    sim.set_state(psi0)
+    (sim.step_order4 if order4 else sim.step)(steps)
+    got = sim.get_state()
+    sim.close()
+    a2 = amp * amp
+    omega = A * q2 - B * D * g0 * a2 / C - (g[0] * a2 + g_log * np.log(a2) + g_pow * a2 ** p) - v0
+    rot = complex(np.exp(1j * omega * dtau * steps))
+    num = den = 0.0
+    g1, p1 = got.reshape(-1), psi0.reshape(-1)
+    for i in range(0, g1.size, 1 << 24):
+        w = p1[i:i + (1 << 24)].astype(np.complex128) * rot
+        num += float(np.sum(np.abs(g1[i:i + (1 << 24)] - w) ** 2))
+        den += float(np.sum(np.abs(w) ** 2))
+    assert np.sqrt(num / den) < 2e-5
