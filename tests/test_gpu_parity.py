@@ -378,3 +378,30 @@ def test_graph_replay_is_bitwise_the_stream_launch_path(mods, monkeypatch):
         sim.close()
     assert np.array_equal(out["0"][0], out["1"][0])
     assert out["0"][1] == out["1"][1]                 # the launch counter counts the kernels inside the graph too
+
+
+def test_runs_on_a_side_stream(mods):
+    """All device work goes to the cudaStream_t given to sn_create: run on a non-default torch stream (graph replay
+    included) and compare with the default-stream result bit for bit."""
+    import torch
+    snref, Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C4"], (64, 128, 64), L=16.0, steps=9)
+    psi0 = cfg.initial_state()
+    ref = sn.Simulation.from_config(cfg)
+    ref.set_state(psi0)
+    ref.step(9)
+    want = ref.get_state()
+    ref.close()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        sim = sn.Simulation.from_config(cfg, stream=side)
+        dev = torch.from_numpy(psi0).to("cuda:0", non_blocking=True)
+        side.synchronize()
+        sim.set_state(dev)
+        sim.step(9)
+        out = torch.empty_like(dev)
+        sim.get_state(out)
+        side.synchronize()
+        got = out.cpu().numpy()
+        sim.close()
+    assert np.array_equal(got, want)
