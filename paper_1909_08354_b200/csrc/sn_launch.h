@@ -73,22 +73,21 @@ template <int N>
 int launch_pass(const PassArgs &a);
 
 // ---- pipelined (persistent, TMA-fed) variants of the hot passes: sn_pipe.cu ----
-// One 512-thread CTA per SM walks over 64 KB tiles; tiles are moved by the TMA unit between
-// HBM and a ring of shared-memory stages, so loads and stores of neighbouring tiles overlap the
-// butterflies of the current one.  Kinds served: P_S_FFT, P_S_KIN, P_H_NLKIN, P_H_R2C (N <= 512)
-// and P_X_KIN, P_X_POISSON (all N).  Tensor maps view an array as [outer][row][2*cols floats]
-// with 128-byte (16 complex) wide, 128B-swizzled boxes.
+// One CTA per SM (512 threads, 64 KB tiles for N = 2^n; 256 threads, 48 KB tiles for N = 6*4^a) walks over the
+// tiles of a pass; tiles are moved by the TMA unit between HBM and a ring of shared-memory stages, so loads and
+// stores of neighbouring tiles overlap the butterflies of the current one.  Kinds served: P_S_FFT, P_S_KIN,
+// P_H_NLKIN, P_H_R2C, P_X_KIN, P_X_POISSON.  Tensor maps view an array as [outer][row][2*cols floats]; a box is
+// 2*CPW complex wide (CPW = pipe_cpw(N) column pairs: 128, 64, 32 or 16 bytes) and swizzled over exactly that width.
 struct PipeArgs {
-    CUtensorMap m_data;   // psi (or the half spectrum for P_S_FFT): box {32 floats, min(N,256) rows, 1}
-    CUtensorMap m_hs;     // P_H_*: half spectrum [N/2+1 rows][2*cols floats]: box {32, N/2 rows, 1}
-    CUtensorMap m_hs_row; // P_H_*: same tensor, box {32, 1, 1} (the row N/2)
+    CUtensorMap m_data;   // psi (or the half spectrum for P_S_FFT): box {4*CPW floats, pipe_box_rows(N) rows, 1}
+    CUtensorMap m_hs;     // P_H_*: half spectrum [N/2+1 rows][2*cols floats]: box {4*CPW, pipe_box_rows(N/2) rows, 1}
+    CUtensorMap m_hs_row; // P_H_*: same tensor, box {4*CPW, 1, 1} (the row N/2)
     PassArgs a;
     int n_tiles;          // tiles of this pass
     int tiles_per_outer;  // strided kinds: column blocks per outer index
     int grid;             // CTAs to launch (<= number of SMs)
 };
 
-// true when launch_pipe<N> serves this kind/geometry (otherwise use launch_pass<N>)
 // geometry of the pipelined kernels, shared by the scheduler (tensor maps, tile counts) and sn_pipe.cu:
 // 8 points per thread and 512 threads for N = 2^n; 12 points per thread and 256 threads for N = 6*4^a
 __host__ __device__ constexpr int pipe_ppt(int N) { return N % 3 == 0 ? 12 : 8; }
@@ -102,6 +101,8 @@ __host__ __device__ constexpr int pipe_box_rows(int rows) // largest divisor of 
     return r;
 }
 
+// true when launch_pipe<N> can serve this kind/geometry (whether it is also the faster choice is decided per line
+// length in sn_api.cu); otherwise launch_pass<N>
 inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 {
     // 6*4^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
