@@ -178,8 +178,8 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=15.0, help="seconds of oracle work for cpu_baseline")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--batch", type=int, default=0,
-                    help="2D workloads only: an ensemble of this many independent systems in one context "
-                         "(sn_create_batch2d; every member a shifted, rescaled copy of the workload's state)")
+                    help="an ensemble of this many independent systems in one context (sn_create_batch; every "
+                         "member a shifted, rescaled copy of the workload's state)")
     ap.add_argument("--order4", action="store_true",
                     help="time sn_step_order4 (Yoshida composition of three Strang steps per step) instead of sn_step")
     ap.add_argument("--extras", action="store_true",
@@ -218,11 +218,10 @@ def main():
     K, W = args.steps, args.warmup
     psi0 = cfg.initial_state()                          # seeded synthetic state, complex64
     if args.batch:
-        assert nd == 2, "--batch needs a 2D workload"
         rng = np.random.default_rng(1)
-        mem = [np.roll(psi0, (int(rng.integers(cfg.dims[0])), int(rng.integers(cfg.dims[1]))), axis=(0, 1)) *
+        mem = [np.roll(psi0, tuple(int(rng.integers(n)) for n in cfg.dims), axis=tuple(range(nd))) *
                np.complex64(0.8 + 0.4 * b / args.batch) for b in range(args.batch)]
-        psi0 = np.ascontiguousarray(np.stack(mem, axis=1).astype(np.complex64))   # storage layout [n0][batch][n1]
+        psi0 = np.ascontiguousarray(np.stack(mem, axis=1).astype(np.complex64))   # storage layout [n0][batch][...]
         del mem
     host_in = torch.from_numpy(psi0).pin_memory()
     host_out = torch.empty_like(host_in).pin_memory()

@@ -70,17 +70,17 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
               double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
               void *cuda_stream);
 
-/* Ensemble of `batch` independent 2D systems advanced together ("batched small-grid
- * ensembles"; parameter scans such as PAPER.md:131 run many small meshes).  Same constants and dtau for every member.
- * dims, L: the two axis lengths and box lengths of ONE system.  Storage layout of every array of the context (state,
- * external potential, source tables): [dims[0]][batch][dims[1]], i.e. the member index sits between the two physical
- * axes, so that the lines of both axes stay dense; member b of a (batch, dims[0], dims[1]) array is at [:, b, :].
- * No pass runs along the member axis.  sn_diagnostics returns the SUM over the ensemble.  1 <= batch <= 2^20;
- * batch * dims[1] must be a multiple of 16. */
-size_t sn_workspace_bytes_batch2d(const int64_t *dims /* host, 2 */, int64_t batch);
-int sn_create_batch2d(sn_ctx **out, const int64_t *dims, int64_t batch, const double *L, double A, double B, double C,
-                      double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
-                      void *cuda_stream);
+/* Ensemble of `batch` independent systems advanced together ("batched small-grid ensembles";
+ * parameter scans such as PAPER.md:131 run many small meshes).  Same constants and dtau for every member.
+ * ndim, dims, L: as for sn_create, describing ONE system.  Storage layout of every array of the context (state,
+ * external potential, source tables): [dims[0]][batch][dims[1]]([dims[2]]), i.e. the member index sits right after
+ * the slowest physical axis, so that the lines of every axis stay dense; member b of a (batch, dims...) array is at
+ * [:, b, ...].  No pass runs along the member index.  sn_diagnostics returns the SUM over the ensemble.
+ * 1 <= batch <= 2^20; batch = 1 is sn_create. */
+size_t sn_workspace_bytes_batch(int ndim, const int64_t *dims /* host, ndim */, int64_t batch);
+int sn_create_batch(sn_ctx **out, int ndim, const int64_t *dims, int64_t batch, const double *L, double A, double B,
+                    double C, double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
+                    void *cuda_stream);
 
 /* Copy a complex64 state in.  psi: host (src_on_device == 0) or device pointer; prod(dims) complex64. */
 int sn_set_state(sn_ctx *ctx, const void *psi, int src_on_device);

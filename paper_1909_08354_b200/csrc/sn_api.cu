@@ -60,24 +60,26 @@ int twiddle_entries(int N)
 
 struct Layout {
     int ndim;
-    bool batch1; // ndim == 3 and axis 1 is an ensemble index, not a physical axis (sn_create_batch2d): no pass runs along it
+    int64_t batch;  // ensemble members (sn_create_batch): storage [n0][batch][n1]([n2]); no pass runs along the member index
+    int64_t pcells; // cells of ONE system (cells = batch * pcells is the storage size)
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
     size_t off_psi, off_hs, off_phi, off_vext, off_beta, off_gamma, off_tw[3], off_ph[5][3], off_ksq[3], off_kother, off_diag, total;
 };
 
-bool make_layout(int ndim, const int64_t *dims, Layout &L, bool batch1 = false)
+bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1)
 {
     if (!dims || (ndim != 2 && ndim != 3)) return false;
-    if (batch1 && (ndim != 3 || dims[1] < 1 || dims[1] > (1 << 20))) return false;
+    if (batch < 1 || batch > (1 << 20)) return false;
     L.ndim = ndim;
-    L.batch1 = batch1;
-    L.cells = 1;
+    L.batch = batch;
+    L.pcells = 1;
     for (int d = 0; d < ndim; d++) {
-        if (!(batch1 && d == 1) && !len_ok(dims[d])) return false;
+        if (!len_ok(dims[d])) return false;
         L.n[d] = dims[d];
-        L.cells *= dims[d];
+        L.pcells *= dims[d];
     }
+    L.cells = L.pcells * batch;
     L.cols0 = L.cells / L.n[0];
     L.nx = L.n[ndim - 1];
     L.hs_lines = (L.n[0] / 2 + 1) * L.cols0 / L.nx;
@@ -91,11 +93,6 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, bool batch1 = false)
     L.off_beta = o; o = align256(o + (size_t)L.cells * 4);
     L.off_gamma = o; o = align256(o + (size_t)L.cells * 4);
     for (int d = 0; d < ndim; d++) {
-        if (batch1 && d == 1) { // no tables for the ensemble axis
-            L.off_tw[d] = L.off_ksq[d] = o;
-            for (int sl = 0; sl < 5; sl++) L.off_ph[sl][d] = o;
-            continue;
-        }
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
         for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
         L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
@@ -271,10 +268,10 @@ int make_tensor_maps(sn_ctx *c)
         if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
         c->m_ok[0] = true;
     }
-    if (l.ndim == 3 && !l.batch1 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
+    if (l.ndim == 3 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
         const int n1 = (int)l.n[1], cpw = snk::pipe_cpw(n1);
-        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0], n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
-        if ((rc = make_map(&c->m_hs1, c->hs, l.n[0] / 2 + 1, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
+        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0] * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs1, c->hs, (l.n[0] / 2 + 1) * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
         c->m_ok[1] = true;
     }
     return SN_OK;
@@ -376,7 +373,6 @@ int upload_phase_tables(sn_ctx *c)
 {
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
-        if (l.batch1 && d == 1) continue;
         const int64_t n = l.n[d];
         std::vector<f4> tab(n);
         for (int sl = 0; sl < PH_SLOTS; sl++) {
@@ -414,7 +410,6 @@ int upload_static_tables(sn_ctx *c)
 {
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
-        if (l.batch1 && d == 1) continue;
         const int N = (int)l.n[d];
         // twiddles: for each stage (NS, R) with NS > 1: entry [r-1][kp] = exp(-2 pi i r kp/(NS R))
         std::vector<f4> tw;
@@ -441,17 +436,19 @@ int upload_static_tables(sn_ctx *c)
     // sum of the non-contiguous axes' k^2 for each contiguous line of the half spectrum
     std::vector<float> ko(l.hs_lines, 0.f);
     const int64_t h0 = l.n[0] / 2 + 1;
-    if (l.ndim == 2) {
-        for (int64_t k0 = 0; k0 < h0; k0++) {
-            const double a = kval(k0, l.n[0], c->L[0]);
-            ko[k0] = (float)(a * a);
-        }
-    } else {
-        for (int64_t k0 = 0; k0 < h0; k0++)
-            for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
-                const double a = kval(k0, l.n[0], c->L[0]), b = l.batch1 ? 0.0 : kval(k1, l.n[1], c->L[1]);
-                ko[k0 * l.n[1] + k1] = (float)(a * a + b * b);
+    // lines of the half spectrum are indexed (k0, member[, k1]); the member index carries no wavenumber
+    for (int64_t k0 = 0; k0 < h0; k0++) {
+        const double a = kval(k0, l.n[0], c->L[0]);
+        for (int64_t b = 0; b < l.batch; b++) {
+            if (l.ndim == 2) {
+                ko[k0 * l.batch + b] = (float)(a * a);
+            } else {
+                for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
+                    const double q = kval(k1, l.n[1], c->L[1]);
+                    ko[(k0 * l.batch + b) * l.n[1] + k1] = (float)(a * a + q * q);
+                }
             }
+        }
     }
     SN_CUDA(cudaMemcpyAsync(c->ws + l.off_kother, ko.data(), ko.size() * 4, cudaMemcpyHostToDevice, c->stream));
     SN_CUDA(cudaMemsetAsync(c->ws + l.off_hs, 0, (size_t)l.hs_elems * 8, c->stream));
@@ -481,7 +478,7 @@ void set_axis_geometry(const sn_ctx *c, PassArgs &a, int axis, int64_t n0)
     if (axis == 0) {
         a.n_outer = 1; a.outer_stride = 0; a.ncols = (int)l.cols0; a.row_stride = l.cols0;
     } else { // axis 1 of a 3D array
-        a.n_outer = (int)n0; a.outer_stride = l.n[1] * l.n[2]; a.ncols = (int)l.n[2]; a.row_stride = l.n[2];
+        a.n_outer = (int)(n0 * l.batch); a.outer_stride = l.n[1] * l.n[2]; a.ncols = (int)l.n[2]; a.row_stride = l.n[2];
     }
 }
 
@@ -494,7 +491,6 @@ int kinetic_sweep(sn_ctx *c, int ph_slot, bool with_nl, bool before_n, int nl_sl
     const Layout &l = c->lay;
     int rc;
     for (int d = 0; d < l.ndim; d++) {
-        if (l.batch1 && d == 1) continue;
         PassArgs a = base_args(c);
         a.data = c->psi;
         a.hs = c->hs;
@@ -526,7 +522,7 @@ int spectrum_chain(sn_ctx *c, bool lap)
 {
     const Layout &l = c->lay;
     int rc;
-    if (l.ndim == 3 && !l.batch1) {
+    if (l.ndim == 3) {
         PassArgs a = base_args(c);
         a.kind = snk::P_S_FFT; a.dir = +1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1];
         set_axis_geometry(c, a, 1, l.n[0] / 2 + 1);
@@ -538,11 +534,11 @@ int spectrum_chain(sn_ctx *c, bool lap)
         a.kind = snk::P_X_POISSON; a.data = c->hs; a.tw = c->tw[dx]; a.ksq = c->ksq[dx]; a.kother2 = c->kother;
         a.nlines = (int)l.hs_lines;
         a.lap = lap ? 1 : 0;
-        const double npts = (double)(l.batch1 ? l.cells / l.n[1] : l.cells); // points of ONE system: the 1/prod(N) of its transforms
+        const double npts = (double)l.pcells; // points of ONE system: the 1/prod(N) of its transforms
         a.pscale = (float)((lap ? 1.0 : c->D) * 0.5 / npts); // 0.5: the packed r2c carries a factor 2
         if ((rc = run_pass(c, (int)l.n[dx], a))) return rc;
     }
-    if (l.ndim == 3 && !l.batch1) {
+    if (l.ndim == 3) {
         PassArgs a = base_args(c);
         a.kind = snk::P_S_FFT; a.dir = -1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1]; a.scale = 1.f;
         set_axis_geometry(c, a, 1, l.n[0] / 2 + 1);
@@ -621,41 +617,36 @@ size_t sn_workspace_bytes(int ndim, const int64_t *dims)
     return make_layout(ndim, dims, l) ? l.total : 0;
 }
 
-size_t sn_workspace_bytes_batch2d(const int64_t *dims, int64_t batch)
+size_t sn_workspace_bytes_batch(int ndim, const int64_t *dims, int64_t batch)
 {
     Layout l;
-    if (!dims) return 0;
-    const int64_t d3[3] = {dims[0], batch, dims[1]};
-    return make_layout(3, d3, l, /*batch1=*/true) ? l.total : 0;
+    return make_layout(ndim, dims, l, batch) ? l.total : 0;
 }
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       bool batch1);
+                       int64_t batch);
 
 int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
               const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
 {
-    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, false);
+    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, 1);
 }
 
-int sn_create_batch2d(sn_ctx **out, const int64_t *dims, int64_t batch, const double *L, double A, double B, double C,
-                      double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
-                      void *cuda_stream)
+int sn_create_batch(sn_ctx **out, int ndim, const int64_t *dims, int64_t batch, const double *L, double A, double B,
+                    double C, double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
+                    void *cuda_stream)
 {
-    if (!dims || !L) return SN_ERR_NULL;
-    const int64_t d3[3] = {dims[0], batch, dims[1]};
-    const double L3[3] = {L[0], 1.0, L[1]};
-    return create_impl(out, 3, d3, L3, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, true);
+    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, batch);
 }
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       bool batch1)
+                       int64_t batch)
 {
     if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
     Layout l;
-    if (!make_layout(ndim, dims, l, batch1)) return SN_ERR_DIMS;
+    if (!make_layout(ndim, dims, l, batch)) return SN_ERR_DIMS;
     if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
     if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
         return SN_ERR_PARAM;
@@ -669,8 +660,8 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
         const int64_t n0 = l.n[0], n1 = l.n[1], n2 = ndim == 3 ? l.n[2] : 1;
         for (int64_t i0 = 0; i0 <= n0 / 2; i0++) {
             const double k0 = kval(i0, n0, L[0]);
-            for (int64_t i1 = 0; i1 <= (batch1 ? 0 : n1 / 2); i1++) {
-                const double k1 = batch1 ? 0.0 : kval(i1, n1, L[1]);
+            for (int64_t i1 = 0; i1 <= n1 / 2; i1++) {
+                const double k1 = kval(i1, n1, L[1]);
                 for (int64_t i2 = 0; i2 <= n2 / 2; i2++) {
                     const double k2 = ndim == 3 ? kval(i2, n2, L[2]) : 0.0;
                     if (std::fabs(C - (k0 * k0 + k1 * k1 + k2 * k2)) < tol) return SN_ERR_SINGULAR;
@@ -866,7 +857,6 @@ int sn_debug_fft(sn_ctx *c, int direction)
     if (direction != 1 && direction != -1) return SN_ERR_PARAM;
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
-        if (l.batch1 && d == 1) continue;
         PassArgs a = base_args(c);
         a.data = c->psi; a.tw = c->tw[d]; a.dir = direction; a.hilo = 1;
         a.scale = direction < 0 ? (float)(1.0 / (double)l.n[d]) : 1.f;
@@ -918,7 +908,6 @@ int sn_diagnostics(sn_ctx *c, sn_diag *out)
     // kinetic energy axis by axis: sum_k k_a^2 |psi^_k|^2 / prod N = sum_lines sum_ka k_a^2 |F_a psi|^2 / N_a
     // (Parseval along the other axes), so one forward line transform per axis suffices.
     for (int d = 0; d < l.ndim; d++) {
-        if (l.batch1 && d == 1) continue;
         PassArgs a = base_args(c);
         a.data = c->psi; a.tw = c->tw[d]; a.ksq = c->ksq[d]; a.diag = c->diag + 3 + d;
         if (d == l.ndim - 1) {
@@ -935,10 +924,10 @@ int sn_diagnostics(sn_ctx *c, sn_diag *out)
     SN_CUDA(cudaStreamSynchronize(c->stream));
     double dV = 1.0;
     for (int d = 0; d < l.ndim; d++)
-        if (!(l.batch1 && d == 1)) dV *= c->L[d] / (double)l.n[d];
+        dV *= c->L[d] / (double)l.n[d];
     double ek = 0.0;
     for (int d = 0; d < l.ndim; d++)
-        if (!(l.batch1 && d == 1)) ek += h[3 + d] / (double)l.n[d];
+        ek += h[3 + d] / (double)l.n[d];
     out->norm = h[0] * dV;
     out->e_kin = -c->A * ek * dV;
     out->e_nonlocal = 0.5 * c->B * h[1] * dV;

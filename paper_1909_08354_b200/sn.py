@@ -23,7 +23,7 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch2d", "sn_create_batch2d")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG", "H_SRC")
@@ -57,11 +57,11 @@ def lib() -> ctypes.CDLL:
         L.sn_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_double, ctypes.c_double,
                                 ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, vp,
                                 ctypes.c_size_t, vp]
-        L.sn_workspace_bytes_batch2d.argtypes = [i64p, ctypes.c_int64]
-        L.sn_workspace_bytes_batch2d.restype = ctypes.c_size_t
-        L.sn_create_batch2d.argtypes = [ctypes.POINTER(vp), i64p, ctypes.c_int64, dp, ctypes.c_double, ctypes.c_double,
-                                        ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, vp,
-                                        ctypes.c_size_t, vp]
+        L.sn_workspace_bytes_batch.argtypes = [ctypes.c_int, i64p, ctypes.c_int64]
+        L.sn_workspace_bytes_batch.restype = ctypes.c_size_t
+        L.sn_create_batch.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, ctypes.c_int64, dp, ctypes.c_double,
+                                      ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, ctypes.c_int,
+                                      ctypes.c_double, vp, ctypes.c_size_t, vp]
         L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_step.argtypes = [vp, ctypes.c_int64]
         L.sn_step_order4.argtypes = [vp, ctypes.c_int64]
@@ -99,14 +99,14 @@ class Simulation:
 
     def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float, g: Sequence[float],
                  dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None):
-        """batch=None: one 2D/3D system of shape dims.  batch=B (dims must be 2D): an ensemble of B systems through
-        sn_create_batch2d; every array then has the STORAGE shape (dims[0], B, dims[1]) (member b at [:, b, :])."""
+        """batch=None: one 2D/3D system of shape dims.  batch=B: an ensemble of B systems through sn_create_batch;
+        every array then has the STORAGE shape (dims[0], B, dims[1][, dims[2]]) (member b at [:, b, ...])."""
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1909_08354_b200 needs a CUDA device (no CPU fallback)")
         if batch is not None:
-            self._init_batch2d(dims, int(batch), L, A, B, C, D, g, dtau, device, stream)
+            self._init_batch(dims, int(batch), L, A, B, C, D, g, dtau, device, stream)
             return
         self.dims = tuple(int(n) for n in dims)
         nd = len(self.dims)
@@ -128,27 +128,28 @@ class Simulation:
                                  ctypes.c_void_p(self._ws.data_ptr()), nbytes,
                                  ctypes.c_void_p(self._stream.cuda_stream)), "sn_create")
 
-    def _init_batch2d(self, dims, batch, L, A, B, C, D, g, dtau, device, stream):
+    def _init_batch(self, dims, batch, L, A, B, C, D, g, dtau, device, stream):
         import torch
-        n0, n1 = (int(n) for n in dims)
-        self.dims = (n0, batch, n1)                       # storage shape of every array
-        Ls = [float(L)] * 2 if np.isscalar(L) else [float(v) for v in L]
+        pd = tuple(int(n) for n in dims)
+        nd = len(pd)
+        self.dims = (pd[0], batch) + pd[1:]               # storage shape of every array
+        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
         g = [float(v) for v in g]
         self.device = torch.device(device)
-        c_dims = (ctypes.c_int64 * 2)(n0, n1)
-        nbytes = int(lib().sn_workspace_bytes_batch2d(c_dims, batch))
+        c_dims = (ctypes.c_int64 * nd)(*pd)
+        nbytes = int(lib().sn_workspace_bytes_batch(nd, c_dims, batch))
         if nbytes == 0:
-            raise SnError(-2, "sn_workspace_bytes_batch2d", lib().sn_strerror(-2).decode())
+            raise SnError(-2, "sn_workspace_bytes_batch", lib().sn_strerror(-2).decode())
         with torch.cuda.device(self.device):
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._h = ctypes.c_void_p()
-        c_L = (ctypes.c_double * 2)(*Ls)
+        c_L = (ctypes.c_double * nd)(*Ls)
         c_g = (ctypes.c_double * max(1, len(g)))(*(g or [0.0]))
         with torch.cuda.device(self.device):
-            _chk(lib().sn_create_batch2d(ctypes.byref(self._h), c_dims, batch, c_L, A, B, C, D, c_g, len(g), dtau,
-                                         ctypes.c_void_p(self._ws.data_ptr()), nbytes,
-                                         ctypes.c_void_p(self._stream.cuda_stream)), "sn_create_batch2d")
+            _chk(lib().sn_create_batch(ctypes.byref(self._h), nd, c_dims, batch, c_L, A, B, C, D, c_g, len(g), dtau,
+                                       ctypes.c_void_p(self._ws.data_ptr()), nbytes,
+                                       ctypes.c_void_p(self._stream.cuda_stream)), "sn_create_batch")
 
     @classmethod
     def from_config(cls, cfg, **kw) -> "Simulation":

@@ -258,15 +258,47 @@ def test_batch2d_members_match_single_system_oracle(mods, dims, batch, steps):
         assert abs(d1[k] - tot[k]) < 2e-5 * max(abs(tot["e_total"]), abs(tot[k])), (k, d1[k], tot[k])
 
 
-def test_batch2d_validation(mods):
+def test_batch_validation(mods):
     Oracle, inputs, sn = mods
     from paper_1909_08354_b200.sn import lib
     import ctypes
     d = (ctypes.c_int64 * 2)(128, 128)
-    assert lib().sn_workspace_bytes_batch2d(d, 0) == 0
-    assert lib().sn_workspace_bytes_batch2d(d, 7) > 7 * 128 * 128 * 8
+    assert lib().sn_workspace_bytes_batch(2, d, 0) == 0
+    assert lib().sn_workspace_bytes_batch(2, d, 7) > 7 * 128 * 128 * 8
+    assert lib().sn_workspace_bytes_batch(2, d, 1) == lib().sn_workspace_bytes(2, d)
     bad = (ctypes.c_int64 * 2)(100, 128)
-    assert lib().sn_workspace_bytes_batch2d(bad, 4) == 0
+    assert lib().sn_workspace_bytes_batch(2, bad, 4) == 0
+
+
+@pytest.mark.parametrize("dims,batch,steps", [((64, 64, 64), 5, 20), ((64, 128, 64), 2, 12), ((96, 64, 128), 3, 6)])
+def test_batch3d_members_match_single_system_oracle(mods, dims, batch, steps):
+    """Ensembles of 3D systems: storage [n0][batch][n1][n2]; the axis-1 passes see n0*batch outer blocks."""
+    Oracle, inputs, sn = mods
+    L = 16.0
+    base = inputs.scaled(inputs.CONFIGS["C4"], dims, L=L, steps=steps)
+    members = [np.roll(base.initial_state(), (3 * b, 5 * b, 7 * b), axis=(0, 1, 2)) * np.complex64(0.8 + 0.1 * b)
+               for b in range(batch)]
+    sim = sn.Simulation(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau, batch=batch)
+    assert sim.dims == (dims[0], batch, dims[1], dims[2])
+    sim.set_state(np.ascontiguousarray(np.stack(members, axis=1).astype(np.complex64)))
+    d0 = sim.diagnostics()
+    sim.step(steps)
+    got = sim.get_state()
+    d1 = sim.diagnostics()
+    sim.close()
+    tot = {k: 0.0 for k in d1}
+    for b in range(batch):
+        orc = Oracle(dims, L, base.A, base.B, base.C, base.D, base.g, base.dtau)
+        orc.set_state(members[b].astype(np.complex64).astype(np.complex128))
+        orc.step(steps)
+        assert rel(got[:, b], orc.get_state()) < TOL_STATE, b
+        r = orc.diagnostics()
+        for k in tot:
+            tot[k] += r[k]
+        orc.close()
+    assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
+    for k in tot:
+        assert abs(d1[k] - tot[k]) < 2e-5 * max(abs(tot["e_total"]), abs(tot[k])), (k, d1[k], tot[k])
 
 
 def test_batch2d_with_nmc_terms_and_order4(mods):
