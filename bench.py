@@ -196,6 +196,8 @@ def main():
 
     import torch
     import torch.distributed as dist
+    from paper_1909_08354_b200 import build as _build
+    _build.build()                                      # no-op when libsn.so is up to date (it travels with the snapshot)
     from paper_1909_08354_b200 import replicas, sn
 
     rank = int(os.environ.get("RANK", "0"))
