@@ -43,10 +43,23 @@ def _compile(args):
 
 
 def build(force: bool = False) -> str:
+    """Build libsn.so if it is missing or older than its sources.  Serialised by a file lock, so several ranks of
+    one node calling it at once compile once."""
+    import fcntl
     os.makedirs(OBJ, exist_ok=True)
+    with open(os.path.join(OBJ, ".lock"), "w") as lk:
+        fcntl.flock(lk, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force)
+        finally:
+            fcntl.flock(lk, fcntl.LOCK_UN)
+
+
+def _build_locked(force: bool) -> str:
     if force:
         for f in os.listdir(OBJ):
-            os.remove(os.path.join(OBJ, f))
+            if f != ".lock":
+                os.remove(os.path.join(OBJ, f))
         if os.path.exists(LIB):
             os.remove(LIB)
     if not _stale(LIB):
