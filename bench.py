@@ -205,10 +205,18 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    # SN_BENCH_BACKEND=gloo: dry run of the multi-rank plumbing on a box with fewer GPUs than ranks (ranks share
+    # devices; replicas do not wait on one another).  Default nccl, one rank per GPU, as the driver launches it.
+    backend = os.environ.get("SN_BENCH_BACKEND", "nccl")
+    if backend != "nccl":
+        local = local % torch.cuda.device_count()
     torch.cuda.set_device(local)
     dev = f"cuda:{local}"
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device(dev))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device(dev))
+        else:
+            dist.init_process_group(backend)
 
     def barrier():
         if world > 1:
@@ -279,7 +287,7 @@ def main():
     sim.close()
 
     # max over ranks
-    ms, e2e_ms = replicas.max_over_ranks([ms, e2e_s * 1e3], device=dev)
+    ms, e2e_ms = replicas.max_over_ranks([ms, e2e_s * 1e3], device=dev if backend == "nccl" else "cpu")
 
     if rank == 0:
         cells = cfg.cells * max(1, args.batch)
