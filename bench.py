@@ -297,13 +297,20 @@ def main():
         dom = max(prof, key=lambda k: prof[k][0])
         dom_ms = prof[dom][0] / prof[dom][1]
         hs_frac = (cfg.dims[0] // 2 + 1) / (cfg.dims[0] / 2)   # exact half-spectrum factor on the 4-byte terms
-        bpc = PASS_BYTES_PER_CELL[dom]
-        if dom == "H_NLKIN":
-            bpc = 16.0 + 4.0 * hs_frac + (4.0 if args.extras else 0.0)   # + the external potential table
-        elif dom == "H_R2C":
-            bpc = 8.0 + 4.0 * hs_frac
-        elif dom in ("S_FFT", "X_POISSON"):
-            bpc = 8.0 * hs_frac
+        def bytes_per_cell(kind):
+            """algorithmic bytes per cell of the full grid for one launch of this pass kind"""
+            if kind == "H_NLKIN":
+                return 16.0 + 4.0 * hs_frac
+            if kind == "H_R2C":
+                return 8.0 + 4.0 * hs_frac
+            if kind in ("S_FFT", "X_POISSON"):
+                return 8.0 * hs_frac
+            if kind == "X_KIN":
+                return 16.0 + (4.0 if args.extras else 0.0)              # + the external potential table
+            if kind == "H_SRC":
+                return 16.0 + 8.0 * hs_frac
+            return PASS_BYTES_PER_CELL.get(kind, 0.0)
+        bpc = bytes_per_cell(dom)
         achieved = bpc * cells / (dom_ms * 1e-3) / 1e9
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
@@ -325,7 +332,10 @@ def main():
                 "traffic_source": "ncu --set full dram bytes per launch, profiles/r01c_ncu_full_C5_512.md",
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
-                "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot}
+                "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot,
+                                 "bytes_per_cell": bytes_per_cell(k),
+                                 "achieved_GBps": bytes_per_cell(k) * cells / (v[0] / v[1] * 1e-3) / 1e9,
+                                 "frac_of_measured_peak": bytes_per_cell(k) * cells / (v[0] / v[1] * 1e-3) / 1e9 / peak}
                              for k, v in sorted(prof.items())},
                 "step": {"b_min_bytes_per_cell_update": B_MIN[nd],
                          "achieved_GBps_over_b_min": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9,
