@@ -143,6 +143,9 @@ STEP_CASES = [
     ("C2", (1024, 1024), 100.0, 40),      # full size, prefix of the 1000 steps
     ("C3", (512, 512), 50.0, 150),        # C = -1 screened case, h as in the config
     ("C3", (4096, 64), 50.0, 20),         # the 4096-point line kernels
+    ("C3", (2048, 128), 50.0, 20),        # 2048-point strided lines: 32-byte rows, SWIZZLE_32B boxes
+    ("C4", (64, 2048, 64), 16.0, 4),      # 2048-point lines along axis 1 of a 3D grid
+    ("C4", (64, 64, 4096), 16.0, 3),      # 4096-point contiguous lines in 3D
     ("C4", (64, 64, 64), 16.0, 100),
     ("C5_64", (64, 64, 64), 128.0, 100),  # full config
     ("C5_128", (128, 128, 128), 128.0, 10),
