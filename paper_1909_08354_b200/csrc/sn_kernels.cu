@@ -44,8 +44,9 @@ __device__ __forceinline__ void block_accumulate(double (&v)[NV], double *out)
 }
 
 // column pairs per CTA tile: 512-point lines run as two 256-thread CTAs per SM (measured 15-30 % faster
-// than one 512-thread CTA: the second CTA's loads overlap the first one's butterflies)
-__host__ __device__ constexpr int cp_for(int N) { return N <= 256 ? 8 : (N <= 1024 ? 4 : (N <= 2048 ? 2 : 1)); }
+// than one 512-thread CTA: the second CTA's loads overlap the first one's butterflies); 384-point lines with
+// 128-byte rows (CP = 8; 384^3 step 2.075 -> 2.036 ms against CP = 4)
+__host__ __device__ constexpr int cp_for(int N) { return N <= 384 ? 8 : (N <= 1024 ? 4 : (N <= 2048 ? 2 : 1)); }
 __host__ __device__ constexpr int sthreads(int N) { return cp_for(N) * (N / ppt_for(N)); }
 // resident CTAs per SM asked of the compiler: 128-thread CTAs (N = 384 and N <= 128) run three (measured at 384^3:
 // S_KIN 0.358 -> 0.329 ms against two), 256-thread CTAs two, 512-thread CTAs one
