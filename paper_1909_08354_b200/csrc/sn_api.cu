@@ -64,7 +64,7 @@ struct Layout {
     int64_t pcells; // cells of ONE system (cells = batch * pcells is the storage size)
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
-    size_t off_psi, off_hs, off_phi, off_vext, off_beta, off_gamma, off_tw[3], off_ph[5][3], off_ksq[3], off_kother, off_diag, total;
+    size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_kother, off_diag, total;
 };
 
 bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1)
@@ -90,8 +90,7 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1)
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
     L.off_phi = o; o = align256(o + (size_t)L.cells * 4);
     L.off_vext = o; o = align256(o + (size_t)L.cells * 4);
-    L.off_beta = o; o = align256(o + (size_t)L.cells * 4);
-    L.off_gamma = o; o = align256(o + (size_t)L.cells * 4);
+    L.off_bg = o; o = align256(o + (size_t)L.cells * 8);
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
         for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
@@ -151,7 +150,7 @@ struct sn_ctx {
     bool v_in_xkin;                         // its phase is applied by the pipelined contiguous-axis kinetic pass
     float *vext;
     bool has_src;                           // position-dependent Poisson source of eq. (12) set
-    float *beta, *gamma;
+    float2 *bg;                             // interleaved (beta, gamma)
     int n_g;
     char *ws;
     cudaStream_t stream;
@@ -563,7 +562,7 @@ int potential_spectrum(sn_ctx *c)
         if ((rc = spectrum_chain(c, /*lap=*/true))) return rc;
         PassArgs a = base_args(c);
         a.kind = snk::P_H_SRC; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
-        a.beta = c->beta; a.gamma = c->gamma;
+        a.bg = c->bg;
         set_axis_geometry(c, a, 0, l.n[0]);
         if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
     }
@@ -682,8 +681,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->hs = reinterpret_cast<float2 *>(c->ws + l.off_hs);
     c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
     c->vext = reinterpret_cast<float *>(c->ws + l.off_vext);
-    c->beta = reinterpret_cast<float *>(c->ws + l.off_beta);
-    c->gamma = reinterpret_cast<float *>(c->ws + l.off_gamma);
+    c->bg = reinterpret_cast<float2 *>(c->ws + l.off_bg);
     c->rho_floor = 1e-30; c->p_pow = 1.0;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
@@ -779,8 +777,19 @@ int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int s
     drop_step_graph(c);
     if (beta) {
         const cudaMemcpyKind k = src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
-        SN_CUDA(cudaMemcpyAsync(c->beta, beta, (size_t)c->lay.cells * 4, k, c->stream));
-        SN_CUDA(cudaMemcpyAsync(c->gamma, gamma, (size_t)c->lay.cells * 4, k, c->stream));
+        // stored interleaved; host tables pass through two scratch regions (phi scratch, half spectrum) that hold
+        // nothing between calls
+        const float *db = beta, *dg = gamma;
+        if (!src_on_device) {
+            float *sb = c->phi, *sg = reinterpret_cast<float *>(c->hs);
+            SN_CUDA(cudaMemcpyAsync(sb, beta, (size_t)c->lay.cells * 4, k, c->stream));
+            SN_CUDA(cudaMemcpyAsync(sg, gamma, (size_t)c->lay.cells * 4, k, c->stream));
+            db = sb; dg = sg;
+        }
+        const int rc = snk::launch_interleave(db, dg, c->bg, c->lay.cells, c->stream);
+        if (rc != 0) return cuda_fail((cudaError_t)rc);
+        if (!src_on_device) // the padding line of the half spectrum (2D, odd line count) must stay finite: clear the scratch
+            SN_CUDA(cudaMemsetAsync(c->hs, 0, (size_t)c->lay.hs_elems * 8, c->stream));
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
     c->has_src = beta != nullptr;

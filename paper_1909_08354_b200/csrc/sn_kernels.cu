@@ -158,15 +158,14 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
             // eq. (12): the half spectrum holds F[lap rho]; bring it back along axis 0 and form the source
             // s = gamma(x) rho + beta(x) lap rho for the thread's four real columns, then transform s like rho
             c2r_potential<N, CP>(p, hs4, rs4, t, j, a, b, sm);
-            const float2 *be2 = reinterpret_cast<const float2 *>(p.beta) + col4, *ga2 = reinterpret_cast<const float2 *>(p.gamma) + col4;
+            const float4 *bg4 = reinterpret_cast<const float4 *>(p.bg) + col4; // (beta, gamma) of two adjacent columns
 #pragma unroll
             for (int m = 0; m < P; m++) {
                 const long long row = (long long)(j + T * m) * rs4;
                 const float4 u = psi4[row + t], v = psi4[row + CP + t];
-                const float2 b0 = __ldg(be2 + row + t), b1 = __ldg(be2 + row + CP + t);
-                const float2 g0 = __ldg(ga2 + row + t), g1 = __ldg(ga2 + row + CP + t);
-                a[m] = make_float2(fmaf(g0.x, abs2(lo2(u)), b0.x * a[m].x), fmaf(g0.y, abs2(hi2(u)), b0.y * a[m].y));
-                b[m] = make_float2(fmaf(g1.x, abs2(lo2(v)), b1.x * b[m].x), fmaf(g1.y, abs2(hi2(v)), b1.y * b[m].y));
+                const float4 q0 = __ldg(bg4 + row + t), q1 = __ldg(bg4 + row + CP + t);
+                a[m] = make_float2(fmaf(q0.y, abs2(lo2(u)), q0.x * a[m].x), fmaf(q0.w, abs2(hi2(u)), q0.z * a[m].y));
+                b[m] = make_float2(fmaf(q1.y, abs2(lo2(v)), q1.x * b[m].x), fmaf(q1.w, abs2(hi2(v)), q1.z * b[m].y));
             }
         } else {
 #pragma unroll
@@ -415,5 +414,19 @@ int launch_pass(const PassArgs &a)
 }
 
 template int launch_pass<SN_LEN>(const PassArgs &a);
+
+#if SN_LEN == 64
+// setup only (sn_set_source_tables), never inside a step: interleave the two source tables of eq. (12)
+__global__ void k_interleave(const float *__restrict__ beta, const float *__restrict__ gamma, float2 *__restrict__ bg, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        bg[i] = make_float2(beta[i], gamma[i]);
+}
+int launch_interleave(const float *beta, const float *gamma, float2 *bg, long long n, cudaStream_t stream)
+{
+    k_interleave<<<1184, 256, 0, stream>>>(beta, gamma, bg, n);
+    return (int)cudaGetLastError();
+}
+#endif
 
 } // namespace snk

@@ -57,7 +57,7 @@ struct PassArgs {
     NLParams nl;
     float *phi_out;         // DEVICE: P_H_POT
     const float *vext;      // DEVICE: external potential (same layout as psi, float) or nullptr
-    const float *beta, *gamma; // DEVICE: P_H_SRC source tables of eq. (12) (layout of psi, float)
+    const float2 *bg;       // DEVICE: P_H_SRC source tables of eq. (12), interleaved (beta, gamma) per cell, layout of psi
     int lap;                // P_X_POISSON: multiply by -k^2 * pscale instead of pscale/(C - k^2)
     double *diag;           // DEVICE: accumulators
     cudaStream_t stream;
@@ -82,6 +82,7 @@ struct PipeArgs {
     CUtensorMap m_data;   // psi (or the half spectrum for P_S_FFT): box {4*CPW floats, pipe_box_rows(N) rows, 1}
     CUtensorMap m_hs;     // P_H_*: half spectrum [N/2+1 rows][2*cols floats]: box {4*CPW, pipe_box_rows(N/2) rows, 1}
     CUtensorMap m_hs_row; // P_H_*: same tensor, box {4*CPW, 1, 1} (the row N/2)
+    CUtensorMap m_bg;     // P_H_SRC: the interleaved (beta, gamma) table, same geometry as m_data
     PassArgs a;
     int n_tiles;          // tiles of this pass
     int tiles_per_outer;  // strided kinds: column blocks per outer index
@@ -124,5 +125,8 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 
 template <int N>
 int launch_pipe(const PipeArgs &a);
+
+// setup helper (not part of a step): bg[i] = (beta[i], gamma[i])
+int launch_interleave(const float *beta, const float *gamma, float2 *bg, long long n, cudaStream_t stream);
 
 } // namespace snk
