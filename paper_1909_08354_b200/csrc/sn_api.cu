@@ -167,7 +167,7 @@ struct sn_ctx {
     bool use_pipe;
     bool pipe_all;  // SN_PIPE_ALL=1: pipelined kernels wherever they are instantiated (tests, A/B runs)
     int sm_count;
-    CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row;
+    CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row, m_bg;
     bool m_ok[2];
     // CUDA graph of one interior step [N(dtau) K(dtau)] for launch-bound grids (<= 2^24 cells): captured once
     // on a private stream, replayed on the caller's stream
@@ -265,6 +265,7 @@ int make_tensor_maps(sn_ctx *c)
         if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, snk::pipe_box_rows(n0 / 2), cpw))) return rc;
         if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
+        if ((rc = make_map(&c->m_bg, c->bg, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         c->m_ok[0] = true;
     }
     if (l.ndim == 3 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
@@ -304,7 +305,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
     int rc;
     if (c->use_pipe) {
         const bool strided = a.kind == snk::P_S_FFT || a.kind == snk::P_S_KIN;
-        const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C;
+        const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C || a.kind == snk::P_H_SRC;
         const int axis = strided ? a.axis : 0;
         const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
                           !(a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin); // then the first-path kernel reads V
@@ -324,6 +325,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
                 pa.m_data = c->m_psi[0];
                 pa.m_hs = c->m_hs0;
                 pa.m_hs_row = c->m_hs0_row;
+                pa.m_bg = c->m_bg;
                 pa.tiles_per_outer = a.ncols / (2 * snk::pipe_groups(N));
                 pa.n_tiles = pa.tiles_per_outer;
             } else {

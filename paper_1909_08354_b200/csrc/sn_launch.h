@@ -114,6 +114,7 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
     case P_S_KIN:
     case P_H_NLKIN:
     case P_H_R2C:
+    case P_H_SRC:
         return ncols % (2 * pipe_groups(N)) == 0; // a tile is 2 G columns wide
     case P_X_KIN:
     case P_X_POISSON:

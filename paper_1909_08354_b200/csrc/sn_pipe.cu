@@ -482,6 +482,145 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_r2c(const __grid_co
     if (tid == 0) bulk_wait<0>();
 }
 
+// P_H_SRC (eq. (12); NEXT-1): the half spectrum holds F[lap rho].  Per tile: c2r along axis 0 ->
+// s = gamma rho + beta lap rho from psi and the interleaved (beta, gamma) table -> packed r2c -> F[s], in place in
+// the half-spectrum tile.  Memory-bound (4 + 8 + 8 + 4 B/cell), so both inputs are prefetched one tile ahead:
+// two half-spectrum buffers (in/out in place) and ONE auxiliary stage (psi tile + table tile) that is reloaded as
+// soon as every warp has turned it into registers.
+template <int N>
+__global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_src(const __grid_constant__ PipeArgs p)
+{
+    using g_ = Geo<N>;
+    constexpr int P = g_::P, TILE_BYTES = g_::TILE_BYTES, PIPE_WARPS = g_::NWARP, T = g_::T, G = g_::G, CPW = g_::CPW,
+                  RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX;
+    constexpr int HS_BYTES = SUB * g_::HS_SUB_BYTES;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t *base = align_1024(smem_raw);       // [psi tile][bg tile][hs buffer 0][hs buffer 1][barriers]
+    uint8_t *hsb = base + 2 * TILE_BYTES;
+    uint64_t *hfull = reinterpret_cast<uint64_t *>(hsb + 2 * HS_BYTES), *done = hfull + 2, *afull = hfull + 4, *ause = hfull + 5;
+    const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g / CPW, t = g % CPW;
+
+    if (tid == 0) {
+        for (int i = 0; i < 2; i++) {
+            mbar_init(hfull + i, 1);
+            mbar_init(done + i, PIPE_WARPS);
+        }
+        mbar_init(afull, 1);
+        mbar_init(ause, PIPE_WARPS);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    auto col_of = [&](int k) { return (int)(blockIdx.x + k * gridDim.x) * 2 * G; };
+    auto issue_hs = [&](int k) {
+        const int col0 = col_of(k), b = k & 1;
+        mbar_arrive_expect_tx(hfull + b, g_::HS_TX);
+#pragma unroll
+        for (int ss = 0; ss < SUB; ss++) {
+            uint8_t *hs = hsb + b * HS_BYTES + ss * g_::HS_SUB_BYTES;
+#pragma unroll
+            for (int bx = 0; bx < g_::NHBOX; bx++)
+                tma_load_3d(hs + bx * g_::HB * RBY, &p.m_hs, hfull + b, 2 * (col0 + 2 * CPW * ss), bx * g_::HB, 0);
+            tma_load_3d(hs + (N / 2) * RBY, &p.m_hs_row, hfull + b, 2 * (col0 + 2 * CPW * ss), N / 2, 0);
+        }
+    };
+    auto issue_aux = [&](int k) {
+        const int col0 = col_of(k);
+        mbar_arrive_expect_tx(afull, 2 * TILE_BYTES);
+#pragma unroll
+        for (int ss = 0; ss < SUB; ss++)
+#pragma unroll
+            for (int bx = 0; bx < NBOX; bx++) {
+                const int off = ss * g_::SUB_BYTES + bx * RB * RBY;
+                tma_load_3d(base + off, &p.m_data, afull, 2 * (col0 + 2 * CPW * ss), bx * RB, 0);
+                tma_load_3d(base + TILE_BYTES + off, &p.m_bg, afull, 2 * (col0 + 2 * CPW * ss), bx * RB, 0);
+            }
+    };
+    if (tid == 0) {
+        if (nk > 0) { issue_hs(0); issue_aux(0); }
+        if (nk > 1) issue_hs(1);
+    }
+
+    for (int k = 0; k < nk; k++) {
+        const int b = k & 1;
+        const uint32_t hpar = (k >> 1) & 1, apar = k & 1;
+        const float4 *psub = reinterpret_cast<const float4 *>(base) + s * g_::SUB_F4;
+        const float4 *qsub = reinterpret_cast<const float4 *>(base + TILE_BYTES) + s * g_::SUB_F4;
+        float4 *hsub = reinterpret_cast<float4 *>(hsb + b * HS_BYTES) + s * g_::HS_SUB_F4;
+        const int jz = opaque(j), jf = opaque(j);
+        SmemSubOne<T, CPW> sm1{reinterpret_cast<float2 *>(hsub), t, 1 + g};
+
+        // c2r of F[lap rho] (two real columns as one complex line)
+        mbar_wait(hfull + b, hpar);
+        float2 z[P];
+        {
+            const float4 *hup = hsub + nat_slot<CPW>(jz, t), *hdn = hsub + nat_slot<CPW>(N / 2 - jz, t);
+#pragma unroll
+            for (int m = 0; m < P; m++) {
+                const float4 u = m < P / 2 ? hup[CPW * T * m] : hdn[-CPW * T * (m - P / 2)];
+                z[m] = m < P / 2 ? make_float2(u.x - u.w, u.y + u.z) : make_float2(u.x + u.w, u.z - u.y);
+            }
+        }
+        fft_single<N, -1, false>(z, jz, p.a.tw, sm1);
+        // the store of tile k-1 has had the whole c2r to drain: prefetch the half spectrum of tile k+1 into its buffer
+        if (tid == 0 && k >= 1 && k + 1 < nk) {
+            bulk_wait_read<0>();
+            issue_hs(k + 1);
+        }
+
+        // s = gamma rho + beta lap rho for the thread's two columns at rows j + T m
+        mbar_wait(afull, apar);
+        {
+            const float4 *pm = psub + nat_slot<CPW>(jf, t), *qm = qsub + nat_slot<CPW>(jf, t);
+#pragma unroll
+            for (int m = 0; m < P; m++) {
+                const float4 v = pm[CPW * T * m], q = qm[CPW * T * m]; // q = (beta0, gamma0, beta1, gamma1)
+                z[m] = make_float2(fmaf(q.y, abs2(lo2(v)), q.x * z[m].x), fmaf(q.w, abs2(hi2(v)), q.z * z[m].y));
+            }
+        }
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(ause);
+
+        // packed r2c of s, in place in the half-spectrum buffer
+        fft_single<N, +1, false>(z, jf, p.a.tw, sm1);
+        if (tid == 0 && k + 1 < nk) { // every warp has consumed the auxiliary stage: reload it for tile k+1
+            mbar_wait(ause, apar);
+            issue_aux(k + 1);
+        }
+        float2 dummy = make_float2(0.f, 0.f), y[P / 2 + 1];
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m < P; m++) sm1.st(jf + T * m, z[m], dummy);
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m <= P / 2; m++)
+            if (m < P / 2 || j == 0) sm1.ld((N - (jf + T * m)) % N, y[m], dummy);
+        sm1.sync();
+#pragma unroll
+        for (int m = 0; m <= P / 2; m++)
+            if (m < P / 2 || j == 0)
+                hsub[nat_slot<CPW>(jf + T * m, t)] =
+                    make_float4(z[m].x + y[m].x, z[m].y - y[m].y, z[m].y + y[m].y, y[m].x - z[m].x);
+        warp_arrive_done(done + b);
+
+        if (tid == 0) {
+            mbar_wait(done + b, hpar);
+            const int col0 = col_of(k);
+#pragma unroll
+            for (int ss = 0; ss < SUB; ss++) {
+                const uint8_t *hs = hsb + b * HS_BYTES + ss * g_::HS_SUB_BYTES;
+#pragma unroll
+                for (int bx = 0; bx < g_::NHBOX; bx++)
+                    tma_store_3d(&p.m_hs, hs + bx * g_::HB * RBY, 2 * (col0 + 2 * CPW * ss), bx * g_::HB, 0);
+                tma_store_3d(&p.m_hs_row, hs + (N / 2) * RBY, 2 * (col0 + 2 * CPW * ss), N / 2, 0);
+            }
+            bulk_commit();
+        }
+    }
+    if (tid == 0) bulk_wait<0>();
+}
+
 // ---------------------------------------------------------------------------- contiguous axis
 // P_X_KIN: forward -> kinetic phase -> inverse along the contiguous axis of psi; P_X_POISSON (S5-S7,
 // eq. (2)): forward -> D/(C - k^2) -> inverse along the contiguous axis of the half
@@ -651,6 +790,7 @@ int launch_pipe(const PipeArgs &a)
             return (a.a.nl.flags & 1) ? launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, true>, NT, S2H, a)
                                       : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, NT, S2H, a);
         case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, NT, S2H, a);
+        case P_H_SRC: return launch_pipe_kernel(k_pipe_src<N>, NT, S2H + 0, a);
         default: break;
         }
     }
