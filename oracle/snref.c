@@ -75,6 +75,10 @@ typedef struct snref_ctx {
     double *vext; /* NULL or cells doubles */
     /* modified Poisson source of eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho) */
     double *beta, *gamma; /* both NULL (plain eq. (2)) or both cells doubles */
+    /* Bohm quantum potential of eq. (15): coefficient c_B (nu^2 there), V_B = lap sqrt(rho)/(2 sqrt(rho)),
+     * with sqrt(rho) clamped from below by sqrt_floor in the denominator (reading Q17 of DESIGN.md) */
+    double c_bohm, sqrt_floor;
+    double *vb; /* scratch, cells doubles, allocated on first use */
     cplx *psi;   /* state */
     cplx *work;  /* rho^ / phi^ scratch */
     int has_state;
@@ -278,7 +282,7 @@ int snref_create(snref_ctx **out, int ndim, const int64_t *dims, const double *L
     c->ndim = ndim;
     for (int d = 0; d < ndim; d++) { c->n[d] = dims[d]; c->L[d] = L[d]; }
     c->A = A; c->B = B; c->C = C; c->D = D; c->n_g = n_g; c->dtau = dtau; c->cells = cells;
-    c->rho_floor = 1e-30; c->p_pow = 1.0;
+    c->rho_floor = 1e-30; c->p_pow = 1.0; c->sqrt_floor = 1e-30;
     for (int j = 0; j < n_g; j++) c->g[j] = g[j];
     /* Q5: C > 0 hitting a grid mode makes eq. (2) unsolvable */
     if (C > 0.0) {
@@ -318,6 +322,28 @@ int snref_set_external_potential(snref_ctx *c, const double *v)
     return SNREF_OK;
 }
 
+static int bohm_potential(snref_ctx *c);
+
+/* c_B V_B added to the N sub-step potential (eq. (15): c_B = nu^2); c_B = 0 switches it off */
+int snref_set_bohm(snref_ctx *c, double c_bohm, double sqrt_floor)
+{
+    if (!c) return SNREF_ERR_NULL;
+    if (!isfinite(c_bohm) || !isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SNREF_ERR_PARAM;
+    c->c_bohm = c_bohm; c->sqrt_floor = sqrt_floor;
+    return SNREF_OK;
+}
+
+/* V_B of the current state (cells doubles); state unchanged */
+int snref_bohm_potential(snref_ctx *c, double *out)
+{
+    if (!c || !out) return SNREF_ERR_NULL;
+    if (!c->has_state) return SNREF_ERR_STATE;
+    int rc = bohm_potential(c);
+    if (rc) return rc;
+    memcpy(out, c->vb, sizeof(double) * (size_t)c->cells);
+    return SNREF_OK;
+}
+
 /* position-dependent source of eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); tables are copied;
  * two NULLs restore eq. (2) (equivalent to gamma = 1, beta = 0) */
 int snref_set_source_tables(snref_ctx *c, const double *beta, const double *gamma)
@@ -338,6 +364,7 @@ int snref_set_source_tables(snref_ctx *c, const double *beta, const double *gamm
 int snref_destroy(snref_ctx *c)
 {
     if (!c) return SNREF_ERR_NULL;
+    free(c->vb);
     free(c->beta);
     free(c->gamma);
     free(c->vext);
@@ -422,16 +449,39 @@ static int potential(snref_ctx *c)
     return SNREF_OK;
 }
 
-/* N(s): psi *= exp(-i s (B phi + G(rho))) with phi, rho from psi at the start of the sub-step */
+/* V_B = lap sqrt(rho) / (2 max(sqrt(rho), sqrt_floor)) into c->vb; lap taken spectrally: F^-1[-k^2 F[sqrt(rho)]] */
+static int bohm_potential(snref_ctx *c)
+{
+    if (!c->vb) {
+        c->vb = (double *)malloc(sizeof(double) * (size_t)c->cells);
+        if (!c->vb) return SNREF_ERR_NOMEM;
+    }
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) c->work[i] = cabs(c->psi[i]);
+    int rc = fftn(c->work, c->ndim, c->n, +1);
+    if (rc) return rc;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) c->work[i] *= -ksq_at(c, i);
+    if ((rc = fftn(c->work, c->ndim, c->n, -1))) return rc;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) c->vb[i] = creal(c->work[i]) / (2.0 * fmax(cabs(c->psi[i]), c->sqrt_floor));
+    return SNREF_OK;
+}
+
+/* N(s): psi *= exp(-i s (B phi + G(rho) + V + c_B V_B)) with phi, rho, V_B from psi at the start of the sub-step
+ * (every factor leaves rho unchanged, so the order of the factors does not matter) */
 static int nonlinear(snref_ctx *c, double s)
 {
-    int rc = potential(c);
+    int rc;
+    if (c->c_bohm != 0.0 && (rc = bohm_potential(c))) return rc;
+    rc = potential(c);
     if (rc) return rc;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < c->cells; i++) {
         double re = creal(c->psi[i]), im = cimag(c->psi[i]);
         double rho = re * re + im * im;
-        double th = -s * (c->B * creal(c->work[i]) + G_of(c, rho) + (c->vext ? c->vext[i] : 0.0));
+        double th = -s * (c->B * creal(c->work[i]) + G_of(c, rho) + (c->vext ? c->vext[i] : 0.0) +
+                          (c->c_bohm != 0.0 ? c->c_bohm * c->vb[i] : 0.0));
         c->psi[i] *= cos(th) + I * sin(th);
     }
     return SNREF_OK;

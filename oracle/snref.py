@@ -52,6 +52,8 @@ def lib() -> ctypes.CDLL:
         L.snref_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
         L.snref_set_external_potential.argtypes = [vp, vp]
         L.snref_set_source_tables.argtypes = [vp, vp, vp]
+        L.snref_set_bohm.argtypes = [vp, ctypes.c_double, ctypes.c_double]
+        L.snref_bohm_potential.argtypes = [vp, vp]
         L.snref_num_threads.restype = ctypes.c_int
         L.snref_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -164,6 +166,15 @@ class Oracle:
         g = np.ascontiguousarray(gamma, dtype=np.float64)
         assert b.shape == self.dims and g.shape == self.dims
         _chk(lib().snref_set_source_tables(self._h, b.ctypes.data, g.ctypes.data), "snref_set_source_tables")
+
+    def set_bohm(self, c_bohm: float, sqrt_floor: float = 1e-30) -> None:
+        """c_B * V_B added to the N sub-step, V_B = lap sqrt(rho)/(2 max(sqrt(rho), sqrt_floor)) (eq. (15))."""
+        _chk(lib().snref_set_bohm(self._h, float(c_bohm), float(sqrt_floor)), "snref_set_bohm")
+
+    def bohm_potential(self) -> np.ndarray:
+        out = np.empty(self.dims, dtype=np.float64)
+        _chk(lib().snref_bohm_potential(self._h, out.ctypes.data), "snref_bohm_potential")
+        return out
 
     def potential(self) -> np.ndarray:
         out = np.empty(self.dims, dtype=np.float64)

@@ -222,3 +222,44 @@ def test_w6_order4_self_convergence_and_invariants():
     rate = -0.5 * float(q @ q) - 1.0 * 0.9 * 0.49 / (-1.0) - 0.2 * 0.49
     assert rel(o.get_state(), pw * np.exp(1j * rate * 5 * 3e-2)) < 1e-12
     o.close()
+
+
+# ------------------------------------------------------------------ W7 Bohm quantum potential of eq. (15)
+
+def test_w7_bohm_potential_closed_form_and_stationarity():
+    """sqrt(rho) = a exp(-r^2/(2 s^2))  =>  V_B = lap sqrt(rho)/(2 sqrt(rho)) = (r^2/s^4 - d/s^2)/2 (closed form).
+    With c_B = -2A the Bohm term cancels the quantum pressure of the kinetic operator exactly (Madelung:
+    A lap sqrt(rho) + c_B V_B sqrt(rho) = 0), so ANY real positive state is stationary: the Gaussian that spreads
+    under K alone stays put to ~1e-6 (splitting error and the floor in the far tails)."""
+    dims, L, s, a = (96, 96), 24.0, 1.7, 0.8
+    X, Y = grid(dims, L)
+    r2 = X * X + Y * Y
+    psi0 = (a * np.exp(-r2 / (2 * s * s))).astype(complex)
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)
+    o.set_bohm(1.0, 1e-300)
+    o.set_state(psi0)
+    vb = o.bohm_potential()
+    core = r2 < (5 * s) ** 2                                   # where sqrt(rho) is above the roundoff of the transform
+    want = 0.5 * (r2 / s ** 4 - 2.0 / s ** 2)
+    assert np.abs(vb - want)[core].max() < 1e-6
+    o.close()
+    errs = []
+    for dtau in (2e-2, 1e-2):
+        o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), dtau)
+        o.set_bohm(1.0, 1e-6)                                  # c_B = -2A
+        o.set_state(psi0)
+        o.step(int(round(1.0 / dtau)))
+        errs.append(rel(o.get_state(), psi0))
+        o.close()
+    assert max(errs) < 1e-5, errs                              # stationary (splitting + floor effects ~1e-6)
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)      # without the Bohm term the packet spreads
+    o.set_state(psi0)
+    o.step(100)
+    assert rel(o.get_state(), psi0) > 0.1
+    o.close()
+    o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)      # wrong sign: spreads faster still
+    o.set_bohm(-1.0, 1e-6)
+    o.set_state(psi0)
+    o.step(100)
+    assert np.abs(o.get_state()).max() < 0.75 * a
+    o.close()
