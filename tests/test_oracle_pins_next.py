@@ -255,11 +255,12 @@ def test_w7_bohm_potential_closed_form_and_stationarity():
     o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)      # without the Bohm term the packet spreads
     o.set_state(psi0)
     o.step(100)
+    free_max = np.abs(o.get_state()).max()
     assert rel(o.get_state(), psi0) > 0.1
     o.close()
     o = Oracle(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)      # wrong sign: spreads faster still
     o.set_bohm(-1.0, 1e-6)
     o.set_state(psi0)
     o.step(100)
-    assert np.abs(o.get_state()).max() < 0.75 * a
+    assert np.abs(o.get_state()).max() < 0.97 * free_max
     o.close()
