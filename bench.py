@@ -47,6 +47,7 @@ PASS_BYTES_PER_CELL = {
     "S_FFT": 8.0,      # read + write half spectrum
     "X_POISSON": 8.0,
     "H_SRC": 24.0,     # eq. (12): read F[lap rho] (4) + psi (8) + beta, gamma (8), write F[s] (4)
+    "H_BOHM": 20.0,    # eq. (15) Bohm phase: read F[lap sqrt(rho)] (4) + psi (8), write psi (8)
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
 B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update
@@ -180,6 +181,8 @@ def main():
     ap.add_argument("--batch", type=int, default=0,
                     help="an ensemble of this many independent systems in one context (sn_create_batch; every "
                          "member a shifted, rescaled copy of the workload's state)")
+    ap.add_argument("--bohm", type=float, default=0.0,
+                    help="with --extras: also the Bohm term c_B V_B of eq. (15) with this coefficient")
     ap.add_argument("--order4", action="store_true",
                     help="time sn_step_order4 (Yoshida composition of three Strang steps per step) instead of sn_step")
     ap.add_argument("--extras", action="store_true",
@@ -250,6 +253,8 @@ def main():
         sim.set_external_potential(np.log(1.0 - f).astype(np.float32))
         # eq. (12) with eq. (9),(10): gamma = (1 - f)/2, beta = lambda f/(r + r0)
         sim.set_source_tables((f / (rs + 2.0)).astype(np.float32), (0.5 * (1.0 - f)).astype(np.float32))
+        if args.bohm:
+            sim.set_bohm(args.bohm, 1e-4)               # eq. (15): + nu^2 V_B
         del rs, f, r2
     step = sim.step_order4 if args.order4 else sim.step
     sim.set_state(dev_in)
@@ -309,6 +314,8 @@ def main():
                 return 16.0 + (4.0 if args.extras else 0.0)              # + the external potential table
             if kind == "H_SRC":
                 return 16.0 + 8.0 * hs_frac
+            if kind == "H_BOHM":
+                return 16.0 + 4.0 * hs_frac
             return PASS_BYTES_PER_CELL.get(kind, 0.0)
         bpc = bytes_per_cell(dom)
         achieved = bpc * cells / (dom_ms * 1e-3) / 1e9

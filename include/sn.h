@@ -117,6 +117,12 @@ int sn_set_dtau(sn_ctx *ctx, double dtau);
  *   workspace); two NULLs restore eq. (2) (= gamma 1, beta 0).  Costs one more half-spectrum chain and one more
  *   axis-0 pass per step.  e_nonlocal of sn_diagnostics stays (B/2) sum phi rho dV (no longer a conserved energy
  *   when beta, gamma vary in space: the kernel of phi[rho] is not symmetric). */
+/* sn_set_bohm: the Bohm quantum potential of eq. (15), PAPER.md:102 -- the N sub-step phase gains the factor
+ *   exp(-i s c_bohm V_B), V_B = lap sqrt(rho) / (2 max(sqrt(rho), sqrt_floor)) (c_bohm = nu^2 in eq. (15); with
+ *   c_bohm = -2A it cancels the quantum pressure of the kinetic operator and real states become stationary).
+ *   sqrt_floor > 0 is reading Q17 (the paper does not regularise 1/sqrt(rho)).  Costs one more r2c + half-spectrum
+ *   chain + axis-0 pass per N sub-step.  c_bohm = 0 switches it off.  Not included in sn_diagnostics' energies. */
+int sn_set_bohm(sn_ctx *ctx, double c_bohm, double sqrt_floor);
 int sn_set_local_terms(sn_ctx *ctx, double g_log, double rho_floor, double g_pow, double p_pow);
 int sn_set_source_tables(sn_ctx *ctx, const float *beta, const float *gamma, int src_on_device);
 int sn_set_external_potential(sn_ctx *ctx, const float *v, int src_on_device);
@@ -138,10 +144,11 @@ int64_t sn_launch_count(const sn_ctx *ctx);
  *   4 H_R2C  axis-0 density + packed r2c           5 H_POT  axis-0 c2r -> phi (test hook)
  *   6 H_DIAG axis-0 c2r + energy sums              7 X_FFT  contiguous-axis plain transform
  *   8 X_KIN  contiguous-axis forward-phase-inverse 9 X_POISSON contiguous-axis forward-D/(C-k^2)-inverse
- *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12)) */
-#define SN_NUM_PASS_KINDS 12
+ *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12))
+ *  12 H_BOHM axis-0 Bohm phase (eq. (15)) */
+#define SN_NUM_PASS_KINDS 13
 int sn_profile(sn_ctx *ctx, int enable);
-int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 12 */, int64_t *launches_by_kind /* host, 12 */,
+int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 13 */, int64_t *launches_by_kind /* host, 13 */,
                     int reset);
 
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */

@@ -150,6 +150,7 @@ struct sn_ctx {
     bool v_in_xkin;                         // its phase is applied by the pipelined contiguous-axis kinetic pass
     float *vext;
     bool has_src;                           // position-dependent Poisson source of eq. (12) set
+    double c_bohm, sqrt_floor;              // Bohm term of eq. (15): c_B V_B in the N sub-step (0 = off)
     float2 *bg;                             // interleaved (beta, gamma)
     int n_g;
     char *ws;
@@ -305,7 +306,8 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
     int rc;
     if (c->use_pipe) {
         const bool strided = a.kind == snk::P_S_FFT || a.kind == snk::P_S_KIN;
-        const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C || a.kind == snk::P_H_SRC;
+        const bool haxis = a.kind == snk::P_H_NLKIN || a.kind == snk::P_H_R2C || a.kind == snk::P_H_SRC ||
+                           a.kind == snk::P_H_BOHM;
         const int axis = strided ? a.axis : 0;
         const bool maps = ((strided || haxis) ? c->m_ok[axis] : true) &&
                           !(a.kind == snk::P_H_NLKIN && c->has_vext && !c->v_in_xkin); // then the first-path kernel reads V
@@ -550,16 +552,21 @@ int spectrum_chain(sn_ctx *c, bool lap)
 
 // phi^ (half spectrum, all scales folded in, ready for the axis-0 c2r) from the current psi.
 // With source tables (eq. (12)): rho -> F[rho] -> -k^2 -> lap rho -> s = gamma rho + beta lap rho -> F[s] -> phi^.
+int density_r2c(sn_ctx *c, bool sqrt_rho)
+{
+    const Layout &l = c->lay;
+    PassArgs a = base_args(c);
+    a.kind = snk::P_H_R2C; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+    a.sqrt_rho = sqrt_rho ? 1 : 0;
+    set_axis_geometry(c, a, 0, l.n[0]);
+    return run_pass(c, (int)l.n[0], a);
+}
+
 int potential_spectrum(sn_ctx *c)
 {
     const Layout &l = c->lay;
     int rc;
-    {
-        PassArgs a = base_args(c);
-        a.kind = snk::P_H_R2C; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
-        set_axis_geometry(c, a, 0, l.n[0]);
-        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
-    }
+    if ((rc = density_r2c(c, false))) return rc;
     if (c->has_src) {
         if ((rc = spectrum_chain(c, /*lap=*/true))) return rc;
         PassArgs a = base_args(c);
@@ -571,6 +578,26 @@ int potential_spectrum(sn_ctx *c)
     return spectrum_chain(c, /*lap=*/false);
 }
 
+// What an N sub-step of length dtau * NL_LEN[nl_slot] needs before the axis-0 pass of the next sweep: the Bohm
+// phase (eq. (15): psi *= exp(-i s c_B lap sqrt(rho)/(2 sqrt(rho))), a pass of its own since it commutes with the
+// rest of the N phase and leaves rho unchanged), then phi^.
+int prepare_n(sn_ctx *c, int nl_slot)
+{
+    const Layout &l = c->lay;
+    int rc;
+    if (c->c_bohm != 0.0) {
+        if ((rc = density_r2c(c, true))) return rc;
+        if ((rc = spectrum_chain(c, /*lap=*/true))) return rc;
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_BOHM; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+        a.hbohm = (float)(-0.25 * c->dtau * NL_LEN[nl_slot] * c->c_bohm);
+        a.sfloor = (float)c->sqrt_floor;
+        set_axis_geometry(c, a, 0, l.n[0]);
+        if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    }
+    return potential_spectrum(c);
+}
+
 // capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
 int build_step_graph(sn_ctx *c)
 {
@@ -579,7 +606,7 @@ int build_step_graph(sn_ctx *c)
     const int64_t before = c->launches;
     SN_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->cap_stream;
-    int rc = potential_spectrum(c);
+    int rc = prepare_n(c, NL_MAIN);
     if (rc == SN_OK) rc = kinetic_sweep(c, PH_FULL, /*with_nl=*/true, /*before_n=*/true);
     c->stream = user;
     cudaGraph_t g = nullptr;
@@ -684,7 +711,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
     c->vext = reinterpret_cast<float *>(c->ws + l.off_vext);
     c->bg = reinterpret_cast<float2 *>(c->ws + l.off_bg);
-    c->rho_floor = 1e-30; c->p_pow = 1.0;
+    c->rho_floor = 1e-30; c->p_pow = 1.0; c->sqrt_floor = 1e-30;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
         for (int sl = 0; sl < PH_SLOTS; sl++) c->ph[sl][d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph[sl][d]);
@@ -771,6 +798,17 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
     return upload_phase_tables(c);
 }
 
+int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
+{
+    if (!c) return SN_ERR_NULL;
+    if (!std::isfinite(c_bohm) || !std::isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SN_ERR_PARAM;
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c);
+    c->c_bohm = c_bohm;
+    c->sqrt_floor = sqrt_floor;
+    return SN_OK;
+}
+
 int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int src_on_device)
 {
     if (!c) return SN_ERR_NULL;
@@ -835,7 +873,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
         }
     }
     for (; rc == SN_OK && i <= nsteps; i++) {
-        rc = potential_spectrum(c);
+        rc = prepare_n(c, NL_MAIN);
         if (rc == SN_OK) rc = kinetic_sweep(c, i == nsteps ? PH_HALF : PH_FULL, /*with_nl=*/true, /*before_n=*/i < nsteps);
     }
     return rc;
@@ -851,11 +889,11 @@ int sn_step_order4(sn_ctx *c, int64_t nsteps)
     // K(w1/2) [N(w1) K((w1+w0)/2) N(w0) K((w0+w1)/2) N(w1) K(w1 or w1/2)]^n
     int rc = kinetic_sweep(c, PH_Y_END, /*with_nl=*/false, /*before_n=*/true, NL_MAIN, NL_Y1);
     for (int64_t i = 1; rc == SN_OK && i <= nsteps; i++) {
-        rc = potential_spectrum(c);
+        rc = prepare_n(c, NL_Y1);
         if (rc == SN_OK) rc = kinetic_sweep(c, PH_Y_MID, true, true, NL_Y1, NL_Y0);
-        if (rc == SN_OK) rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = prepare_n(c, NL_Y0);
         if (rc == SN_OK) rc = kinetic_sweep(c, PH_Y_MID, true, true, NL_Y0, NL_Y1);
-        if (rc == SN_OK) rc = potential_spectrum(c);
+        if (rc == SN_OK) rc = prepare_n(c, NL_Y1);
         if (rc == SN_OK) rc = kinetic_sweep(c, i == nsteps ? PH_Y_END : PH_Y_JOIN, true, /*before_n=*/i < nsteps, NL_Y1, NL_Y1);
     }
     return rc;

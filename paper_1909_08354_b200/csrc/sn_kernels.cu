@@ -174,6 +174,10 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
                 const float4 v = psi4[(long long)(j + T * m) * rs4 + CP + t];
                 a[m] = make_float2(abs2(lo2(u)), abs2(hi2(u)));
                 b[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+                if (p.sqrt_rho) { // Bohm term: the transform of sqrt(rho)
+                    a[m] = make_float2(sqrtf(a[m].x), sqrtf(a[m].y));
+                    b[m] = make_float2(sqrtf(b[m].x), sqrtf(b[m].y));
+                }
             }
         }
         fft_pair<N, +1, false>(a, b, j, p.tw, sm);
@@ -238,6 +242,22 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
         }
         double v[3] = {(double)s_rho, (double)s_pr, (double)s_f};
         block_accumulate<3>(v, p.diag);
+        return;
+    }
+
+    if (MODE == P_H_BOHM) { // fa, fb hold W = lap sqrt(rho): rotate psi by -s c_B W/(2 max(sqrt(rho), floor))
+#pragma unroll
+        for (int half = 0; half < 2; half++) {
+            float4 *g4 = psi4 + half * CP + t;
+#pragma unroll
+            for (int m = 0; m < P; m++) {
+                const float4 v = g4[(long long)(j + T * m) * rs4];
+                const float2 w = half == 0 ? fa[m] : fb[m];
+                const float2 x0 = rotate_half_angle(lo2(v), p.hbohm * w.x / fmaxf(sqrtf(abs2(lo2(v))), p.sfloor));
+                const float2 x1 = rotate_half_angle(hi2(v), p.hbohm * w.y / fmaxf(sqrtf(abs2(hi2(v))), p.sfloor));
+                g4[(long long)(j + T * m) * rs4] = pack4(x0, x1);
+            }
+        }
         return;
     }
 
@@ -388,12 +408,14 @@ int launch_pass(const PassArgs &a)
     case P_H_R2C:
     case P_H_POT:
     case P_H_SRC:
+    case P_H_BOHM:
     case P_H_DIAG: {
         const unsigned grid = (unsigned)(a.ncols / (4 * CP));
         if (a.kind == P_H_NLKIN) return launch_kernel(k_haxis<N, CP, P_H_NLKIN>, grid, ST, SSMEM, a);
         if (a.kind == P_H_R2C) return launch_kernel(k_haxis<N, CP, P_H_R2C>, grid, ST, SSMEM, a);
         if (a.kind == P_H_POT) return launch_kernel(k_haxis<N, CP, P_H_POT>, grid, ST, SSMEM, a);
         if (a.kind == P_H_SRC) return launch_kernel(k_haxis<N, CP, P_H_SRC>, grid, ST, SSMEM, a);
+        if (a.kind == P_H_BOHM) return launch_kernel(k_haxis<N, CP, P_H_BOHM>, grid, ST, SSMEM, a);
         return launch_kernel(k_haxis<N, CP, P_H_DIAG>, grid, ST, SSMEM, a);
     }
     case P_X_FFT:

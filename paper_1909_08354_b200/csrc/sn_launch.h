@@ -18,7 +18,8 @@ enum PassKind {
     P_X_KIN,       // contiguous axis: forward -> kinetic phase -> inverse
     P_X_POISSON,   // contiguous axis of the half spectrum: forward -> D/(C-k^2) -> inverse (S5-S7)
     P_X_KDIAG,     // contiguous axis: forward, accumulate sum k_x^2 |psi^|^2
-    P_H_SRC        // axis 0: c2r of F[lap rho] -> s = gamma rho + beta lap rho -> packed r2c   (eq. (12), NEXT-1)
+    P_H_SRC,       // axis 0: c2r of F[lap rho] -> s = gamma rho + beta lap rho -> packed r2c   (eq. (12), NEXT-1)
+    P_H_BOHM       // axis 0: c2r of F[lap sqrt(rho)] -> psi *= exp(-i s c_B lap sqrt(rho)/(2 sqrt(rho)))  (eq. (15))
 };
 
 // Nonlinear phase psi *= exp(-i dtau (B phi + sum_j g_j rho^j)), stored as HALF-angle
@@ -59,6 +60,8 @@ struct PassArgs {
     const float *vext;      // DEVICE: external potential (same layout as psi, float) or nullptr
     const float2 *bg;       // DEVICE: P_H_SRC source tables of eq. (12), interleaved (beta, gamma) per cell, layout of psi
     int lap;                // P_X_POISSON: multiply by -k^2 * pscale instead of pscale/(C - k^2)
+    int sqrt_rho;           // P_H_R2C: transform sqrt(rho) instead of rho (Bohm term)
+    float hbohm, sfloor;    // P_H_BOHM: half angle = hbohm * W / max(sqrt(rho), sfloor), hbohm = -s c_B/4; floor of sqrt(rho)
     double *diag;           // DEVICE: accumulators
     cudaStream_t stream;
 };
@@ -115,6 +118,7 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
     case P_H_NLKIN:
     case P_H_R2C:
     case P_H_SRC:
+    case P_H_BOHM:
         return ncols % (2 * pipe_groups(N)) == 0; // a tile is 2 G columns wide
     case P_X_KIN:
     case P_X_POISSON:

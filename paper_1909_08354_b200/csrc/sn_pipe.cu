@@ -275,7 +275,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
     constexpr int P = g_::P, TILE_BYTES = g_::TILE_BYTES, PIPE_WARPS = g_::NWARP, T = g_::T, G = g_::G, CPW = g_::CPW, RBY = g_::RBY, SUB = g_::SUB, RB = g_::RB, NBOX = g_::NBOX, NST = 2;
     constexpr int STAGE_BYTES = TILE_BYTES + SUB * g_::HS_SUB_BYTES;
     constexpr bool LOAD_HS = true;
-    static_assert(MODE == P_H_NLKIN, "k_pipe_haxis serves P_H_NLKIN");
+    static_assert(MODE == P_H_NLKIN || MODE == P_H_BOHM, "k_pipe_haxis serves P_H_NLKIN and P_H_BOHM");
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
@@ -344,18 +344,30 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
                 issue_load(k + 1);
             }
             float2 a[P], c[P];
+            if (MODE == P_H_BOHM) {
+                // z = W = lap sqrt(rho) of the thread's two columns: psi *= exp(-i s c_B W/(2 max(sqrt(rho), floor))),
+                // eq. (15); each thread rewrites only its own slots
 #pragma unroll
-            for (int m = 0; m < P; m++) {
-                const float4 v = mine[CPW * T * m];
-                a[m] = nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl);
-                c[m] = nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl);
+                for (int m = 0; m < P; m++) {
+                    const float4 v = mine[CPW * T * m];
+                    a[m] = rotate_half_angle(lo2(v), p.a.hbohm * z[m].x / fmaxf(sqrtf(abs2(lo2(v))), p.a.sfloor));
+                    c[m] = rotate_half_angle(hi2(v), p.a.hbohm * z[m].y / fmaxf(sqrtf(abs2(hi2(v))), p.a.sfloor));
+                    mine[CPW * T * m] = pack4(a[m], c[m]);
+                }
+            } else {
+#pragma unroll
+                for (int m = 0; m < P; m++) {
+                    const float4 v = mine[CPW * T * m];
+                    a[m] = nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl);
+                    c[m] = nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl);
+                }
+                fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+                apply_phase<T, P>(a, c, jf, p.a.phase);
+                fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
+                __syncwarp();
+#pragma unroll
+                for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
             }
-            fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-            apply_phase<T, P>(a, c, jf, p.a.phase);
-            fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
-            __syncwarp();
-#pragma unroll
-            for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
         }
         warp_arrive_done(done + b);
 
@@ -432,6 +444,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_r2c(const __grid_co
             for (int m = 0; m < P; m++) {
                 const float4 v = mine[CPW * T * m];
                 z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
+                if (p.a.sqrt_rho) z[m] = make_float2(sqrtf(z[m].x), sqrtf(z[m].y)); // Bohm term: transform of sqrt(rho)
             }
         }
         __syncwarp();
@@ -791,6 +804,7 @@ int launch_pipe(const PipeArgs &a)
                                       : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, NT, S2H, a);
         case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, NT, S2H, a);
         case P_H_SRC: return launch_pipe_kernel(k_pipe_src<N>, NT, S2H + 0, a);
+        case P_H_BOHM: return launch_pipe_kernel(k_pipe_haxis<N, P_H_BOHM, false>, NT, S2H, a);
         default: break;
         }
     }

@@ -23,10 +23,10 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
-              "X_KDIAG", "H_SRC")
+              "X_KDIAG", "H_SRC", "H_BOHM")
 
 
 class SnDiag(ctypes.Structure):
@@ -80,6 +80,7 @@ def lib() -> ctypes.CDLL:
         L.sn_set_local_terms.argtypes = [vp, ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_double]
         L.sn_set_external_potential.argtypes = [vp, vp, ctypes.c_int]
         L.sn_set_source_tables.argtypes = [vp, vp, vp, ctypes.c_int]
+        L.sn_set_bohm.argtypes = [vp, ctypes.c_double, ctypes.c_double]
         _lib = L
     return _lib
 
@@ -230,6 +231,10 @@ class Simulation:
             assert v.dtype == torch.float32 and v.is_contiguous() and tuple(v.shape) == self.dims
             _chk(lib().sn_set_external_potential(self._h, ctypes.c_void_p(v.data_ptr()), 1 if v.is_cuda else 0),
                  "sn_set_external_potential")
+
+    def set_bohm(self, c_bohm: float, sqrt_floor: float = 1e-30) -> None:
+        """c_bohm * V_B in the N sub-step, V_B = lap sqrt(rho)/(2 max(sqrt(rho), sqrt_floor)) (eq. (15))."""
+        _chk(lib().sn_set_bohm(self._h, float(c_bohm), float(sqrt_floor)), "sn_set_bohm")
 
     def set_source_tables(self, beta, gamma) -> None:
         """eq. (12): lap phi + C phi = D (gamma(x) rho + beta(x) lap rho); numpy float32 arrays or CUDA float32

@@ -368,3 +368,65 @@ def test_plane_wave_full_size_with_next_terms(mods, dims, C, order4):
         num += float(np.sum(np.abs(g1[i:i + (1 << 24)] - w) ** 2))
         den += float(np.sum(np.abs(w) ** 2))
     assert np.sqrt(num / den) < 2e-5
+
+
+# ------------------------------------------------------------------ Bohm quantum potential of eq. (15)
+
+def smooth_positive_state(inputs, dims, Ls):
+    """rho = 1 + 0.3 cos(q1.x) + 0.2 cos(q2.x) > 0 everywhere, phase 0.25 sin(q3.x): no nodes, so V_B is well conditioned
+    (a state with interference zeros makes lap sqrt(rho)/sqrt(rho) singular and fp32 and fp64 runs decorrelate)."""
+    nd = len(dims)
+    X = np.meshgrid(*[inputs.coords(n, L) for n, L in zip(dims, Ls)], indexing="ij")
+    ph = lambda m: sum(2 * np.pi / L * mi * x for mi, x, L in zip(m, X, Ls))
+    rho = 1.0 + 0.3 * np.cos(ph((1, 2, -1)[:nd])) + 0.2 * np.cos(ph((-2, 1, 1)[:nd]))
+    return (np.sqrt(rho) * np.exp(0.25j * np.sin(ph((1, -1, 2)[:nd])))).astype(np.complex64)
+
+
+@pytest.mark.parametrize("dims,steps,order4", [((256, 256), 60, False), ((64, 128, 64), 30, False), ((512, 128), 30, False),
+                                               ((128, 96), 30, True), ((2048, 64), 10, False)])
+def test_bohm_term_matches_oracle(mods, dims, steps, order4):
+    """The Bohm phase is a derivative-dependent potential treated explicitly: dtau c_B k_max^2 must stay small or the
+    scheme itself (oracle included) amplifies grid-scale noise; h = 0.15 on every axis keeps it at 0.2 per step."""
+    Oracle, inputs, sn = mods
+    Ls = tuple(0.15 * n for n in dims)
+    psi0 = smooth_positive_state(inputs, dims, Ls)
+    par = dict(A=-0.5, B=1.0, C=-1.0, D=0.5, g=(0.1,), dtau=2e-3)
+    sim = sn.Simulation(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"])
+    sim.set_bohm(0.4, 1e-3)
+    sim.set_state(psi0)
+    d0 = sim.diagnostics()
+    (sim.step_order4 if order4 else sim.step)(steps)
+    got = sim.get_state()
+    d1 = sim.diagnostics()
+    sim.close()
+    orc = Oracle(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"])
+    orc.set_bohm(0.4, 1e-3)
+    orc.set_state(psi0.astype(np.complex128))
+    (orc.step_order4 if order4 else orc.step)(steps)
+    want = orc.get_state()
+    orc.set_bohm(0.0, 1e-3)
+    orc.set_state(psi0.astype(np.complex128))
+    (orc.step_order4 if order4 else orc.step)(steps)
+    without = orc.get_state()
+    orc.close()
+    assert rel(want, without) > 1e-4                       # the term matters in this run
+    assert rel(got, want) < TOL_STATE
+    assert abs(d1["norm"] - d0["norm"]) < TOL_NORM * d0["norm"]
+
+
+def test_bohm_term_makes_real_states_stationary(mods):
+    """c_B = -2A cancels the quantum pressure: the Gaussian that spreads under K alone stays put (pin W7)."""
+    Oracle, inputs, sn = mods
+    dims, L, s, a = (128, 128), 24.0, 1.7, 0.8
+    X = np.meshgrid(*[inputs.coords(n, L) for n in dims], indexing="ij")
+    psi0 = (a * np.exp(-(X[0] ** 2 + X[1] ** 2) / (2 * s * s))).astype(np.complex64)
+    sim = sn.Simulation(dims, L, -0.5, 0.0, 0.0, 0.0, (), 1e-2)
+    sim.set_state(psi0)
+    sim.step(100)
+    assert rel(sim.get_state(), psi0) > 0.1               # spreads without the Bohm term
+    sim.set_bohm(1.0, 1e-4)
+    sim.set_state(psi0)
+    sim.step(100)
+    assert rel(sim.get_state(), psi0) < 2e-4               # stationary with it (fp32 transform noise in the tails)
+    sim.set_bohm(0.0, 1e-4)
+    sim.close()
