@@ -389,7 +389,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
 // Memory-bound (12 B/cell, one single-line FFT per column pair), so the two rings are decoupled:
 // a psi stage is reloaded as soon as every warp has pulled its values into registers, and the
 // transform runs in the OUTPUT buffer (a group's N/2+1 output slots hold its N float2 positions).
-template <int N>
+template <int N, bool SQRT>
 __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_r2c(const __grid_constant__ PipeArgs p)
 {
     using g_ = Geo<N>;
@@ -444,7 +444,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_r2c(const __grid_co
             for (int m = 0; m < P; m++) {
                 const float4 v = mine[CPW * T * m];
                 z[m] = make_float2(abs2(lo2(v)), abs2(hi2(v)));
-                if (p.a.sqrt_rho) z[m] = make_float2(sqrtf(z[m].x), sqrtf(z[m].y)); // Bohm term: transform of sqrt(rho)
+                if (SQRT) z[m] = make_float2(sqrtf(z[m].x), sqrtf(z[m].y)); // Bohm term: transform of sqrt(rho)
             }
         }
         __syncwarp();
@@ -802,7 +802,9 @@ int launch_pipe(const PipeArgs &a)
         case P_H_NLKIN:
             return (a.a.nl.flags & 1) ? launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, true>, NT, S2H, a)
                                       : launch_pipe_kernel(k_pipe_haxis<N, P_H_NLKIN, false>, NT, S2H, a);
-        case P_H_R2C: return launch_pipe_kernel(k_pipe_r2c<N>, NT, S2H, a);
+        case P_H_R2C:
+            return a.a.sqrt_rho ? launch_pipe_kernel(k_pipe_r2c<N, true>, NT, S2H, a)
+                                : launch_pipe_kernel(k_pipe_r2c<N, false>, NT, S2H, a);
         case P_H_SRC: return launch_pipe_kernel(k_pipe_src<N>, NT, S2H + 0, a);
         case P_H_BOHM: return launch_pipe_kernel(k_pipe_haxis<N, P_H_BOHM, false>, NT, S2H, a);
         default: break;
