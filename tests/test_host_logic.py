@@ -82,6 +82,13 @@ def test_null_context_calls(lib):
     assert lib.sn_destroy(None) == -1
     assert lib.sn_debug_fft(None, 1) == -1
     assert lib.sn_launch_count(None) == 0
+    assert lib.sn_step_order4(None, 1) == -1
+    assert lib.sn_set_local_terms(None, 0.0, 0.0, 1.0, 1e-6) == -1
+    assert lib.sn_set_external_potential(None, None, 0) == -1
+    assert lib.sn_set_source_tables(None, None, None, 0) == -1
+    assert lib.sn_set_bohm(None, 0.0, 1e-6) == -1
+    assert lib.sn_profile(None, 1) == -1
+    assert lib.sn_debug_potential(None, None, 0) == -1
     assert lib.sn_strerror(-4).decode().startswith("C > 0")
     assert lib.sn_strerror(0).decode() == "ok"
 
