@@ -430,3 +430,62 @@ def test_bohm_term_makes_real_states_stationary(mods):
     assert rel(sim.get_state(), psi0) < 2e-4               # stationary with it (fp32 transform noise in the tails)
     sim.set_bohm(0.0, 1e-4)
     sim.close()
+
+
+@pytest.mark.parametrize("dims,batch,steps", [((128, 64), 3, 30), ((64, 64, 64), 2, 16)])
+def test_bohm_term_in_an_ensemble(mods, dims, batch, steps):
+    """The Bohm chain (sqrt(rho) r2c, Laplacian multiplier, axis-0 phase pass) on the ensemble layout: each member
+    matches the single-system oracle."""
+    Oracle, inputs, sn = mods
+    Ls = tuple(0.15 * n for n in dims)
+    par = dict(A=-0.5, B=1.0, C=-1.0, D=0.5, g=(0.1,), dtau=2e-3)
+    base = smooth_positive_state(inputs, dims, Ls)
+    members = [(np.roll(base, 5 * b, axis=len(dims) - 1) * np.complex64(0.8 + 0.15 * b)).astype(np.complex64)
+               for b in range(batch)]
+    sim = sn.Simulation(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"], batch=batch)
+    sim.set_bohm(0.4, 1e-3)
+    sim.set_state(np.ascontiguousarray(np.stack(members, axis=1)))
+    sim.step(steps)
+    got = sim.get_state()
+    sim.close()
+    for b in range(batch):
+        orc = Oracle(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"])
+        orc.set_bohm(0.4, 1e-3)
+        orc.set_state(members[b].astype(np.complex128))
+        orc.step(steps)
+        assert rel(got[:, b], orc.get_state()) < TOL_STATE, b
+        orc.close()
+
+
+@pytest.mark.parametrize("dims,order4", [((128, 128), False), ((64, 96, 64), False), ((256, 64), True)])
+def test_every_term_at_once(mods, dims, order4):
+    """Eq. (12) source tables, eq. (15)/(16) log and power terms, external potential and Bohm term in one run."""
+    Oracle, inputs, sn = mods
+    Ls = tuple(0.15 * n for n in dims)
+    nd = len(dims)
+    X = np.meshgrid(*[inputs.coords(n, L) for n, L in zip(dims, Ls)], indexing="ij")
+    ph = lambda m: sum(2 * np.pi / L * mi * x for mi, x, L in zip(m, X, Ls))
+    beta = (1.0 + 0.2 * np.cos(ph((1, 0, 1)[:nd]))).astype(np.float32)
+    gamma = (0.05 * np.sin(ph((0, 1, 1)[:nd]))).astype(np.float32)
+    V = (0.3 * np.cos(ph((1, 1, 0)[:nd]))).astype(np.float32)
+    psi0 = smooth_positive_state(inputs, dims, Ls)
+    par = dict(A=-0.5, B=1.0, C=-1.0, D=0.5, g=(0.1, -0.02), dtau=2e-3)
+    steps = 20
+
+    def drive(o, cast):
+        o.set_local_terms(0.04, 1e-12, 0.03, 0.5)
+        o.set_source_tables(cast(beta), cast(gamma))
+        o.set_external_potential(cast(V))
+        o.set_bohm(0.3, 1e-3)
+        o.set_state(psi0.astype(np.complex128) if cast is f64 else psi0)
+        (o.step_order4 if order4 else o.step)(steps)
+        return o.get_state()
+
+    f64 = lambda a: a.astype(np.float64)
+    sim = sn.Simulation(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"])
+    got = drive(sim, lambda a: a)
+    sim.close()
+    orc = Oracle(dims, Ls, par["A"], par["B"], par["C"], par["D"], par["g"], par["dtau"])
+    want = drive(orc, f64)
+    orc.close()
+    assert rel(got, want) < TOL_STATE
