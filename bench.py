@@ -336,7 +336,7 @@ def main():
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras else None,
-                "traffic_source": "ncu --set full dram bytes per launch, profiles/r01c_ncu_full_C5_512.md",
+                "traffic_source": "ncu --set full dram bytes per launch, profiles/r01c_ncu_full_C5_512.md (re-captured at round end, same values: r01g)",
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
                 "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot,
