@@ -133,10 +133,20 @@ def oracle_rate(cfg_name: str, budget_s: float, inputs):
     t0 = time.perf_counter()
     orc.step(k)
     dt = time.perf_counter() - t0
+    cores = snref.num_threads()
+    # the same program on ONE host thread too (the paper's single-thread comparison, Fig. 1):
+    # a third of the budget, at least two steps
+    snref.set_num_threads(1)
+    k1 = int(max(2, min(k, budget_s / 3.0 / max(t1 * cores, 1e-6))))
+    t0 = time.perf_counter()
+    orc.step(k1)
+    dt1 = time.perf_counter() - t0
+    snref.set_num_threads(cores)
     orc.close()
-    return {"value": cfg.cells * k / dt, "unit": UNIT, "cores": snref.num_threads(), "kind": "oracle",
+    return {"value": cfg.cells * k / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{base.name} recipe on a {'x'.join(map(str, cfg.dims))} grid, {k} Strang steps, float64, "
-                      f"{dt:.1f} s wall"}, cfg, k, dt
+                      f"{dt:.1f} s wall",
+            "single_thread": {"value": cfg.cells * k1 / dt1, "steps": k1, "wall_s": dt1}}, cfg, k, dt
 
 
 def run_reference(args, inputs):
