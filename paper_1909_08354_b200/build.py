@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsn.so")
 LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)   # pipelined + first-path kernels
-LENGTHS3 = (96, 384, 1536)                         # 6*4^a: 12 points per thread
+LENGTHS3 = (96, 192, 384, 768, 1536, 3072)        # 3*2^a: 12 points per thread
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
          "-Xcompiler", "-fPIC", "-diag-suppress", "128"]

@@ -31,11 +31,11 @@ const double NL_LEN[NL_SLOTS] = {1.0, YW1, YW0};
 
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
-// supported line lengths: 2^n in [64, 4096] and 6*4^a (96, 384, 1536); keep in step with build.py LENGTHS
+// supported line lengths: 2^n in [64, 4096] and 3*2^a in [96, 3072]; keep in step with build.py LENGTHS
 inline bool len_ok(int64_t n)
 {
     if (n >= 64 && n <= 4096 && (n & (n - 1)) == 0) return true;
-    return n == 96 || n == 384 || n == 1536;
+    return n == 96 || n == 192 || n == 384 || n == 768 || n == 1536 || n == 3072;
 }
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
@@ -43,7 +43,12 @@ inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 int radix_for(int N, int ns)
 {
     const int rem = N / ns;
-    if (N % 3 == 0) return rem == 6 ? 6 : 4;
+    if (N % 3 == 0) {
+        if (rem == 6) return 6;
+        int m = N / 6;
+        while (m % 4 == 0) m /= 4;
+        return (ns == 1 && m == 2) ? 2 : 4;
+    }
     return rem >= 8 ? 8 : rem;
 }
 
@@ -339,6 +344,9 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
             case 96: rc = snk::launch_pipe<96>(pa); break;
             case 384: rc = snk::launch_pipe<384>(pa); break;
             case 1536: rc = snk::launch_pipe<1536>(pa); break;
+            case 192: rc = snk::launch_pipe<192>(pa); break;
+            case 768: rc = snk::launch_pipe<768>(pa); break;
+            case 3072: rc = snk::launch_pipe<3072>(pa); break;
             case 64: rc = snk::launch_pipe<64>(pa); break;
             case 128: rc = snk::launch_pipe<128>(pa); break;
             case 256: rc = snk::launch_pipe<256>(pa); break;
@@ -357,6 +365,9 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
     case 96: rc = snk::launch_pass<96>(a); break;
     case 384: rc = snk::launch_pass<384>(a); break;
     case 1536: rc = snk::launch_pass<1536>(a); break;
+    case 192: rc = snk::launch_pass<192>(a); break;
+    case 768: rc = snk::launch_pass<768>(a); break;
+    case 3072: rc = snk::launch_pass<3072>(a); break;
     case 64: rc = snk::launch_pass<64>(a); break;
     case 128: rc = snk::launch_pass<128>(a); break;
     case 256: rc = snk::launch_pass<256>(a); break;
@@ -1024,7 +1035,7 @@ const char *sn_strerror(int code)
     switch (code) {
     case SN_OK: return "ok";
     case SN_ERR_NULL: return "null pointer argument";
-    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths 2^n in [64, 4096] or 96, 384, 1536)";
+    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths 2^n in [64, 4096] or 3*2^a in [96, 3072])";
     case SN_ERR_PARAM: return "invalid parameter";
     case SN_ERR_SINGULAR: return "C > 0 coincides with k^2 of a grid mode: eq. (2) is singular";
     case SN_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";

@@ -2,7 +2,7 @@
 //
 // The "Fourier methods" of PAPER.md:113 (section III) are hand-written here: one line of
 // N = 2^n complex64 points is held by T = N/8 threads, 8 points per thread in registers
-// (N = 6*4^a: T = N/12 threads, 12 points per thread, radix-4 stages and a final radix-6 stage
+// (N = 3*2^a: T = N/12 threads, 12 points per thread, radix-4 stages and a final radix-6 stage
 // done as 2 x 3 with prime-factor index maps).
 // Every thread carries TWO independent lines (a[], b[]) so that each twiddle load, each
 // shared-memory instruction (128-bit: one point of each line) and each index computation is
@@ -157,12 +157,19 @@ __device__ __forceinline__ void butterfly(float2 (&x)[P], int q)
 }
 
 // Engine shape per length.  N = 2^n: 8 points per thread and line, radix-8 stages with a trailing
-// radix-4/2.  N = 6 * 4^a (96, 384, 1536): 12 points per thread, radix-4 stages and a final radix-6.
+// radix-4/2.  N = 3 * 2^a (96 ... 3072): 12 points per thread, radix-4 stages (after one leading radix-2 stage
+// when N/6 is not a power of 4) and a final radix-6.
 __host__ __device__ constexpr int ppt_for(int N) { return N % 3 == 0 ? 12 : 8; }
 __host__ __device__ constexpr int radix_for(int N, int NS)
 {
     const int rem = N / NS;
-    if (N % 3 == 0) return rem == 6 ? 6 : 4;
+    if (N % 3 == 0) {
+        if (rem == 6) return 6;
+        // N/6 = 2 * 4^a (192, 768, 3072): one leading radix-2 stage (untwiddled), then radix 4
+        int m = N / 6;
+        while (m % 4 == 0) m /= 4;
+        return (NS == 1 && m == 2) ? 2 : 4;
+    }
     return rem >= 8 ? 8 : rem;
 }
 

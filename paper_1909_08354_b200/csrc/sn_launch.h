@@ -76,7 +76,7 @@ template <int N>
 int launch_pass(const PassArgs &a);
 
 // ---- pipelined (persistent, TMA-fed) variants of the hot passes: sn_pipe.cu ----
-// One CTA per SM (512 threads, 64 KB tiles for N = 2^n; 256 threads, 48 KB tiles for N = 6*4^a) walks over the
+// One CTA per SM (512 threads, 64 KB tiles for N = 2^n; 256 threads, 48 KB tiles for N = 3*2^a) walks over the
 // tiles of a pass; tiles are moved by the TMA unit between HBM and a ring of shared-memory stages, so loads and
 // stores of neighbouring tiles overlap the butterflies of the current one.  Kinds served: P_S_FFT, P_S_KIN,
 // P_H_NLKIN, P_H_R2C, P_X_KIN, P_X_POISSON.  Tensor maps view an array as [outer][row][2*cols floats]; a box is
@@ -93,7 +93,7 @@ struct PipeArgs {
 };
 
 // geometry of the pipelined kernels, shared by the scheduler (tensor maps, tile counts) and sn_pipe.cu:
-// 8 points per thread and 512 threads for N = 2^n; 12 points per thread and 256 threads for N = 6*4^a
+// 8 points per thread and 512 threads for N = 2^n; 12 points per thread and 256 threads for N = 3*2^a
 __host__ __device__ constexpr int pipe_ppt(int N) { return N % 3 == 0 ? 12 : 8; }
 __host__ __device__ constexpr int pipe_threads(int N) { return N % 3 == 0 ? 256 : 512; }
 __host__ __device__ constexpr int pipe_groups(int N) { return pipe_threads(N) / (N / pipe_ppt(N)); } // line pairs per tile
@@ -109,7 +109,7 @@ __host__ __device__ constexpr int pipe_box_rows(int rows) // largest divisor of 
 // length in sn_api.cu); otherwise launch_pass<N>
 inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 {
-    // 6*4^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
+    // 3*2^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
     // first-path kernels (2+ CTAs per SM) for the heavy axis-0 pass (0.94 vs 1.24 ms); the others stay first-path
     if (N % 3 == 0 && kind != P_H_NLKIN) return false;
     switch (kind) {

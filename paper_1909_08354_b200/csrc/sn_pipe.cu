@@ -11,7 +11,7 @@
 // k+1/k+2 are landing and tile k-1 is draining.  No register is spent on global addresses.
 //
 // Tile geometry (strided kinds): T = N/P threads carry one PAIR of adjacent columns (a "line pair", one float4 =
-// 2 complex per row; P = 8 points per thread, 12 for N = 6*4^a); G = threads/T groups per CTA; a tile is N rows x
+// 2 complex per row; P = 8 points per thread, 12 for N = 3*2^a); G = threads/T groups per CTA; a tile is N rows x
 // 2G columns, stored as sub-tiles of [N rows][16*CPW bytes], CPW = min(G, 8) column pairs per row.  The TMA
 // swizzle of that width (128B / 64B / 32B / none) puts the 16-byte chunk c of row r at chunk c ^ swz(r), and in
 // every case the bank unit is a bijection of (r & 7): the 8 lanes of a quarter-warp (consecutive rows, same
@@ -40,7 +40,7 @@ struct Geo {
     static constexpr int NWARP = NTHR / 32;
     static constexpr int T = N / P;                       // threads per line pair
     static constexpr int G = NTHR / T;                    // line pairs (groups) per tile
-    static constexpr int TILE_BYTES = N * 2 * G * 8;      // 64 KB (N = 2^n) or 48 KB (N = 6*4^a)
+    static constexpr int TILE_BYTES = N * 2 * G * 8;      // 64 KB (N = 2^n) or 48 KB (N = 3*2^a)
     static constexpr int CPW = G < 8 ? G : 8;             // column pairs per sub-tile row (8 for N <= 512, then 4, 2, 1)
     static constexpr int RBY = 16 * CPW;                  // bytes of a sub-tile row: 128, 64, 32, 16
     static constexpr int SUB = G / CPW;                   // sub-tiles per tile

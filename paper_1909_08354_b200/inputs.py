@@ -140,7 +140,7 @@ def _configs() -> Dict[str, Config]:
                      make=lambda: super_gaussian_noise((4096, 4096), 400.0, 20.0, 0.01, seed=3))
     c["C4"] = Config("C4", (256, 256, 256), 64.0, -0.5, 1.0, 0.0, 4.0 * np.pi, (0.02,), 1e-2, 300,
                      make=lambda: gaussian_blobs((256, 256, 256), 64.0, 16, (1.0, 3.0), (0.1, 0.2), 0.2, seed=4))
-    for n in (64, 128, 256, 384, 512):
+    for n in (64, 128, 192, 256, 384, 512, 768):  # 192 and 768: beyond BASELINE.json's sweep, same recipe
         c[f"C5_{n}"] = _c5(n)
     return c
 

@@ -59,7 +59,8 @@ def run_pair(mods, cfg, steps, split=None):
 
 FFT_DIMS = [(64, 64), (128, 256), (512, 64), (64, 1024), (2048, 64), (64, 4096), (4096, 128),
             (64, 64, 64), (128, 64, 256), (64, 512, 128),
-            (96, 96), (384, 64), (64, 384), (1536, 64), (64, 1536), (96, 384, 64)]   # 6*4^a lengths (radix-6 stage)
+            (96, 96), (384, 64), (64, 384), (1536, 64), (64, 1536), (96, 384, 64),   # 6*4^a lengths (radix-6 stage)
+            (192, 64), (64, 192), (768, 192), (3072, 64), (64, 3072), (192, 64, 768)]  # 12*4^a: leading radix-2 stage
 
 
 @pytest.mark.parametrize("dims", FFT_DIMS)
@@ -155,6 +156,10 @@ STEP_CASES = [
     ("C5_384", (96, 96, 96), 128.0, 20),    # the sweep's 3*2^7 family, coarse
     ("C5_384", (384, 64, 128), 128.0, 4),   # 384-point strided lines next to pipelined axes
     ("C5_384", (64, 128, 384), 128.0, 4),   # 384-point contiguous lines
+    ("C2", (192, 768), 25.0, 60),           # 12*4^a line lengths (leading radix-2 stage) on both axes
+    ("C5_384", (192, 192, 192), 128.0, 6),  # 192^3
+    ("C3", (3072, 64), 50.0, 12),           # 3072-point strided lines
+    ("C4", (64, 768, 192), 16.0, 6),
 ]
 
 
