@@ -53,7 +53,7 @@ typedef struct {
     double norm, e_kin, e_nonlocal, e_local, e_total;
 } sn_diag;
 
-/* Supported axis lengths: powers of two with 64 <= N <= 4096, and 3*2^a with 96 <= N <= 3072 (96, 192, 384, 768,
+/* Supported axis lengths: powers of two with 32 <= N <= 4096, and 3*2^a with 96 <= N <= 3072 (96, 192, 384, 768,
  * 1536, 3072: radix-4 stages, a leading radix-2 stage where needed, and one radix-6 stage; the grid-size sweep's 384^3).  Any other length: sn_workspace_bytes
  * returns 0 and sn_create returns SN_ERR_DIMS.  Bytes of device workspace needed. */
 size_t sn_workspace_bytes(int ndim, const int64_t *dims /* host, ndim entries */);

@@ -15,6 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsn.so")
 LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)   # pipelined + first-path kernels
+LENGTHS_FIRST = (32,)                              # first-path kernels only
 LENGTHS3 = (96, 192, 384, 768, 1536, 3072)        # 3*2^a: 12 points per thread
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
@@ -65,7 +66,7 @@ def _build_locked(force: bool) -> str:
     if not _stale(LIB):
         return LIB
     jobs = [(os.path.join(CSRC, "sn_kernels.cu"), os.path.join(OBJ, f"sn_kernels_{n}.o"), [f"-DSN_LEN={n}"])
-            for n in LENGTHS + LENGTHS3]
+            for n in LENGTHS_FIRST + LENGTHS + LENGTHS3]
     jobs += [(os.path.join(CSRC, "sn_pipe.cu"), os.path.join(OBJ, f"sn_pipe_{n}.o"), [f"-DSN_LEN={n}"])
              for n in LENGTHS + LENGTHS3]
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))

@@ -31,10 +31,11 @@ const double NL_LEN[NL_SLOTS] = {1.0, YW1, YW0};
 
 thread_local char g_cuda_msg[256] = "no CUDA error recorded";
 
-// supported line lengths: 2^n in [64, 4096] and 3*2^a in [96, 3072]; keep in step with build.py LENGTHS
+// supported line lengths: 2^n in [32, 4096] and 3*2^a in [96, 3072]; keep in step with build.py LENGTHS
+// (32: first-path kernels only -- a 64 KB pipelined tile would be 256 columns wide)
 inline bool len_ok(int64_t n)
 {
-    if (n >= 64 && n <= 4096 && (n & (n - 1)) == 0) return true;
+    if (n >= 32 && n <= 4096 && (n & (n - 1)) == 0) return true;
     return n == 96 || n == 192 || n == 384 || n == 768 || n == 1536 || n == 3072;
 }
 inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -266,7 +267,7 @@ int make_tensor_maps(sn_ctx *c)
     const Layout &l = c->lay;
     int rc;
     c->m_ok[0] = c->m_ok[1] = false;
-    if (l.cols0 % (2 * snk::pipe_groups((int)l.n[0])) == 0) {
+    if (l.n[0] >= 64 && l.cols0 % (2 * snk::pipe_groups((int)l.n[0])) == 0) {
         const int n0 = (int)l.n[0], cpw = snk::pipe_cpw(n0);
         if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, snk::pipe_box_rows(n0 / 2), cpw))) return rc;
@@ -274,7 +275,7 @@ int make_tensor_maps(sn_ctx *c)
         if ((rc = make_map(&c->m_bg, c->bg, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         c->m_ok[0] = true;
     }
-    if (l.ndim == 3 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
+    if (l.ndim == 3 && l.n[1] >= 64 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
         const int n1 = (int)l.n[1], cpw = snk::pipe_cpw(n1);
         if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0] * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
         if ((rc = make_map(&c->m_hs1, c->hs, (l.n[0] / 2 + 1) * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
@@ -368,6 +369,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
     case 192: rc = snk::launch_pass<192>(a); break;
     case 768: rc = snk::launch_pass<768>(a); break;
     case 3072: rc = snk::launch_pass<3072>(a); break;
+    case 32: rc = snk::launch_pass<32>(a); break;
     case 64: rc = snk::launch_pass<64>(a); break;
     case 128: rc = snk::launch_pass<128>(a); break;
     case 256: rc = snk::launch_pass<256>(a); break;
@@ -805,7 +807,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
     c->has_vext = v != nullptr;
-    c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0; // the pipelined contiguous pass serves 2^n only
+    c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0 && c->lay.nx >= 64; // the pipelined contiguous pass serves 2^n >= 64 only
     return upload_phase_tables(c);
 }
 
@@ -1035,7 +1037,7 @@ const char *sn_strerror(int code)
     switch (code) {
     case SN_OK: return "ok";
     case SN_ERR_NULL: return "null pointer argument";
-    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths 2^n in [64, 4096] or 3*2^a in [96, 3072])";
+    case SN_ERR_DIMS: return "unsupported dimensions (ndim 2 or 3; axis lengths 2^n in [32, 4096] or 3*2^a in [96, 3072])";
     case SN_ERR_PARAM: return "invalid parameter";
     case SN_ERR_SINGULAR: return "C > 0 coincides with k^2 of a grid mode: eq. (2) is singular";
     case SN_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";

@@ -112,6 +112,7 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
     // 3*2^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
     // first-path kernels (2+ CTAs per SM) for the heavy axis-0 pass (0.94 vs 1.24 ms); the others stay first-path
     if (N % 3 == 0 && kind != P_H_NLKIN) return false;
+    if (N < 64) return false; // 32-point lines: first-path kernels only (no pipelined instantiation)
     switch (kind) {
     case P_S_FFT:
     case P_S_KIN:

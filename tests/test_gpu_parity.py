@@ -60,7 +60,8 @@ def run_pair(mods, cfg, steps, split=None):
 FFT_DIMS = [(64, 64), (128, 256), (512, 64), (64, 1024), (2048, 64), (64, 4096), (4096, 128),
             (64, 64, 64), (128, 64, 256), (64, 512, 128),
             (96, 96), (384, 64), (64, 384), (1536, 64), (64, 1536), (96, 384, 64),   # 6*4^a lengths (radix-6 stage)
-            (192, 64), (64, 192), (768, 192), (3072, 64), (64, 3072), (192, 64, 768)]  # 12*4^a: leading radix-2 stage
+            (192, 64), (64, 192), (768, 192), (3072, 64), (64, 3072), (192, 64, 768),  # 12*4^a: leading radix-2 stage
+            (32, 32), (32, 512), (1024, 32), (32, 32, 32), (64, 32, 96), (32, 128, 32)]  # 32-point lines (first-path kernels)
 
 
 @pytest.mark.parametrize("dims", FFT_DIMS)
@@ -93,7 +94,8 @@ def test_round_trip_on_config_states(mods, name):
 # ------------------------------------------------------------------ eq. (2): potential
 
 @pytest.mark.parametrize("dims,C", [((64, 128), 0.0), ((128, 64), -1.0), ((64, 64, 128), 0.0), ((64, 128, 64), -0.7),
-                                    ((384, 96), 0.0), ((96, 64, 384), -0.7)])
+                                    ((384, 96), 0.0), ((96, 64, 384), -0.7),
+                                    ((32, 32), 0.0), ((32, 64, 32), -0.7)])
 def test_potential_matches_oracle(mods, dims, C):
     snref, Oracle, inputs, sn = mods
     cfg = inputs.scaled(inputs.CONFIGS["C2" if len(dims) == 2 else "C4"], dims, L=16.0)
@@ -160,6 +162,10 @@ STEP_CASES = [
     ("C5_384", (192, 192, 192), 128.0, 6),  # 192^3
     ("C3", (3072, 64), 50.0, 12),           # 3072-point strided lines
     ("C4", (64, 768, 192), 16.0, 6),
+    ("C2", (32, 32), 6.25, 200),            # 32-point lines (first-path kernels only), both axes
+    ("C4", (32, 32, 32), 8.0, 100),
+    ("C4", (32, 256, 32), 16.0, 10),        # 32-point axis-0 and contiguous lines around a pipelined axis
+    ("C3", (512, 32), 25.0, 40),
 ]
 
 

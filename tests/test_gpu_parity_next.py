@@ -38,6 +38,8 @@ CASES = [
     ("C2", (256, 256), 25.0, 200, (0.0, 1e-30, 0.0, 1.0), True),         # phi_C table only
     ("C4", (64, 128, 64), 16.0, 60, (0.02, 1e-12, 0.05, 0.5), True),     # everything on, 3D
     ("C5_384", (96, 64, 64), 128.0, 20, (0.02, 1e-12, 0.0, 1.0), True),  # 6*4^a axis with the extras
+    ("C4", (32, 64, 32), 16.0, 40, (0.02, 1e-12, 0.05, 0.5), True),      # 32-point lines: V on the first-path axis-0 pass
+    ("C2", (64, 32), 12.5, 100, (0.05, 1e-12, 0.0, 1.0), True),
 ]
 
 
@@ -432,7 +434,7 @@ def test_bohm_term_makes_real_states_stationary(mods):
     sim.close()
 
 
-@pytest.mark.parametrize("dims,batch,steps", [((128, 64), 3, 30), ((64, 64, 64), 2, 16)])
+@pytest.mark.parametrize("dims,batch,steps", [((128, 64), 3, 30), ((64, 64, 64), 2, 16), ((32, 32), 7, 30)])
 def test_bohm_term_in_an_ensemble(mods, dims, batch, steps):
     """The Bohm chain (sqrt(rho) r2c, Laplacian multiplier, axis-0 phase pass) on the ensemble layout: each member
     matches the single-system oracle."""
@@ -457,7 +459,8 @@ def test_bohm_term_in_an_ensemble(mods, dims, batch, steps):
         orc.close()
 
 
-@pytest.mark.parametrize("dims,order4", [((128, 128), False), ((64, 96, 64), False), ((256, 64), True)])
+@pytest.mark.parametrize("dims,order4", [((128, 128), False), ((64, 96, 64), False), ((256, 64), True), ((32, 32, 64), False),
+                                         ((64, 32), True)])
 def test_every_term_at_once(mods, dims, order4):
     """Eq. (12) source tables, eq. (15)/(16) log and power terms, external potential and Bohm term in one run."""
     Oracle, inputs, sn = mods

@@ -36,7 +36,7 @@ def test_workspace_bytes(lib):
     # + beta, gamma tables of eq. (12) (4 B each) + FFT tables
     assert cells * 28 < w < cells * 28.2
     assert w % 256 == 0
-    for bad in [(64,), (64, 64, 64, 64), (48, 64), (32, 64), (8192, 64), (64, 100), (0, 64), (160, 64), (6144, 64), (288, 64)]:
+    for bad in [(64,), (64, 64, 64, 64), (48, 64), (16, 64), (8192, 64), (64, 100), (0, 64), (160, 64), (6144, 64), (288, 64)]:
         assert sn.workspace_bytes(bad) == 0
 
 
