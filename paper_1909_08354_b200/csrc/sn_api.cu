@@ -170,6 +170,7 @@ struct sn_ctx {
     snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
     const float *ksq[3], *kother;
     double *diag;
+    int *sched;                             // tile counters of the dynamically scheduled pipelined kernels
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
     bool use_pipe;
     bool pipe_all;  // SN_PIPE_ALL=1: pipelined kernels wherever they are instantiated (tests, A/B runs)
@@ -325,6 +326,7 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
             snk::PipeArgs pa;
             std::memset(&pa, 0, sizeof(pa));
             pa.a = a;
+            pa.sched = c->sched;
             if (strided) {
                 pa.m_data = axis == 1 ? (a.data == c->hs ? c->m_hs1 : c->m_psi[1]) : c->m_psi[0];
                 pa.tiles_per_outer = a.ncols / (2 * snk::pipe_groups(N));
@@ -732,8 +734,10 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     }
     c->kother = reinterpret_cast<const float *>(c->ws + l.off_kother);
     c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
+    c->sched = reinterpret_cast<int *>(c->ws + l.off_diag + 128); // inside the 256-byte block of the diagnostics
     int rc = upload_static_tables(c);
     if (rc == SN_OK) rc = upload_phase_tables(c);
+    if (rc == SN_OK && cudaMemsetAsync(c->sched, 0, 2 * sizeof(int), c->stream) != cudaSuccess) rc = cuda_fail(cudaGetLastError());
     if (rc == SN_OK) {
         int dev = 0;
         const char *ng = std::getenv("SN_NO_GRAPH"); // SN_NO_GRAPH=1: plain stream launches for every grid

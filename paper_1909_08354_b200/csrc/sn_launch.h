@@ -90,6 +90,7 @@ struct PipeArgs {
     int n_tiles;          // tiles of this pass
     int tiles_per_outer;  // strided kinds: column blocks per outer index
     int grid;             // CTAs to launch (<= number of SMs)
+    int *sched;           // device: {next tile, CTAs finished} of the dynamically scheduled kernels (k_pipe_haxis); both 0 between launches
 };
 
 // geometry of the pipelined kernels, shared by the scheduler (tensor maps, tile counts) and sn_pipe.cu:

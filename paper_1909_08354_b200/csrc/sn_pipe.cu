@@ -279,6 +279,10 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
     extern __shared__ uint8_t smem_raw[];
     uint8_t *base = align_1024(smem_raw);
     uint64_t *full = reinterpret_cast<uint64_t *>(base + NST * STAGE_BYTES), *done = full + NST;
+    // tiles are handed out by a device-wide counter (p.sched[0]), not round-robin: measured at 384^3 and 256^3 a
+    // few CTAs of the static schedule ran up to twice as long as the rest (sm__cycles_active min/avg/max
+    // 0.93/1.2/1.9 Mcycles, profiles/r01i).  tile_of[stage] = tile in that stage, -1 = no tile left.
+    volatile int *tile_of = reinterpret_cast<volatile int *>(done + NST);
     const int tid = threadIdx.x, g = tid / T, j = tid % T, s = g / CPW, t = g % CPW;
 
     if (tid == 0) {
@@ -290,10 +294,18 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
     }
     __syncthreads();
 
-    const int nk = (p.n_tiles - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+    bool more = true; // issuer only: the counter has not run out yet
     auto issue_load = [&](int k) {
-        const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
         const int b = k % NST;
+        const int tile = atomicAdd(p.sched, 1);
+        if (tile >= p.n_tiles) {
+            more = false;
+            tile_of[b] = -1;
+            mbar_arrive(full + b); // completes the phase with no bytes: every warp wakes up and sees -1
+            return;
+        }
+        tile_of[b] = tile;
+        const int col0 = tile * 2 * G;
         uint8_t *st = base + b * STAGE_BYTES;
         mbar_arrive_expect_tx(full + b, TILE_BYTES + (LOAD_HS ? g_::HS_TX : 0));
 #pragma unroll
@@ -311,11 +323,11 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
         }
     };
     if (tid == 0) {
-        if (nk > 0) issue_load(0);
-        if (nk > 1) issue_load(1);
+        issue_load(0);
+        if (more) issue_load(1);
     }
 
-    for (int k = 0; k < nk; k++) {
+    for (int k = 0;; k++) {
         const int b = k % NST;
         const uint32_t par = (k / NST) & 1;
         uint8_t *st = base + b * STAGE_BYTES;
@@ -323,6 +335,8 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
         float4 *hsub = reinterpret_cast<float4 *>(st + TILE_BYTES) + s * g_::HS_SUB_F4;
         SmemSub<T, CPW> sm{sub, t, 1 + g};
         mbar_wait(full + b, par);
+        const int tile = tile_of[b];
+        if (tile < 0) break;
 
         const int jf = opaque(j), ji = opaque(j), jz = opaque(j); // per-tile copies: see opaque()
         float4 *mine = sub + nat_slot<CPW>(jf, t);
@@ -339,7 +353,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
             fft_single<N, -1, false>(z, jz, p.a.tw, sm1);
             // z[m] = (phi[col 2t], phi[col 2t+1]) at row j + T m.  The previous tile's store has had the
             // whole c2r to leave its stage: reload it now.
-            if (tid == 0 && k >= 1 && k + 1 < nk) {
+            if (tid == 0 && k >= 1 && more) {
                 bulk_wait_read<0>();
                 issue_load(k + 1);
             }
@@ -373,7 +387,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
 
         if (tid == 0) {
             mbar_wait(done + b, par);
-            const int col0 = (blockIdx.x + k * gridDim.x) * 2 * G;
+            const int col0 = tile * 2 * G;
 #pragma unroll
             for (int ss = 0; ss < SUB; ss++)
 #pragma unroll
@@ -382,7 +396,15 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
             bulk_commit();
         }
     }
-    if (tid == 0) bulk_wait<0>();
+    if (tid == 0) {
+        bulk_wait<0>();
+        // the last CTA to leave rewinds the counters for the next launch on the stream
+        __threadfence();
+        if (atomicAdd(p.sched + 1, 1) == (int)gridDim.x - 1) {
+            p.sched[0] = 0;
+            p.sched[1] = 0;
+        }
+    }
 }
 
 // P_H_R2C (S4, S5): rho = |psi|^2 -> packed real-to-complex transform along axis 0 -> half spectrum.
