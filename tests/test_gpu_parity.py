@@ -200,6 +200,19 @@ def test_split_calls_equal_one_call(mods):
     assert rel(a, b) < 5e-6
 
 
+def test_counter_scheduled_axis0_kernel_over_many_launches(mods):
+    """512 tiles along axis 0 (> 2 per CTA): the pipelined axis-0 kernel takes its tiles from the device-wide counter
+    (DESIGN.md 4.2), which the last CTA rewinds; consecutive launches and separate calls must all start from zero."""
+    snref, Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C4"], (256, 64, 256), L=32.0, steps=6)
+    a, want, s1 = run_pair(mods, cfg, 6)
+    b, _, s2 = run_pair(mods, cfg, 6, split=(1, 2, 3))
+    s1.close()
+    s2.close()
+    assert rel(a, want) < TOL_STATE and rel(b, want) < TOL_STATE
+    assert rel(a, b) < 5e-6
+
+
 # ------------------------------------------------------------------ full-size properties
 
 def plane_wave(inputs, dims, L, mode, amp):
