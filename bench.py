@@ -199,8 +199,22 @@ def main():
                     help="NEXT-1 row: also run with the pressure potential 0.02 ln(rho) (eq. (16)) and the "
                          "phi_C table of eq. (11) as external potential and the beta, gamma tables of eq. (12) "
                          "(DESIGN.md section 8)")
+    ap.add_argument("--repeats", type=int, default=5,
+                    help="timed repetitions of the K-step call (SURVEY.md 8(d): median of >= 5); value = median")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "b200" else args.warmup
+    args.repeats = max(args.repeats, 1)
+
+    # --gpus N without a launcher: become N replica processes (torchrun sets WORLD_SIZE; plain `python bench.py
+    # --gpus 8` must not silently run one replica and print n_gpus 1)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        import socket
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1", "--master-port",
+                                  str(port), os.path.abspath(__file__), *sys.argv[1:]])
 
     from paper_1909_08354_b200 import inputs
     if args.impl == "reference":
@@ -218,6 +232,8 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    if world != args.gpus:
+        raise SystemExit(f"bench.py --gpus {args.gpus} launched with WORLD_SIZE={world}: one rank per GPU")
     # SN_BENCH_BACKEND=gloo: dry run of the multi-rank plumbing on a box with fewer GPUs than ranks (ranks share
     # devices; replicas do not wait on one another).  Default nccl, one rank per GPU, as the driver launches it.
     backend = os.environ.get("SN_BENCH_BACKEND", "nccl")
@@ -251,7 +267,8 @@ def main():
     dev_in = host_in.to(dev, non_blocking=True)
 
     stream = torch.cuda.current_stream()
-    sim = sn.Simulation.from_config(cfg, device=dev, stream=stream, batch=args.batch or None)
+    sim = sn.Simulation.from_config(cfg, device=dev, stream=stream, batch=args.batch or None,
+                                    features=(sn.FEAT_VEXT | sn.FEAT_SOURCE) if args.extras else 0)
     if args.extras:
         # eq. (16) n = 1: V_pressure = w ln(rho), w = 0.02; eq. (11): phi_C = ln[1 - (r0/(r + r0))^lambda], lambda = 1,
         # r0 = 2, radius softened to sqrt(r^2 + 1) (the grid has a point at r = 0)
@@ -271,17 +288,20 @@ def main():
     step(W)                                             # untimed warm-up steps
     barrier()
 
-    # ---- timed region: exactly K Strang steps, state resident in HBM ----
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    n0 = sim.launch_count()
+    # ---- timed region: exactly K Strang steps, state resident in HBM; repeated, each repetition bracketed by
+    # barrier + synchronize with its own event pair; the reported time is the MEDIAN repetition ----
+    reps = []
     with ClockSampler(local) as clk:
-        barrier()
-        e0.record(stream)
-        step(K)
-        e1.record(stream)
-        barrier()
-    launches = sim.launch_count() - n0
-    ms = e0.elapsed_time(e1)
+        for r in range(args.repeats):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            n0 = sim.launch_count()
+            barrier()
+            e0.record(stream)
+            step(K)
+            e1.record(stream)
+            barrier()
+            launches = sim.launch_count() - n0
+            reps.append(e0.elapsed_time(e1))
 
     # ---- per-launch CUDA events over the same K steps (roofline of the dominant kernel) ----
     sim.profile(True)
@@ -301,8 +321,10 @@ def main():
     e2e_s = time.perf_counter() - t0
     sim.close()
 
-    # max over ranks
-    ms, e2e_ms = replicas.max_over_ranks([ms, e2e_s * 1e3], device=dev if backend == "nccl" else "cpu")
+    # max over ranks (per repetition), then the median repetition
+    red = replicas.max_over_ranks(reps + [e2e_s * 1e3], device=dev if backend == "nccl" else "cpu")
+    reps, e2e_ms = red[:-1], red[-1]
+    ms = statistics.median(reps)
 
     if rank == 0:
         cells = cfg.cells * max(1, args.batch)
@@ -339,7 +361,10 @@ def main():
                        "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
                            cells, cells * 8 / 2 ** 20) if cells * 8 > 126e6 else
                        "state fits L2: launch/L2-bound regime, HBM fraction is an effective figure only",
-                       "timed_call": f"one {'sn_step_order4' if args.order4 else 'sn_step'}({K}) (merged half kinetics)"},
+                       "timed_call": f"one {'sn_step_order4' if args.order4 else 'sn_step'}({K}) (merged half kinetics) per "
+                                     f"repetition; value = median of {len(reps)} repetitions"},
+            "repeats": {"n": len(reps), "ms_per_step_median": ms / K, "ms_per_step_min": min(reps) / K,
+                        "ms_per_step_max": max(reps) / K},
             "gpu_launches": launches,
             "clocks": clk.summary(),
             "roofline": {

@@ -20,9 +20,15 @@
  *     memory: state, half-spectrum buffer and tables live in the caller's workspace
  *     (e.g. a torch uint8 tensor), which must stay alive until sn_destroy.
  *   - Every call returns 0 on success or a negative SN_ERR_* code; nothing throws, nothing
- *     calls exit.  On error, outputs are untouched and the context state is unchanged.
+ *     calls exit.  Argument errors (every code except SN_ERR_CUDA) are detected before any
+ *     device work is enqueued: outputs are untouched and the context is unchanged.  After
+ *     SN_ERR_CUDA (a launch or copy failed part-way through a call) the state and the tables of
+ *     the context are undefined: destroy it and create a new one.
  *   - A context is not thread-safe; different contexts are independent.
- *   - All device work is enqueued on the cudaStream_t given to sn_create.
+ *   - All device work is enqueued on the cudaStream_t given to sn_create, on the device that
+ *     owns the workspace: every call switches to that device for its duration and restores the
+ *     caller's current device on return.
+ *   - The library reads no environment variables; every switch is an argument or sn_set_option.
  */
 #ifndef SN_H
 #define SN_H
@@ -42,6 +48,8 @@ extern "C" {
 #define SN_ERR_WORKSPACE -5 /* workspace too small or not 256-byte aligned */
 #define SN_ERR_STATE -6     /* step/get/diagnostics before sn_set_state */
 #define SN_ERR_CUDA -7      /* a CUDA runtime call failed (sticky; text via sn_strerror) */
+#define SN_ERR_NOMEM -8     /* host allocation failed */
+#define SN_ERR_FEATURE -9   /* the call needs a workspace region that was not requested at create (sn_options.features) */
 
 typedef struct sn_ctx sn_ctx; /* opaque host object, owned by the library */
 
@@ -53,10 +61,25 @@ typedef struct {
     double norm, e_kin, e_nonlocal, e_local, e_total;
 } sn_diag;
 
+/* Optional workspace regions.  The stepper itself needs the state (8 B/cell), the half spectrum (~4 B/cell) and
+ * the FFT tables: about 12 B/cell.  Everything else is requested at create time: */
+#define SN_FEAT_STAGING 1u  /* 4 B/cell scratch: host destination of sn_debug_potential, host sources of sn_set_source_tables */
+#define SN_FEAT_VEXT 2u     /* 4 B/cell: the external potential table of sn_set_external_potential */
+#define SN_FEAT_SOURCE 4u   /* 8 B/cell: the interleaved (beta, gamma) tables of sn_set_source_tables */
+#define SN_FEAT_ALL 7u
+
+typedef struct {
+    size_t struct_size;  /* sizeof(sn_options), filled in by the caller (a mismatch is SN_ERR_PARAM) */
+    int64_t batch;       /* ensemble members, >= 1 (see sn_create_batch) */
+    uint32_t features;   /* SN_FEAT_* bits */
+    uint32_t reserved;   /* 0 */
+} sn_options;
+
 /* Supported axis lengths: powers of two with 32 <= N <= 4096, and 3*2^a with 96 <= N <= 3072 (96, 192, 384, 768,
  * 1536, 3072: radix-4 stages, a leading radix-2 stage where needed, and one radix-6 stage; the grid-size sweep's 384^3).  Any other length: sn_workspace_bytes
  * returns 0 and sn_create returns SN_ERR_DIMS.  Bytes of device workspace needed. */
-size_t sn_workspace_bytes(int ndim, const int64_t *dims /* host, ndim entries */);
+size_t sn_workspace_bytes(int ndim, const int64_t *dims /* host, ndim entries */);  /* = options {batch 1, features 0} */
+size_t sn_workspace_bytes_opt(int ndim, const int64_t *dims /* host */, const sn_options *opt /* host */);
 
 /* Create a context.
  *   out          host; receives the context
@@ -70,13 +93,20 @@ int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, doub
               double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
               void *cuda_stream);
 
+/* Same with options (ensemble size, optional workspace regions).  sn_create = {batch 1, features 0};
+ * sn_create_batch = {batch, features 0}. */
+int sn_create_opt(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C,
+                  double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
+                  void *cuda_stream, const sn_options *opt /* host */);
+
 /* Ensemble of `batch` independent systems advanced together ("batched small-grid ensembles";
  * parameter scans such as PAPER.md:131 run many small meshes).  Same constants and dtau for every member.
  * ndim, dims, L: as for sn_create, describing ONE system.  Storage layout of every array of the context (state,
  * external potential, source tables): [dims[0]][batch][dims[1]]([dims[2]]), i.e. the member index sits right after
  * the slowest physical axis, so that the lines of every axis stay dense; member b of a (batch, dims...) array is at
  * [:, b, ...].  No pass runs along the member index.  sn_diagnostics returns the SUM over the ensemble.
- * 1 <= batch <= 2^20; batch = 1 is sn_create. */
+ * 1 <= batch <= 2^20; batch = 1 is sn_create.  An ensemble whose line or column counts do not fit a 32-bit int
+ * (more than 2^31-1 lines along any axis) is rejected with SN_ERR_DIMS. */
 size_t sn_workspace_bytes_batch(int ndim, const int64_t *dims /* host, ndim */, int64_t batch);
 int sn_create_batch(sn_ctx **out, int ndim, const int64_t *dims, int64_t batch, const double *L, double A, double B,
                     double C, double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
@@ -108,13 +138,13 @@ int sn_set_dtau(sn_ctx *ctx, double dtau);
  *   potential V_pressure = w ln(rho) (n = 1) or (n w/(n-1)) rho^(n-1) of eq. (16).  rho_floor > 0 (reading Q15:
  *   the paper does not say how ln(0) is avoided), p_pow != -1.  g_log = g_pow = 0 switches the terms off.
  * sn_set_external_potential: a fixed real potential V(x) (float32, prod(dims) values, layout of psi; host or
- *   device pointer, copied into the workspace) enters the N sub-step as exp(-i s (B phi + G(rho) + V)) -- phi_C
+ *   device pointer, copied into the workspace; needs SN_FEAT_VEXT) enters the N sub-step as exp(-i s (B phi + G(rho) + V)) -- phi_C
  *   of eq. (11),(15).  NULL removes it.  exp(-i s V) commutes with the rest of the N phase, so it is applied by the
  *   contiguous-axis kinetic pass that precedes each N sub-step (by the axis-0 pass when that one is first-path).
  * Both rebuild the nonlinear-phase coefficients; e_local of sn_diagnostics then includes sum (F(rho) + V rho) dV. */
 /* sn_set_source_tables: eq. (12), PAPER.md:92 -- lap phi + C phi = D (gamma(x) rho + beta(x) lap rho) instead of
  *   eq. (2).  beta, gamma: float32, prod(dims) values each, layout of psi, host or device (copied into the
- *   workspace); two NULLs restore eq. (2) (= gamma 1, beta 0).  Costs one more half-spectrum chain and one more
+ *   workspace; needs SN_FEAT_SOURCE, host sources also SN_FEAT_STAGING); two NULLs restore eq. (2) (= gamma 1, beta 0).  Costs one more half-spectrum chain and one more
  *   axis-0 pass per step.  e_nonlocal of sn_diagnostics stays (B/2) sum phi rho dV (no longer a conserved energy
  *   when beta, gamma vary in space: the kernel of phi[rho] is not symmetric). */
 /* sn_set_bohm: the Bohm quantum potential of eq. (15), PAPER.md:102 -- the N sub-step phase gains the factor
@@ -153,11 +183,22 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 13 */, int64_t *lau
 
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */
 
+/* Switches for A/B runs and tests (none changes results beyond rounding).  Takes effect from the next call;
+ * synchronises the stream.
+ *   SN_OPT_GRAPH    1 (default): sn_step(n >= 4) on grids of <= 2^24 cells replays a captured CUDA graph of the
+ *                   interior step; 0: plain stream launches.
+ *   SN_OPT_DISPATCH 0 (default): each pass runs the kernel measured fastest for its line length; 1: first-path
+ *                   kernels (sn_kernels.cu) everywhere; 2: TMA-pipelined kernels (sn_pipe.cu) wherever instantiated. */
+#define SN_OPT_GRAPH 1
+#define SN_OPT_DISPATCH 2
+int sn_set_option(sn_ctx *ctx, int option, int value);
+
 /* In-place d-dimensional FFT of the internal state: direction +1 forward (e^{-i k x}, unscaled),
  * -1 inverse (scaled by 1/prod N).  Uses the same line-FFT engine as sn_step. */
 int sn_debug_fft(sn_ctx *ctx, int direction);
 
-/* phi (float32, prod(dims) values, same layout as psi) solving eq. (2) for the current state. */
+/* phi (float32, prod(dims) values, same layout as psi) solving eq. (2) for the current state.  A host destination
+ * needs SN_FEAT_STAGING. */
 int sn_debug_potential(sn_ctx *ctx, float *phi_out, int dst_on_device);
 
 #ifdef __cplusplus

@@ -6,6 +6,8 @@
 #include "../../include/sn.h"
 #include "sn_launch.h"
 
+#include <algorithm>
+#include <climits>
 #include <cmath>
 #include <cstdlib>
 #include <cstdio>
@@ -70,15 +72,19 @@ struct Layout {
     int64_t pcells; // cells of ONE system (cells = batch * pcells is the storage size)
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
-    size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_kother, off_diag, total;
+    unsigned features; // SN_FEAT_*: which optional regions exist
+    size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_ksq2[3], off_kother[2],
+        off_diag, total;
 };
 
-bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1)
+bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, unsigned features = 0)
 {
     if (!dims || (ndim != 2 && ndim != 3)) return false;
     if (batch < 1 || batch > (1 << 20)) return false;
+    if (features & ~SN_FEAT_ALL) return false;
     L.ndim = ndim;
     L.batch = batch;
+    L.features = features;
     L.pcells = 1;
     for (int d = 0; d < ndim; d++) {
         if (!len_ok(dims[d])) return false;
@@ -91,19 +97,23 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1)
     L.hs_lines = (L.n[0] / 2 + 1) * L.cols0 / L.nx;
     if (L.hs_lines & 1) L.hs_lines++; // line pairs: one dummy line (2D)
     L.hs_elems = L.hs_lines * L.nx;
+    // the kernels index columns, lines and outer blocks with 32-bit ints: reject ensembles that do not fit
+    if (L.cols0 > INT_MAX || L.cells / L.nx > INT_MAX || L.hs_lines > INT_MAX || L.n[0] * batch > INT_MAX) return false;
     size_t o = 0;
     L.off_psi = o; o = align256(o + (size_t)L.cells * 8);
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
-    L.off_phi = o; o = align256(o + (size_t)L.cells * 4);
-    L.off_vext = o; o = align256(o + (size_t)L.cells * 4);
-    L.off_bg = o; o = align256(o + (size_t)L.cells * 8);
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
         for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
         L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
+        L.off_ksq2[d] = o; o = align256(o + (size_t)L.n[d] * 8);
     }
-    L.off_kother = o; o = align256(o + (size_t)L.hs_lines * 4);
+    for (int i = 0; i < 2; i++) { L.off_kother[i] = o; o = align256(o + (size_t)L.hs_lines * 8); }
     L.off_diag = o; o = align256(o + 8 * sizeof(double));
+    // optional regions (sn_options.features)
+    L.off_phi = o; if (features & SN_FEAT_STAGING) o = align256(o + (size_t)L.cells * 4);
+    L.off_vext = o; if (features & SN_FEAT_VEXT) o = align256(o + (size_t)L.cells * 4);
+    L.off_bg = o; if (features & SN_FEAT_SOURCE) o = align256(o + (size_t)L.cells * 8);
     L.total = o;
     return true;
 }
@@ -116,6 +126,15 @@ inline f4 split_hilo(double re, double im)
     r.x = (float)re; r.y = (float)im;
     r.z = (float)(re - (double)r.x);
     r.w = (float)(im - (double)r.y);
+    return r;
+}
+
+struct f2 { float x, y; };
+inline f2 split_real(double v)
+{
+    f2 r;
+    r.x = (float)v;
+    r.y = (float)(v - (double)r.x);
     return r;
 }
 
@@ -159,6 +178,7 @@ struct sn_ctx {
     double c_bohm, sqrt_floor;              // Bohm term of eq. (15): c_B V_B in the N sub-step (0 = off)
     float2 *bg;                             // interleaved (beta, gamma)
     int n_g;
+    int device;                             // the device that owns the workspace: every entry point runs under it
     char *ws;
     cudaStream_t stream;
     bool has_state;
@@ -168,12 +188,14 @@ struct sn_ctx {
     float *phi;
     const float4 *tw[3], *ph[5][3]; // kinetic phase tables per slot (PH_*) and axis
     snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
-    const float *ksq[3], *kother;
+    const float *ksq[3];
+    const float2 *ksq2[3];                  // k_a^2 as hi + lo (Helmholtz denominator, evaluated without cancellation)
+    const float2 *kother[2];                // per half-spectrum line: [0] C - k_other^2, [1] -k_other^2 (Laplacian), hi + lo
     double *diag;
     int *sched;                             // tile counters of the dynamically scheduled pipelined kernels
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
-    bool use_pipe;
-    bool pipe_all;  // SN_PIPE_ALL=1: pipelined kernels wherever they are instantiated (tests, A/B runs)
+    bool use_pipe;  // SN_OPT_DISPATCH != 1
+    bool pipe_all;  // SN_OPT_DISPATCH == 2: pipelined kernels wherever they are instantiated (tests, A/B runs)
     int sm_count;
     CUtensorMap m_psi[2], m_hs1, m_hs0, m_hs0_row, m_bg;
     bool m_ok[2];
@@ -203,6 +225,20 @@ int cuda_fail(cudaError_t e)
         cudaError_t e_ = (call);                        \
         if (e_ != cudaSuccess) return cuda_fail(e_);    \
     } while (0)
+
+// every entry point runs on the device that owns the workspace and restores the caller's device on return
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(int dev)
+    {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != dev) switched = cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard()
+    {
+        if (switched) cudaSetDevice(prev);
+    }
+};
 
 // fold the recorded event pairs into the per-kind sums (synchronises the stream)
 int profile_flush(sn_ctx *c)
@@ -443,32 +479,43 @@ int upload_static_tables(sn_ctx *c)
             ns *= r;
         }
         std::vector<float> ksq(N);
+        std::vector<f2> ksq2(N);
         for (int k = 0; k < N; k++) {
             const double kk = kval(k, N, c->L[d]);
             ksq[k] = (float)(kk * kk);
+            ksq2[k] = split_real(kk * kk);
         }
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d], tw.data(), tw.size() * 16, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq.data(), (size_t)N * 4, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq2[d], ksq2.data(), (size_t)N * 8, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
-    // sum of the non-contiguous axes' k^2 for each contiguous line of the half spectrum
-    std::vector<float> ko(l.hs_lines, 0.f);
+    // Denominator of eq. (2) per contiguous line of the half spectrum, without the contiguous axis' own k^2:
+    // table 0 holds C - k_other^2, table 1 (Laplacian passes of eq. (12),(15)) -k_other^2, both as hi + lo floats
+    // built in double, so that the kernel's (hi - kx_hi) + (lo - kx_lo) is C - k^2 to ~1e-7 RELATIVE even where C > 0
+    // nearly cancels k^2 (a plain float C - k^2 has an absolute error of 1e-7 k^2 there).
+    // Lines of the half spectrum are indexed (k0, member[, k1]); the member index carries no wavenumber.
+    std::vector<f2> ko(l.hs_lines);
     const int64_t h0 = l.n[0] / 2 + 1;
-    // lines of the half spectrum are indexed (k0, member[, k1]); the member index carries no wavenumber
-    for (int64_t k0 = 0; k0 < h0; k0++) {
-        const double a = kval(k0, l.n[0], c->L[0]);
-        for (int64_t b = 0; b < l.batch; b++) {
-            if (l.ndim == 2) {
-                ko[k0 * l.batch + b] = (float)(a * a);
-            } else {
-                for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
-                    const double q = kval(k1, l.n[1], c->L[1]);
-                    ko[(k0 * l.batch + b) * l.n[1] + k1] = (float)(a * a + q * q);
+    for (int tab = 0; tab < 2; tab++) {
+        const double c0 = tab == 0 ? c->C : 0.0;
+        std::fill(ko.begin(), ko.end(), split_real(tab == 0 && c->C != 0.0 ? c->C : -1.0)); // padding line: any finite non-zero value
+        for (int64_t k0 = 0; k0 < h0; k0++) {
+            const double a = kval(k0, l.n[0], c->L[0]);
+            for (int64_t b = 0; b < l.batch; b++) {
+                if (l.ndim == 2) {
+                    ko[k0 * l.batch + b] = split_real(c0 - a * a);
+                } else {
+                    for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
+                        const double q = kval(k1, l.n[1], c->L[1]);
+                        ko[(k0 * l.batch + b) * l.n[1] + k1] = split_real(c0 - (a * a + q * q));
+                    }
                 }
             }
         }
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_kother[tab], ko.data(), ko.size() * 8, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaStreamSynchronize(c->stream));
     }
-    SN_CUDA(cudaMemcpyAsync(c->ws + l.off_kother, ko.data(), ko.size() * 4, cudaMemcpyHostToDevice, c->stream));
     SN_CUDA(cudaMemsetAsync(c->ws + l.off_hs, 0, (size_t)l.hs_elems * 8, c->stream));
     SN_CUDA(cudaStreamSynchronize(c->stream));
     return SN_OK;
@@ -481,7 +528,6 @@ PassArgs base_args(const sn_ctx *c)
     a.hilo = 1;
     a.dir = +1;
     a.scale = 1.f;
-    a.C = (float)c->C;
     a.nl = c->nl;
     a.diag = c->diag;
     a.vext = c->has_vext ? c->vext : nullptr;
@@ -549,7 +595,7 @@ int spectrum_chain(sn_ctx *c, bool lap)
     {
         const int dx = l.ndim - 1;
         PassArgs a = base_args(c);
-        a.kind = snk::P_X_POISSON; a.data = c->hs; a.tw = c->tw[dx]; a.ksq = c->ksq[dx]; a.kother2 = c->kother;
+        a.kind = snk::P_X_POISSON; a.data = c->hs; a.tw = c->tw[dx]; a.ksq2 = c->ksq2[dx]; a.dko = c->kother[lap ? 1 : 0];
         a.nlines = (int)l.hs_lines;
         a.lap = lap ? 1 : 0;
         const double npts = (double)l.pcells; // points of ONE system: the 1/prod(N) of its transforms
@@ -654,6 +700,8 @@ void drop_step_graph(sn_ctx *c)
 
 extern "C" {
 
+static bool options_ok(const sn_options *opt) { return opt && opt->struct_size == sizeof(sn_options) && opt->reserved == 0; }
+
 size_t sn_workspace_bytes(int ndim, const int64_t *dims)
 {
     Layout l;
@@ -666,30 +714,77 @@ size_t sn_workspace_bytes_batch(int ndim, const int64_t *dims, int64_t batch)
     return make_layout(ndim, dims, l, batch) ? l.total : 0;
 }
 
+size_t sn_workspace_bytes_opt(int ndim, const int64_t *dims, const sn_options *opt)
+{
+    Layout l;
+    if (!options_ok(opt)) return 0;
+    return make_layout(ndim, dims, l, opt->batch, opt->features) ? l.total : 0;
+}
+
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch);
+                       int64_t batch, unsigned features);
 
 int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
               const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
 {
-    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, 1);
+    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, 1, 0);
 }
 
 int sn_create_batch(sn_ctx **out, int ndim, const int64_t *dims, int64_t batch, const double *L, double A, double B,
                     double C, double D, const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes,
                     void *cuda_stream)
 {
-    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, batch);
+    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, batch, 0);
+}
+
+int sn_create_opt(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
+                  const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
+                  const sn_options *opt)
+{
+    if (!opt) return SN_ERR_NULL;
+    if (!options_ok(opt)) return SN_ERR_PARAM;
+    if (opt->features & ~SN_FEAT_ALL) return SN_ERR_PARAM;
+    return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, opt->batch,
+                       opt->features);
+}
+
+// reading Q5: C > 0 within 1e-12 (relative) of k^2 of a grid mode makes eq. (2) unsolvable.  Per axis: the distinct
+// k_a^2 values are sorted once, and for every pair (k0^2, k1^2) the remainder C - k0^2 - k1^2 is looked up among the
+// last axis' values (O(N0 N1 log N2) instead of a sweep over all modes).
+static bool helmholtz_singular(const Layout &l, const double *L, double C)
+{
+    const double tol = 1e-12 * std::fmax(1.0, std::fabs(C));
+    std::vector<double> k2[3];
+    for (int d = 0; d < 3; d++) {
+        if (d >= l.ndim) {
+            k2[d].push_back(0.0);
+            continue;
+        }
+        for (int64_t i = 0; i <= l.n[d] / 2; i++) {
+            const double k = kval(i, l.n[d], L[d]);
+            k2[d].push_back(k * k);
+        }
+    }
+    const std::vector<double> &last = k2[l.ndim - 1]; // ascending in i
+    const std::vector<double> &a0 = k2[0], &a1 = l.ndim == 3 ? k2[1] : k2[2];
+    for (double x : a0)
+        for (double y : a1) {
+            const double want = C - x - y;
+            if (want < -tol) break; // y ascending: the remainder only decreases
+            auto it = std::lower_bound(last.begin(), last.end(), want - tol);
+            if (it != last.end() && std::fabs(*it - want) < tol) return true;
+        }
+    return false;
 }
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch)
+                       int64_t batch, unsigned features)
 {
     if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
     Layout l;
-    if (!make_layout(ndim, dims, l, batch)) return SN_ERR_DIMS;
+    if (!make_layout(ndim, dims, l, batch, features)) return SN_ERR_DIMS;
     if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
     if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
         return SN_ERR_PARAM;
@@ -698,22 +793,9 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     for (int j = 0; j < n_g; j++)
         if (!std::isfinite(g[j])) return SN_ERR_PARAM;
     if (workspace_bytes < l.total || ((uintptr_t)d_workspace & 255) != 0) return SN_ERR_WORKSPACE;
-    if (C > 0.0) { // reading Q5: a grid mode with k^2 == C makes eq. (2) unsolvable
-        const double tol = 1e-12 * std::fmax(1.0, std::fabs(C));
-        const int64_t n0 = l.n[0], n1 = l.n[1], n2 = ndim == 3 ? l.n[2] : 1;
-        for (int64_t i0 = 0; i0 <= n0 / 2; i0++) {
-            const double k0 = kval(i0, n0, L[0]);
-            for (int64_t i1 = 0; i1 <= n1 / 2; i1++) {
-                const double k1 = kval(i1, n1, L[1]);
-                for (int64_t i2 = 0; i2 <= n2 / 2; i2++) {
-                    const double k2 = ndim == 3 ? kval(i2, n2, L[2]) : 0.0;
-                    if (std::fabs(C - (k0 * k0 + k1 * k1 + k2 * k2)) < tol) return SN_ERR_SINGULAR;
-                }
-            }
-        }
-    }
+    if (C > 0.0 && helmholtz_singular(l, L, C)) return SN_ERR_SINGULAR;
     sn_ctx *c = new (std::nothrow) sn_ctx;
-    if (!c) return SN_ERR_PARAM;
+    if (!c) return SN_ERR_NOMEM;
     std::memset(c, 0, sizeof(*c));
     c->lay = l;
     for (int d = 0; d < ndim; d++) c->L[d] = L[d];
@@ -723,34 +805,44 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->stream = static_cast<cudaStream_t>(cuda_stream);
     c->psi = reinterpret_cast<float2 *>(c->ws + l.off_psi);
     c->hs = reinterpret_cast<float2 *>(c->ws + l.off_hs);
-    c->phi = reinterpret_cast<float *>(c->ws + l.off_phi);
-    c->vext = reinterpret_cast<float *>(c->ws + l.off_vext);
-    c->bg = reinterpret_cast<float2 *>(c->ws + l.off_bg);
+    c->phi = (features & SN_FEAT_STAGING) ? reinterpret_cast<float *>(c->ws + l.off_phi) : nullptr;
+    c->vext = (features & SN_FEAT_VEXT) ? reinterpret_cast<float *>(c->ws + l.off_vext) : nullptr;
+    c->bg = (features & SN_FEAT_SOURCE) ? reinterpret_cast<float2 *>(c->ws + l.off_bg) : nullptr;
     c->rho_floor = 1e-30; c->p_pow = 1.0; c->sqrt_floor = 1e-30;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
         for (int sl = 0; sl < PH_SLOTS; sl++) c->ph[sl][d] = reinterpret_cast<const float4 *>(c->ws + l.off_ph[sl][d]);
         c->ksq[d] = reinterpret_cast<const float *>(c->ws + l.off_ksq[d]);
+        c->ksq2[d] = reinterpret_cast<const float2 *>(c->ws + l.off_ksq2[d]);
     }
-    c->kother = reinterpret_cast<const float *>(c->ws + l.off_kother);
+    for (int i = 0; i < 2; i++) c->kother[i] = reinterpret_cast<const float2 *>(c->ws + l.off_kother[i]);
     c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
     c->sched = reinterpret_cast<int *>(c->ws + l.off_diag + 128); // inside the 256-byte block of the diagnostics
-    int rc = upload_static_tables(c);
-    if (rc == SN_OK) rc = upload_phase_tables(c);
-    if (rc == SN_OK && cudaMemsetAsync(c->sched, 0, 2 * sizeof(int), c->stream) != cudaSuccess) rc = cuda_fail(cudaGetLastError());
+    c->use_graph = l.cells <= ((int64_t)1 << 24);
+    c->use_pipe = true;
+    c->pipe_all = false;
+    // the device that owns the workspace is the context's device
+    int rc = SN_OK;
+    {
+        cudaPointerAttributes pat;
+        const cudaError_t e = cudaPointerGetAttributes(&pat, d_workspace);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+        else if (pat.type != cudaMemoryTypeDevice && pat.type != cudaMemoryTypeManaged) {
+            cudaGetLastError();
+            rc = SN_ERR_WORKSPACE;
+        } else c->device = pat.device;
+    }
     if (rc == SN_OK) {
-        int dev = 0;
-        const char *ng = std::getenv("SN_NO_GRAPH"); // SN_NO_GRAPH=1: plain stream launches for every grid
-        c->use_graph = l.cells <= ((int64_t)1 << 24) && !(ng && ng[0] == '1');
-        const char *pa = std::getenv("SN_PIPE_ALL");
-        c->pipe_all = pa && pa[0] == '1';
-        const char *np = std::getenv("SN_NO_PIPE"); // SN_NO_PIPE=1: first-path kernels only (A/B runs, tests)
-        c->use_pipe = !(np && np[0] == '1');
-        if (cudaGetDevice(&dev) != cudaSuccess ||
-            cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || c->sm_count < 1)
-            rc = cuda_fail(cudaGetLastError());
-        else if (c->use_pipe)
-            rc = make_tensor_maps(c);
+        DeviceGuard guard(c->device);
+        rc = upload_static_tables(c);
+        if (rc == SN_OK) rc = upload_phase_tables(c);
+        if (rc == SN_OK && cudaMemsetAsync(c->sched, 0, 2 * sizeof(int), c->stream) != cudaSuccess) rc = cuda_fail(cudaGetLastError());
+        if (rc == SN_OK) {
+            if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sm_count < 1)
+                rc = cuda_fail(cudaGetLastError());
+            else
+                rc = make_tensor_maps(c);
+        }
     }
     if (rc != SN_OK) {
         delete c;
@@ -760,9 +852,34 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     return SN_OK;
 }
 
+int sn_set_option(sn_ctx *c, int option, int value)
+{
+    if (!c) return SN_ERR_NULL;
+    if (option == SN_OPT_GRAPH) {
+        if (value != 0 && value != 1) return SN_ERR_PARAM;
+    } else if (option == SN_OPT_DISPATCH) {
+        if (value < 0 || value > 2) return SN_ERR_PARAM;
+    } else {
+        return SN_ERR_PARAM;
+    }
+    DeviceGuard guard(c->device);
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    drop_step_graph(c);
+    if (option == SN_OPT_GRAPH) {
+        c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24);
+    } else {
+        c->use_pipe = value != 1;
+        c->pipe_all = value == 2;
+        c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0 && c->lay.nx >= 64;
+        return upload_phase_tables(c); // the external-potential flag of the nonlinear coefficients follows v_in_xkin
+    }
+    return SN_OK;
+}
+
 int sn_destroy(sn_ctx *c)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     cudaStreamSynchronize(c->stream);
     drop_step_graph(c);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -778,19 +895,21 @@ int sn_destroy(sn_ctx *c)
 int sn_set_dtau(sn_ctx *c, double dtau)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!std::isfinite(dtau)) return SN_ERR_PARAM;
-    const double old = c->dtau;
-    c->dtau = dtau;
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c); // the nonlinear-phase coefficients are kernel arguments baked into the graph
+    const double old = c->dtau;
+    c->dtau = dtau;
     const int rc = upload_phase_tables(c);
-    if (rc != SN_OK) c->dtau = old;
+    if (rc != SN_OK) c->dtau = old; // SN_ERR_CUDA: the tables are undefined (sn.h), the context must be destroyed
     return rc;
 }
 
 int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, double p_pow)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!std::isfinite(g_log) || !std::isfinite(rho_floor) || !std::isfinite(g_pow) || !std::isfinite(p_pow))
         return SN_ERR_PARAM;
     if (rho_floor <= 0.0 || p_pow == -1.0) return SN_ERR_PARAM;
@@ -803,6 +922,8 @@ int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, 
 int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
+    if (v && !c->vext) return SN_ERR_FEATURE; // SN_FEAT_VEXT not requested at create
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     if (v) {
@@ -818,6 +939,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
 int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!std::isfinite(c_bohm) || !std::isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SN_ERR_PARAM;
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
@@ -829,7 +951,9 @@ int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
 int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int src_on_device)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if ((beta == nullptr) != (gamma == nullptr)) return SN_ERR_NULL;
+    if (beta && (!c->bg || (!src_on_device && !c->phi))) return SN_ERR_FEATURE; // SN_FEAT_SOURCE (+ SN_FEAT_STAGING for host tables)
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     if (beta) {
@@ -856,6 +980,7 @@ int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int s
 int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)
 {
     if (!c || !psi) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * 8,
                             src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!src_on_device) SN_CUDA(cudaStreamSynchronize(c->stream)); // caller may reuse its host buffer
@@ -866,6 +991,7 @@ int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)
 int sn_get_state(sn_ctx *c, void *psi_out, int dst_on_device)
 {
     if (!c || !psi_out) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * 8,
                             dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
@@ -876,6 +1002,7 @@ int sn_get_state(sn_ctx *c, void *psi_out, int dst_on_device)
 int sn_step(sn_ctx *c, int64_t nsteps)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
@@ -899,6 +1026,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
 int sn_step_order4(sn_ctx *c, int64_t nsteps)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
@@ -919,6 +1047,7 @@ int sn_step_order4(sn_ctx *c, int64_t nsteps)
 int sn_debug_fft(sn_ctx *c, int direction)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     if (direction != 1 && direction != -1) return SN_ERR_PARAM;
     const Layout &l = c->lay;
@@ -942,7 +1071,9 @@ int sn_debug_fft(sn_ctx *c, int direction)
 int sn_debug_potential(sn_ctx *c, float *phi_out, int dst_on_device)
 {
     if (!c || !phi_out) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
+    if (!dst_on_device && !c->phi) return SN_ERR_FEATURE; // a host destination is staged through the SN_FEAT_STAGING scratch
     int rc = potential_spectrum(c);
     if (rc) return rc;
     PassArgs a = base_args(c);
@@ -960,6 +1091,7 @@ int sn_debug_potential(sn_ctx *c, float *phi_out, int dst_on_device)
 int sn_diagnostics(sn_ctx *c, sn_diag *out)
 {
     if (!c || !out) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     const Layout &l = c->lay;
     SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));
@@ -1007,10 +1139,11 @@ int64_t sn_launch_count(const sn_ctx *c) { return c ? c->launches : 0; }
 int sn_profile(sn_ctx *c, int enable)
 {
     if (!c) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     if (enable && !c->ev) {
         c->ev = new (std::nothrow) std::vector<cudaEvent_t>();
         c->ev_kind = new (std::nothrow) std::vector<int>();
-        if (!c->ev || !c->ev_kind) return SN_ERR_PARAM;
+        if (!c->ev || !c->ev_kind) return SN_ERR_NOMEM;
     }
     if (!enable && c->profiling) {
         const int rc = profile_flush(c);
@@ -1023,6 +1156,7 @@ int sn_profile(sn_ctx *c, int enable)
 int sn_profile_read(sn_ctx *c, double *ms_by_kind, int64_t *launches_by_kind, int reset)
 {
     if (!c || !ms_by_kind || !launches_by_kind) return SN_ERR_NULL;
+    DeviceGuard guard(c->device);
     const int rc = profile_flush(c);
     if (rc) return rc;
     for (int k = 0; k < SN_NUM_PASS_KINDS; k++) {
@@ -1047,6 +1181,8 @@ const char *sn_strerror(int code)
     case SN_ERR_WORKSPACE: return "workspace too small or not 256-byte aligned";
     case SN_ERR_STATE: return "no state set";
     case SN_ERR_CUDA: return g_cuda_msg;
+    case SN_ERR_NOMEM: return "host allocation failed";
+    case SN_ERR_FEATURE: return "the call needs a workspace region that was not requested at create (sn_options.features)";
     default: return "unknown error code";
     }
 }

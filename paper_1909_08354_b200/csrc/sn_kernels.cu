@@ -342,14 +342,11 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
     } else if (MODE == P_X_POISSON) {
         // eq. (2) in Fourier space: phi^ = D rho^/(C - k^2); C == 0: phi^(k=0) = 0
         fft_pair<N, +1, false>(a, b, j, p.tw, sm);
-        const float ka = __ldg(p.kother2 + 2 * pair), kb = __ldg(p.kother2 + 2 * pair + 1);
+        const float2 ka = __ldg(p.dko + 2 * pair), kb = __ldg(p.dko + 2 * pair + 1);
 #pragma unroll
         for (int m = 0; m < P; m++) {
-            const float kx2 = __ldg(p.ksq + j + T * m);
-            const float da = p.C - kx2 - ka, db = p.C - kx2 - kb;
-            // lap != 0: multiply by -k^2 instead (Laplacian of the density, eq. (12))
-            const float ga = p.lap ? -(kx2 + ka) * p.pscale : (da == 0.f ? 0.f : p.pscale / da);
-            const float gb = p.lap ? -(kx2 + kb) * p.pscale : (db == 0.f ? 0.f : p.pscale / db);
+            const float2 kx = __ldg(p.ksq2 + j + T * m);
+            const float ga = helmholtz_mult(ka, kx, p.pscale, p.lap), gb = helmholtz_mult(kb, kx, p.pscale, p.lap);
             a[m].x *= ga; a[m].y *= ga; b[m].x *= gb; b[m].y *= gb;
         }
         fft_pair<N, -1, false>(a, b, j, p.tw, sm);

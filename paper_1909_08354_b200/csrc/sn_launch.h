@@ -51,15 +51,15 @@ struct PassArgs {
     const float4 *tw;       // DEVICE: twiddle table for this length
     const float4 *phase;    // DEVICE: kinetic phase table (hi/lo, includes 1/N)
     const float *ksq;       // DEVICE: k_a^2 per index of this axis
-    const float *kother2;   // DEVICE: P_X_POISSON: sum of the other axes' k^2 per line
+    const float2 *ksq2;     // DEVICE: P_X_POISSON: k_x^2 per index of the contiguous axis as hi + lo
+    const float2 *dko;      // DEVICE: P_X_POISSON: per line, C - (other axes' k^2) (lap: -(other axes' k^2)) as hi + lo
     float scale;            // P_*_FFT: output scale (1/N on inverse)
-    float C;                // eq. (2) constant
     float pscale;           // P_X_POISSON: D * 0.5 / prod(N)   (0.5 from the packed r2c)
     NLParams nl;
     float *phi_out;         // DEVICE: P_H_POT
     const float *vext;      // DEVICE: external potential (same layout as psi, float) or nullptr
     const float2 *bg;       // DEVICE: P_H_SRC source tables of eq. (12), interleaved (beta, gamma) per cell, layout of psi
-    int lap;                // P_X_POISSON: multiply by -k^2 * pscale instead of pscale/(C - k^2)
+    int lap;                // P_X_POISSON: multiply by d * pscale instead of pscale/d, d = (dko - ksq2) = -k^2
     int sqrt_rho;           // P_H_R2C: transform sqrt(rho) instead of rho (Bohm term)
     float hbohm, sfloor;    // P_H_BOHM: half angle = hbohm * W / max(sqrt(rho), sfloor), hbohm = -s c_B/4; floor of sqrt(rho)
     double *diag;           // DEVICE: accumulators

@@ -756,14 +756,11 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
                 }
             } else { // P_X_POISSON
                 fft_pair<N, +1, false>(a, c, jf, p.a.tw, sm);
-                const float ka = __ldg(p.a.kother2 + line0 + 2 * g), kb = __ldg(p.a.kother2 + line0 + 2 * g + 1);
+                const float2 ka = __ldg(p.a.dko + line0 + 2 * g), kb = __ldg(p.a.dko + line0 + 2 * g + 1);
 #pragma unroll
                 for (int m = 0; m < P; m++) {
-                    const float kx2 = __ldg(p.a.ksq + jf + T * m);
-                    const float da = p.a.C - kx2 - ka, db = p.a.C - kx2 - kb;
-                    // lap != 0: multiply by -k^2 instead (Laplacian of the density, eq. (12))
-                    const float ga = p.a.lap ? -(kx2 + ka) * p.a.pscale : (da == 0.f ? 0.f : __fdividef(p.a.pscale, da));
-                    const float gb = p.a.lap ? -(kx2 + kb) * p.a.pscale : (db == 0.f ? 0.f : __fdividef(p.a.pscale, db));
+                    const float2 kx = __ldg(p.a.ksq2 + jf + T * m);
+                    const float ga = helmholtz_mult(ka, kx, p.a.pscale, p.a.lap), gb = helmholtz_mult(kb, kx, p.a.pscale, p.a.lap);
                     a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
                 }
                 fft_pair<N, -1, false>(a, c, ji, p.a.tw, sm);

@@ -18,12 +18,19 @@ LIB_PATH = os.path.join(_HERE, "libsn.so")
 
 SN_OK = 0
 ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_ERR_SINGULAR",
-             -5: "SN_ERR_WORKSPACE", -6: "SN_ERR_STATE", -7: "SN_ERR_CUDA"}
+             -5: "SN_ERR_WORKSPACE", -6: "SN_ERR_STATE", -7: "SN_ERR_CUDA", -8: "SN_ERR_NOMEM", -9: "SN_ERR_FEATURE"}
+
+# optional workspace regions (sn_options.features)
+FEAT_STAGING, FEAT_VEXT, FEAT_SOURCE, FEAT_ALL = 1, 2, 4, 7
+# sn_set_option
+OPT_GRAPH, OPT_DISPATCH = 1, 2
+DISPATCH_DEFAULT, DISPATCH_FIRST_PATH, DISPATCH_PIPELINED = 0, 1, 2
 
 # every symbol include/sn.h declares
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
-           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm")
+           "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm", "sn_workspace_bytes_opt",
+           "sn_create_opt", "sn_set_option")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG", "H_SRC", "H_BOHM")
@@ -32,6 +39,15 @@ PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG"
 class SnDiag(ctypes.Structure):
     _fields_ = [("norm", ctypes.c_double), ("e_kin", ctypes.c_double), ("e_nonlocal", ctypes.c_double),
                 ("e_local", ctypes.c_double), ("e_total", ctypes.c_double)]
+
+
+class SnOptions(ctypes.Structure):
+    _fields_ = [("struct_size", ctypes.c_size_t), ("batch", ctypes.c_int64), ("features", ctypes.c_uint32),
+                ("reserved", ctypes.c_uint32)]
+
+
+def _options(batch: int, features: int) -> SnOptions:
+    return SnOptions(ctypes.sizeof(SnOptions), int(batch), int(features), 0)
 
 
 class SnError(RuntimeError):
@@ -62,6 +78,12 @@ def lib() -> ctypes.CDLL:
         L.sn_create_batch.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, ctypes.c_int64, dp, ctypes.c_double,
                                       ctypes.c_double, ctypes.c_double, ctypes.c_double, dp, ctypes.c_int,
                                       ctypes.c_double, vp, ctypes.c_size_t, vp]
+        L.sn_workspace_bytes_opt.argtypes = [ctypes.c_int, i64p, ctypes.POINTER(SnOptions)]
+        L.sn_workspace_bytes_opt.restype = ctypes.c_size_t
+        L.sn_create_opt.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_double, ctypes.c_double,
+                                    ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, vp,
+                                    ctypes.c_size_t, vp, ctypes.POINTER(SnOptions)]
+        L.sn_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_int]
         L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_step.argtypes = [vp, ctypes.c_int64]
         L.sn_step_order4.argtypes = [vp, ctypes.c_int64]
@@ -90,67 +112,46 @@ def _chk(rc: int, what: str) -> None:
         raise SnError(rc, what, lib().sn_strerror(rc).decode())
 
 
-def workspace_bytes(dims: Sequence[int]) -> int:
+def workspace_bytes(dims: Sequence[int], batch: int = 1, features: int = 0) -> int:
     d = (ctypes.c_int64 * len(dims))(*[int(n) for n in dims])
-    return int(lib().sn_workspace_bytes(len(dims), d))
+    opt = _options(batch, features)
+    return int(lib().sn_workspace_bytes_opt(len(dims), d, ctypes.byref(opt)))
 
 
 class Simulation:
     """One sn_ctx plus the torch tensor that backs its workspace."""
 
     def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float, g: Sequence[float],
-                 dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None):
-        """batch=None: one 2D/3D system of shape dims.  batch=B: an ensemble of B systems through sn_create_batch;
-        every array then has the STORAGE shape (dims[0], B, dims[1][, dims[2]]) (member b at [:, b, ...])."""
+                 dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None, features: int = 0):
+        """batch=None: one 2D/3D system of shape dims.  batch=B: an ensemble of B systems; every array then has the
+        STORAGE shape (dims[0], B, dims[1][, dims[2]]) (member b at [:, b, ...]).  features: FEAT_* bits, the optional
+        workspace regions (external potential table, source tables, host staging); 0 = the stepper alone, ~12 B/cell."""
         import torch
 
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1909_08354_b200 needs a CUDA device (no CPU fallback)")
-        if batch is not None:
-            self._init_batch(dims, int(batch), L, A, B, C, D, g, dtau, device, stream)
-            return
-        self.dims = tuple(int(n) for n in dims)
-        nd = len(self.dims)
-        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
-        g = [float(v) for v in g]
-        self.device = torch.device(device)
-        nbytes = workspace_bytes(self.dims)
-        if nbytes == 0:
-            raise SnError(-2, "sn_workspace_bytes", lib().sn_strerror(-2).decode())
-        with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
-            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
-        self._h = ctypes.c_void_p()
-        c_dims = (ctypes.c_int64 * nd)(*self.dims)
-        c_L = (ctypes.c_double * nd)(*Ls)
-        c_g = (ctypes.c_double * max(1, len(g)))(*(g or [0.0]))
-        with torch.cuda.device(self.device):
-            _chk(lib().sn_create(ctypes.byref(self._h), nd, c_dims, c_L, A, B, C, D, c_g, len(g), dtau,
-                                 ctypes.c_void_p(self._ws.data_ptr()), nbytes,
-                                 ctypes.c_void_p(self._stream.cuda_stream)), "sn_create")
-
-    def _init_batch(self, dims, batch, L, A, B, C, D, g, dtau, device, stream):
-        import torch
         pd = tuple(int(n) for n in dims)
         nd = len(pd)
-        self.dims = (pd[0], batch) + pd[1:]               # storage shape of every array
+        self.dims = pd if batch is None else (pd[0], int(batch)) + pd[1:]   # storage shape of every array
+        self.features = int(features)
         Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
         g = [float(v) for v in g]
         self.device = torch.device(device)
+        opt = _options(1 if batch is None else int(batch), features)
         c_dims = (ctypes.c_int64 * nd)(*pd)
-        nbytes = int(lib().sn_workspace_bytes_batch(nd, c_dims, batch))
+        nbytes = int(lib().sn_workspace_bytes_opt(nd, c_dims, ctypes.byref(opt)))
         if nbytes == 0:
-            raise SnError(-2, "sn_workspace_bytes_batch", lib().sn_strerror(-2).decode())
+            raise SnError(-2, "sn_workspace_bytes_opt", lib().sn_strerror(-2).decode())
         with torch.cuda.device(self.device):
             self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._h = ctypes.c_void_p()
         c_L = (ctypes.c_double * nd)(*Ls)
         c_g = (ctypes.c_double * max(1, len(g)))(*(g or [0.0]))
-        with torch.cuda.device(self.device):
-            _chk(lib().sn_create_batch(ctypes.byref(self._h), nd, c_dims, batch, c_L, A, B, C, D, c_g, len(g), dtau,
-                                       ctypes.c_void_p(self._ws.data_ptr()), nbytes,
-                                       ctypes.c_void_p(self._stream.cuda_stream)), "sn_create_batch")
+        # the library runs every call on the device that owns the workspace, whatever device is current here
+        _chk(lib().sn_create_opt(ctypes.byref(self._h), nd, c_dims, c_L, A, B, C, D, c_g, len(g), dtau,
+                                 ctypes.c_void_p(self._ws.data_ptr()), nbytes,
+                                 ctypes.c_void_p(self._stream.cuda_stream), ctypes.byref(opt)), "sn_create_opt")
 
     @classmethod
     def from_config(cls, cfg, **kw) -> "Simulation":
@@ -245,18 +246,37 @@ class Simulation:
             b = np.ascontiguousarray(beta, dtype=np.float32)
             g = np.ascontiguousarray(gamma, dtype=np.float32)
             assert b.shape == self.dims and g.shape == self.dims
-            _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
-                 "sn_set_source_tables")
+            if self.features & FEAT_STAGING:
+                _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
+                     "sn_set_source_tables")
+            else:  # no staging region in the workspace: hand the library device copies
+                import torch
+                with torch.cuda.device(self.device), torch.cuda.stream(self._stream):
+                    db, dg = torch.from_numpy(b).to(self.device), torch.from_numpy(g).to(self.device)
+                    _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(db.data_ptr()),
+                                                    ctypes.c_void_p(dg.data_ptr()), 1), "sn_set_source_tables")
+                    self._stream.synchronize()
         else:
             assert beta.is_cuda and gamma.is_cuda and beta.is_contiguous() and gamma.is_contiguous()
             assert tuple(beta.shape) == self.dims and tuple(gamma.shape) == self.dims
             _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(beta.data_ptr()),
                                             ctypes.c_void_p(gamma.data_ptr()), 1), "sn_set_source_tables")
 
+    def _set_source_tables_host(self, beta: np.ndarray, gamma: np.ndarray) -> None:
+        """sn_set_source_tables with HOST pointers, whatever the features (used by the tests of SN_ERR_FEATURE)."""
+        b = np.ascontiguousarray(beta, dtype=np.float32)
+        g = np.ascontiguousarray(gamma, dtype=np.float32)
+        _chk(lib().sn_set_source_tables(self._h, ctypes.c_void_p(b.ctypes.data), ctypes.c_void_p(g.ctypes.data), 0),
+             "sn_set_source_tables")
+
     def diagnostics(self) -> dict:
         d = SnDiag()
         _chk(lib().sn_diagnostics(self._h, ctypes.byref(d)), "sn_diagnostics")
         return {k: getattr(d, k) for k, _ in SnDiag._fields_}
+
+    def set_option(self, option: int, value: int) -> None:
+        """OPT_GRAPH 0/1; OPT_DISPATCH DISPATCH_DEFAULT / DISPATCH_FIRST_PATH / DISPATCH_PIPELINED (A/B runs, tests)."""
+        _chk(lib().sn_set_option(self._h, int(option), int(value)), "sn_set_option")
 
     def launch_count(self) -> int:
         return int(lib().sn_launch_count(self._h))
@@ -277,6 +297,14 @@ class Simulation:
         _chk(lib().sn_debug_fft(self._h, int(direction)), "sn_debug_fft")
 
     def debug_potential(self) -> np.ndarray:
-        out = np.empty(self.dims, dtype=np.float32)
-        _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_debug_potential")
-        return out
+        """phi of eq. (2) for the current state, as a numpy float32 array (written to a device tensor by the library,
+        copied to the host by torch; with FEAT_STAGING the library copies it itself)."""
+        if self.features & FEAT_STAGING:
+            out = np.empty(self.dims, dtype=np.float32)
+            _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_debug_potential")
+            return out
+        import torch
+        with torch.cuda.device(self.device), torch.cuda.stream(self._stream):
+            dev = torch.empty(self.dims, dtype=torch.float32, device=self.device)
+            _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(dev.data_ptr()), 1), "sn_debug_potential")
+            return dev.cpu().numpy()

@@ -32,10 +32,16 @@ def test_workspace_bytes(lib):
     assert sn.workspace_bytes((64, 64)) > 64 * 64 * 8
     w = sn.workspace_bytes((512, 512, 512))
     cells = 512 ** 3
-    # psi (8 B) + half spectrum (~4 B) + phi scratch for the test hook (4 B) + external potential (4 B)
-    # + beta, gamma tables of eq. (12) (4 B each) + FFT tables
-    assert cells * 28 < w < cells * 28.2
+    # default: psi (8 B) + half spectrum (~4 B) + FFT tables -- the stepper alone
+    assert cells * 12 < w < cells * 12.1
     assert w % 256 == 0
+    # + staging scratch (4 B) + external potential (4 B) + beta, gamma tables of eq. (12) (8 B)
+    assert cells * 28 < sn.workspace_bytes((512, 512, 512), features=sn.FEAT_ALL) < cells * 28.2
+    assert sn.workspace_bytes((512, 512, 512), features=sn.FEAT_VEXT) - w == cells * 4
+    assert sn.workspace_bytes((64, 64), features=8) == 0          # unknown feature bit
+    # ensembles whose line counts overflow a 32-bit int are rejected, not wrapped
+    assert sn.workspace_bytes((4096, 4096), batch=1 << 20) == 0
+    assert sn.workspace_bytes((64, 64), batch=1 << 20) > 0
     for bad in [(64,), (64, 64, 64, 64), (48, 64), (16, 64), (8192, 64), (64, 100), (0, 64), (160, 64), (6144, 64), (288, 64)]:
         assert sn.workspace_bytes(bad) == 0
 
@@ -89,8 +95,17 @@ def test_null_context_calls(lib):
     assert lib.sn_set_bohm(None, 0.0, 1e-6) == -1
     assert lib.sn_profile(None, 1) == -1
     assert lib.sn_debug_potential(None, None, 0) == -1
+    assert lib.sn_set_option(None, 1, 0) == -1
+    assert lib.sn_create_opt(None, 2, None, None, 0.0, 0.0, 0.0, 0.0, None, 0, 0.0, None, 0, None, None) == -1
+    assert lib.sn_strerror(-9).decode().startswith("the call needs")
     assert lib.sn_strerror(-4).decode().startswith("C > 0")
     assert lib.sn_strerror(0).decode() == "ok"
+
+
+def test_library_reads_no_environment_variables():
+    """every switch is an argument (sn_options, sn_set_option), none an environment variable."""
+    for f in os.listdir(os.path.join(ROOT, "paper_1909_08354_b200", "csrc")):
+        assert "getenv" not in open(os.path.join(ROOT, "paper_1909_08354_b200", "csrc", f)).read(), f
 
 
 def test_no_cpu_fallback():
