@@ -103,7 +103,7 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, un
     L.off_psi = o; o = align256(o + (size_t)L.cells * 8);
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
     for (int d = 0; d < ndim; d++) {
-        L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 16);
+        L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 24); // float4 hi/lo table + float2 plain copy
         for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
         L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
         L.off_ksq2[d] = o; o = align256(o + (size_t)L.n[d] * 8);
@@ -485,7 +485,10 @@ int upload_static_tables(sn_ctx *c)
             ksq[k] = (float)(kk * kk);
             ksq2[k] = split_real(kk * kk);
         }
+        std::vector<f2> twp(tw.size()); // the same entries, hi part only (stages / transforms that apply them plainly)
+        for (size_t i = 0; i < tw.size(); i++) twp[i] = f2{tw[i].x, tw[i].y};
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d], tw.data(), tw.size() * 16, cudaMemcpyHostToDevice, c->stream));
+        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d] + tw.size() * 16, twp.data(), twp.size() * 8, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq.data(), (size_t)N * 4, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq2[d], ksq2.data(), (size_t)N * 8, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaStreamSynchronize(c->stream));

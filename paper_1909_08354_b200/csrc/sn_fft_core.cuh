@@ -194,19 +194,30 @@ __host__ __device__ constexpr int twiddle_entries(int N)
 #define SN_TW_PREFETCH 1 // load a stage's twiddles between the exchange's stores and loads (data registers are dead there)
 #endif
 
-template <int N, int R, int NS, bool HILO, int P>
+// Table of length N: twiddle_entries(N) float4 (hi + lo) followed by the same entries as plain float2 (hi only).
+// A stage whose twiddles are applied plainly reads the compact float2 copy: 256 B instead of 512 B per warp-wide
+// load, i.e. 2 instead of 4 L1 wavefronts -- the pass kernels are bound by L1/shared-memory wavefronts
+// (profiles/r02c).  OFF = entries of the earlier stages.
+#ifndef SN_HILO_MAX_NS
+#define SN_HILO_MAX_NS (1 << 30) // hi/lo twiddles on stages with NS <= this (psi transforms); larger NS: plain
+#endif
+template <bool HILO, int NS>
+__host__ __device__ constexpr bool stage_hilo() { return HILO && NS <= SN_HILO_MAX_NS; }
+
+template <int N, int R, int NS, int OFF, bool HILO, int P>
 __device__ __forceinline__ void load_twiddles(float4 (&w)[(P / R) * (R - 1)], int j, const float4 *__restrict__ tw)
 {
     constexpr int T = N / P, NB = P / R;
+    const float2 *__restrict__ tw2 = reinterpret_cast<const float2 *>(tw + twiddle_entries(N));
 #pragma unroll
     for (int q = 0; q < NB; q++) {
-        const float4 *src = tw + ((j + T * q) & (NS - 1));
+        const int kp = (j + T * q) & (NS - 1);
 #pragma unroll
         for (int r = 1; r < R; r++) {
             if (HILO) {
-                w[q * (R - 1) + r - 1] = __ldg(src + (r - 1) * NS);
+                w[q * (R - 1) + r - 1] = __ldg(tw + OFF + kp + (r - 1) * NS);
             } else {
-                const float2 h = __ldg(reinterpret_cast<const float2 *>(src + (r - 1) * NS));
+                const float2 h = __ldg(tw2 + OFF + kp + (r - 1) * NS);
                 w[q * (R - 1) + r - 1] = make_float4(h.x, h.y, 0.f, 0.f);
             }
         }
@@ -283,18 +294,19 @@ __device__ __forceinline__ void exchange_load(float2 (&a)[P], float2 (&b)[P], in
     for (int m = 0; m < P; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), a[m], b[m]);
 }
 
-// exchange after stage (NSP, RP), then stage NS = NSP * RP and everything after it
-template <int N, int NSP, int RP, int DIR, bool HILO, bool ONE, class SM, int P>
+// exchange after stage (NSP, RP), then stage NS = NSP * RP and everything after it (OFF: table entries before it)
+template <int N, int NSP, int RP, int OFF, int DIR, bool HILO, bool ONE, class SM, int P>
 __device__ __forceinline__ void fft_next(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
     constexpr int NS = NSP * RP, R = radix_for(N, NS);
+    constexpr bool H = stage_hilo<HILO, NS>();
     float4 w[(P / R) * (R - 1)];
     exchange_store<N, RP, NSP>(a, b, j, sm);
-    if (SN_TW_PREFETCH) load_twiddles<N, R, NS, HILO, P>(w, j, tw);
+    if (SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
     exchange_load<N>(a, b, j, sm);
-    if (!SN_TW_PREFETCH) load_twiddles<N, R, NS, HILO, P>(w, j, tw);
-    stage_compute<N, R, NS, DIR, HILO, ONE>(a, b, w);
-    if constexpr (NS * R < N) fft_next<N, NS, R, DIR, HILO, ONE, SM>(a, b, j, tw + NS * (R - 1), sm);
+    if (!SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
+    stage_compute<N, R, NS, DIR, H, ONE>(a, b, w);
+    if constexpr (NS * R < N) fft_next<N, NS, R, OFF + NS * (R - 1), DIR, HILO, ONE, SM>(a, b, j, tw, sm);
 }
 
 template <int N, int NS, int DIR, bool HILO, bool ONE, class SM, int P>
@@ -306,13 +318,13 @@ __device__ __forceinline__ void fft_stages(float2 (&a)[P], float2 (&b)[P], int j
     constexpr int R = radix_for(N, 1);
     const float4 none[(P / R) * (R - 1)] = {};
     stage_compute<N, R, 1, DIR, HILO, ONE>(a, b, none);
-    if constexpr (R < N) fft_next<N, 1, R, DIR, HILO, ONE, SM>(a, b, j, tw, sm);
+    if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, ONE, SM>(a, b, j, tw, sm);
 }
 
 // Unscaled DFT of two lines.  In: thread j holds points j + T*m of each line (T = N/P, P = ppt_for(N)).
 // Out: thread j holds outputs j + T*m.  DIR = +1: sum x e^{-2 pi i jk/N}; DIR = -1: e^{+...}.
 template <int N, int DIR, bool HILO, class SM, int P>
-__device__ __forceinline__ void fft_pair(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
+__device__ __forceinline__ void fft_pair_scalar(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
     fft_stages<N, 1, DIR, HILO, false, SM>(a, b, j, tw, sm);
 }
@@ -323,6 +335,235 @@ __device__ __forceinline__ void fft_single(float2 (&a)[P], int j, const float4 *
 {
     float2 dummy[P];
     fft_stages<N, 1, DIR, HILO, true, SM>(a, dummy, j, tw, sm);
+}
+
+// ---- packed (fp32x2) line-pair engine ------------------------------------------------------
+// The two lines of a pair see the same twiddles and the same butterfly structure, so point m of the pair is held
+// as two register pairs  r = (a.re, b.re), i = (a.im, b.im)  and every operation is one sm_100 packed instruction
+// (FADD2 / FMUL2 / FFMA2: two fp32 lanes per thread, a twiddle enters as a broadcast scalar operand) instead of two
+// scalar ones.  The fp32 pipe does the same lane-work either way; what halves is the number of ISSUED floating-point
+// instructions, and the pass kernels are issue-bound (profiles/r01g: issue slots 65 % busy, fp32 pipe ~50 %).
+// Multiplications by -i / +i are register renames plus sign flips that fold into operand modifiers.
+// Rounding is identical to the scalar engine (same operations in the same order, lane by lane).
+#ifndef SN_PACKED
+#define SN_PACKED 1
+#endif
+
+struct cp2 {
+    float2 r, i;
+};
+
+__device__ __forceinline__ float2 neg2(float2 v) { return make_float2(-v.x, -v.y); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) { return __fadd2_rn(a, neg2(b)); }
+__device__ __forceinline__ float2 mul2s(float2 a, float s) { return __fmul2_rn(a, make_float2(s, s)); }
+__device__ __forceinline__ float2 fma2s(float2 a, float s, float2 c) { return __ffma2_rn(a, make_float2(s, s), c); }
+
+__device__ __forceinline__ cp2 cadd(cp2 a, cp2 b) { return cp2{add2(a.r, b.r), add2(a.i, b.i)}; }
+__device__ __forceinline__ cp2 csub(cp2 a, cp2 b) { return cp2{sub2(a.r, b.r), sub2(a.i, b.i)}; }
+
+__device__ __forceinline__ cp2 pack_pair(float2 a, float2 b) { return cp2{make_float2(a.x, b.x), make_float2(a.y, b.y)}; }
+__device__ __forceinline__ float2 line_a(cp2 v) { return make_float2(v.r.x, v.i.x); }
+__device__ __forceinline__ float2 line_b(cp2 v) { return make_float2(v.r.y, v.i.y); }
+
+// tile slot (a.re, a.im, b.re, b.im) <-> packed pair
+__device__ __forceinline__ cp2 unpack4(float4 v) { return cp2{make_float2(v.x, v.z), make_float2(v.y, v.w)}; }
+__device__ __forceinline__ float4 pack4(cp2 v) { return make_float4(v.r.x, v.i.x, v.r.y, v.i.y); }
+// both lines times a real scalar / times one real factor per line (ga for line a, gb for line b)
+__device__ __forceinline__ cp2 cscale(cp2 v, float s) { return cp2{mul2s(v.r, s), mul2s(v.i, s)}; }
+__device__ __forceinline__ cp2 cscale(cp2 v, float ga, float gb)
+{
+    const float2 g = make_float2(ga, gb);
+    return cp2{__fmul2_rn(v.r, g), __fmul2_rn(v.i, g)};
+}
+
+// v * w for both lines (w as in twmul)
+template <int DIR, bool HILO>
+__device__ __forceinline__ cp2 twmul(cp2 v, float4 w)
+{
+    const float wi = DIR > 0 ? w.y : -w.y;
+    const float2 ni = neg2(v.i);
+    cp2 o;
+    if (HILO) {
+        const float li = DIR > 0 ? w.w : -w.w;
+        o.r = fma2s(v.r, w.x, fma2s(ni, wi, fma2s(v.r, w.z, mul2s(ni, li))));
+        o.i = fma2s(v.r, wi, fma2s(v.i, w.x, fma2s(v.r, li, mul2s(v.i, w.z))));
+    } else {
+        o.r = fma2s(v.r, w.x, mul2s(ni, wi));
+        o.i = fma2s(v.r, wi, mul2s(v.i, w.x));
+    }
+    return o;
+}
+
+template <bool HILO>
+__device__ __forceinline__ float2 scale8(float2 s)
+{
+    return HILO ? fma2s(s, C8_HI, mul2s(s, C8_LO)) : mul2s(s, C8_HI);
+}
+template <int DIR, bool HILO>
+__device__ __forceinline__ cp2 mul_w8_1(cp2 v)
+{
+    return DIR > 0 ? cp2{scale8<HILO>(add2(v.r, v.i)), scale8<HILO>(sub2(v.i, v.r))}
+                   : cp2{scale8<HILO>(sub2(v.r, v.i)), scale8<HILO>(add2(v.r, v.i))};
+}
+template <int DIR, bool HILO>
+__device__ __forceinline__ cp2 mul_w8_3(cp2 v)
+{
+    return DIR > 0 ? cp2{scale8<HILO>(sub2(v.i, v.r)), scale8<HILO>(neg2(add2(v.r, v.i)))}
+                   : cp2{scale8<HILO>(neg2(add2(v.r, v.i))), scale8<HILO>(sub2(v.r, v.i))};
+}
+template <int DIR>
+__device__ __forceinline__ cp2 mul_w4_1(cp2 v)
+{
+    return DIR > 0 ? cp2{v.i, neg2(v.r)} : cp2{neg2(v.i), v.r};
+}
+
+template <int DIR>
+__device__ __forceinline__ void bf2(cp2 &x0, cp2 &x1)
+{
+    const cp2 t = x0;
+    x0 = cadd(t, x1);
+    x1 = csub(t, x1);
+}
+template <int DIR>
+__device__ __forceinline__ void bf4(cp2 &x0, cp2 &x1, cp2 &x2, cp2 &x3)
+{
+    const cp2 c0 = cadd(x0, x2), d0 = csub(x0, x2);
+    const cp2 c1 = cadd(x1, x3), d1 = mul_w4_1<DIR>(csub(x1, x3));
+    x0 = cadd(c0, c1);
+    x2 = csub(c0, c1);
+    x1 = cadd(d0, d1);
+    x3 = csub(d0, d1);
+}
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf8(cp2 &x0, cp2 &x1, cp2 &x2, cp2 &x3, cp2 &x4, cp2 &x5, cp2 &x6, cp2 &x7)
+{
+    cp2 a0 = cadd(x0, x4), b0 = csub(x0, x4);
+    cp2 a1 = cadd(x1, x5), b1 = mul_w8_1<DIR, HILO>(csub(x1, x5));
+    cp2 a2 = cadd(x2, x6), b2 = mul_w4_1<DIR>(csub(x2, x6));
+    cp2 a3 = cadd(x3, x7), b3 = mul_w8_3<DIR, HILO>(csub(x3, x7));
+    bf4<DIR>(a0, a1, a2, a3);
+    bf4<DIR>(b0, b1, b2, b3);
+    x0 = a0; x1 = b0; x2 = a1; x3 = b1; x4 = a2; x5 = b2; x6 = a3; x7 = b3;
+}
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf3(cp2 &x0, cp2 &x1, cp2 &x2)
+{
+    const cp2 t = cadd(x1, x2), u = csub(x1, x2);
+    const cp2 m{fma2s(t.r, -0.5f, x0.r), fma2s(t.i, -0.5f, x0.i)};
+    const float2 vx = HILO ? fma2s(u.r, S3_HI, mul2s(u.r, S3_LO)) : mul2s(u.r, S3_HI);
+    const float2 vy = HILO ? fma2s(u.i, S3_HI, mul2s(u.i, S3_LO)) : mul2s(u.i, S3_HI);
+    const cp2 iv = DIR > 0 ? cp2{vy, neg2(vx)} : cp2{neg2(vy), vx};
+    x0 = cadd(x0, t);
+    x1 = cadd(m, iv);
+    x2 = csub(m, iv);
+}
+template <int DIR, bool HILO>
+__device__ __forceinline__ void bf6(cp2 &x0, cp2 &x1, cp2 &x2, cp2 &x3, cp2 &x4, cp2 &x5)
+{
+    cp2 s0 = cadd(x0, x3), d0 = csub(x0, x3);
+    cp2 s1 = cadd(x2, x5), d1 = csub(x2, x5);
+    cp2 s2 = cadd(x4, x1), d2 = csub(x4, x1);
+    bf3<DIR, HILO>(s0, s1, s2);
+    bf3<DIR, HILO>(d0, d1, d2);
+    x0 = s0; x4 = s1; x2 = s2; x3 = d0; x1 = d1; x5 = d2;
+}
+template <int R, int NB, int DIR, bool HILO, int P>
+__device__ __forceinline__ void butterfly(cp2 (&x)[P], int q)
+{
+    if constexpr (R == 8) {
+        bf8<DIR, HILO>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB], x[q + 4 * NB], x[q + 5 * NB], x[q + 6 * NB],
+                       x[q + 7 * NB]);
+    } else if constexpr (R == 6) {
+        bf6<DIR, HILO>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB], x[q + 4 * NB], x[q + 5 * NB]);
+    } else if constexpr (R == 4) {
+        bf4<DIR>(x[q], x[q + NB], x[q + 2 * NB], x[q + 3 * NB]);
+    } else {
+        bf2<DIR>(x[q], x[q + NB]);
+    }
+}
+
+template <int N, int R, int NS, int DIR, bool HILO, int P>
+__device__ __forceinline__ void stage_compute(cp2 (&x)[P], const float4 (&w)[(P / R) * (R - 1)])
+{
+    constexpr int NB = P / R;
+#pragma unroll
+    for (int q = 0; q < NB; q++) {
+        if constexpr (NS > 1) {
+#pragma unroll
+            for (int r = 1; r < R; r++) x[q + r * NB] = twmul<DIR, HILO>(x[q + r * NB], w[q * (R - 1) + r - 1]);
+        }
+        butterfly<R, NB, DIR, HILO>(x, q);
+    }
+}
+
+// the exchange stores one float4 per position: (r.x, r.y, i.x, i.y) = (a.re, b.re, a.im, b.im)
+template <int N, int R, int NS, class SM, int P>
+__device__ __forceinline__ void exchange_store(cp2 (&x)[P], int j, SM &sm)
+{
+    constexpr int T = N / P, NB = P / R;
+    constexpr int WPM = ((T - 1) & ~(NS - 1)) * R | ((T - 1) & (NS - 1));
+    sm.sync();
+    const int tbw = sm.idx((j & ~(NS - 1)) * R + (j & (NS - 1)));
+#pragma unroll
+    for (int q = 0; q < NB; q++) {
+        const int kq = ((T * q) & ~(NS - 1)) * R + ((T * q) & (NS - 1));
+#pragma unroll
+        for (int r = 0; r < R; r++) sm.st_i(comb<SM>(tbw, kq + r * NS, WPM), x[q + r * NB].r, x[q + r * NB].i);
+    }
+}
+template <int N, class SM, int P>
+__device__ __forceinline__ void exchange_load(cp2 (&x)[P], int j, SM &sm)
+{
+    constexpr int T = N / P;
+    sm.sync();
+    const int tbr = sm.idx(j);
+#pragma unroll
+    for (int m = 0; m < P; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), x[m].r, x[m].i);
+}
+
+template <int N, int NSP, int RP, int OFF, int DIR, bool HILO, class SM, int P>
+__device__ __forceinline__ void fft_next(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm)
+{
+    constexpr int NS = NSP * RP, R = radix_for(N, NS);
+    constexpr bool H = stage_hilo<HILO, NS>();
+    float4 w[(P / R) * (R - 1)];
+    exchange_store<N, RP, NSP>(x, j, sm);
+    if (SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
+    exchange_load<N>(x, j, sm);
+    if (!SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
+    stage_compute<N, R, NS, DIR, H>(x, w);
+    if constexpr (NS * R < N) fft_next<N, NS, R, OFF + NS * (R - 1), DIR, HILO, SM>(x, j, tw, sm);
+}
+
+// Unscaled DFT of a packed line pair; same contract as fft_pair.
+template <int N, int DIR, bool HILO, class SM, int P>
+__device__ __forceinline__ void fft_pair(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm)
+{
+    static_assert(P == ppt_for(N), "points per thread");
+    constexpr int R = radix_for(N, 1);
+    const float4 none[(P / R) * (R - 1)] = {};
+    stage_compute<N, R, 1, DIR, HILO>(x, none);
+    if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, SM>(x, j, tw, sm);
+}
+
+// Line pair given as two complex arrays: through the packed engine (the repacking is register naming).
+template <int N, int DIR, bool HILO, class SM, int P>
+__device__ __forceinline__ void fft_pair(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
+{
+#if SN_PACKED
+    cp2 x[P];
+#pragma unroll
+    for (int m = 0; m < P; m++) x[m] = pack_pair(a[m], b[m]);
+    fft_pair<N, DIR, HILO>(x, j, tw, sm);
+#pragma unroll
+    for (int m = 0; m < P; m++) {
+        a[m] = line_a(x[m]);
+        b[m] = line_b(x[m]);
+    }
+#else
+    fft_pair_scalar<N, DIR, HILO>(a, b, j, tw, sm);
+#endif
 }
 
 // ---- shared-memory accessors -------------------------------------------------------------

@@ -143,14 +143,10 @@ __device__ __forceinline__ void warp_arrive_done(uint64_t *bar)
 
 // kinetic phase on a line pair: a, b *= phase[j + T m]   (S2 of SURVEY.md 8(a), separable per axis)
 template <int T, int P>
-__device__ __forceinline__ void apply_phase(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ phase)
+__device__ __forceinline__ void apply_phase(cp2 (&x)[P], int j, const float4 *__restrict__ phase)
 {
 #pragma unroll
-    for (int m = 0; m < P; m++) {
-        const float4 ph = __ldg(phase + j + T * m);
-        a[m] = twmul<+1, true>(a[m], ph);
-        b[m] = twmul<+1, true>(b[m], ph);
-    }
+    for (int m = 0; m < P; m++) x[m] = twmul<+1, true>(x[m], __ldg(phase + j + T * m));
 }
 
 // ---------------------------------------------------------------------------- strided axis
@@ -209,31 +205,25 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
 
         const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
         float4 *mine = sub + nat_slot<CPW>(jf, t);     // row jf; rows jf + T m are CPW T m slots further (T % 8 == 0)
-        float2 a[P], c[P];
+        cp2 x[P]; // the column pair, packed (sn_fft_core.cuh)
 #pragma unroll
-        for (int m = 0; m < P; m++) {
-            const float4 v = mine[CPW * T * m];
-            a[m] = lo2(v);
-            c[m] = hi2(v);
-        }
+        for (int m = 0; m < P; m++) x[m] = unpack4(mine[CPW * T * m]);
         if (MODE == P_S_FFT) {
-            fft_pair<N, DIR, HILO>(a, c, jf, p.a.tw, sm);
+            fft_pair<N, DIR, HILO>(x, jf, p.a.tw, sm);
             if (DIR < 0) {
                 const float sc = p.a.scale;
 #pragma unroll
-                for (int m = 0; m < P; m++) {
-                    a[m].x *= sc; a[m].y *= sc; c[m].x *= sc; c[m].y *= sc;
-                }
+                for (int m = 0; m < P; m++) x[m] = cscale(x[m], sc);
             }
         } else { // P_S_KIN
-            fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-            apply_phase<T, P>(a, c, jf, p.a.phase);
-            fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
+            fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
+            apply_phase<T, P>(x, jf, p.a.phase);
+            fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
         }
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
         __syncwarp();
 #pragma unroll
-        for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
+        for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(x[m]);
         warp_arrive_done(done + b);
 
         if (tid == 0) {
@@ -360,8 +350,8 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
                 bulk_wait_read<0>();
                 issue_load(k + 1);
             }
-            float2 a[P], c[P];
             if (MODE == P_H_BOHM) {
+                float2 a[P], c[P];
                 // z = W = lap sqrt(rho) of the thread's two columns: psi *= exp(-i s c_B W/(2 max(sqrt(rho), floor))),
                 // eq. (15); each thread rewrites only its own slots
 #pragma unroll
@@ -372,18 +362,18 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
                     mine[CPW * T * m] = pack4(a[m], c[m]);
                 }
             } else {
+                cp2 x[P];
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float4 v = mine[CPW * T * m];
-                    a[m] = nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl);
-                    c[m] = nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl);
+                    x[m] = pack_pair(nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl), nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl));
                 }
-                fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
-                apply_phase<T, P>(a, c, jf, p.a.phase);
-                fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
+                fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
+                apply_phase<T, P>(x, jf, p.a.phase);
+                fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
                 __syncwarp();
 #pragma unroll
-                for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(a[m], c[m]);
+                for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(x[m]);
             }
         }
         warp_arrive_done(done + b);
@@ -732,44 +722,39 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
 
         if (2 * g < nl) {
             const int jf = opaque(j), ji = opaque(j); // per-tile copies: see opaque()
-            float2 a[P], c[P];
+            cp2 x[P]; // the two lines, packed (sn_fft_core.cuh)
 #pragma unroll
-            for (int m = 0; m < P; m++) {
-                a[m] = la[jf + T * m];
-                c[m] = lb[jf + T * m];
-            }
+            for (int m = 0; m < P; m++) x[m] = pack_pair(la[jf + T * m], lb[jf + T * m]);
             if (MODE == P_X_KIN) {
-                fft_pair<N, +1, true>(a, c, jf, p.a.tw, sm);
+                fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
                 if (NST == 2 && tid == 0 && k >= 1 && k + 1 < nk) { // reload the stage tile k-1 was stored from
                     bulk_wait_read<0>();
                     issue_load(k + 1);
                 }
-                apply_phase<T, P>(a, c, jf, p.a.phase);
-                fft_pair<N, -1, true>(a, c, ji, p.a.tw, sm);
+                apply_phase<T, P>(x, jf, p.a.phase);
+                fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
                 if (VEXT) {
                     const float *va = reinterpret_cast<const float *>(base + b * STAGE_BYTES + TILE_BYTES) + 2 * g * N;
 #pragma unroll
-                    for (int m = 0; m < P; m++) {
-                        a[m] = rotate_half_angle(a[m], p.a.nl.hv * va[ji + T * m]);
-                        c[m] = rotate_half_angle(c[m], p.a.nl.hv * va[N + ji + T * m]);
-                    }
+                    for (int m = 0; m < P; m++)
+                        x[m] = pack_pair(rotate_half_angle(line_a(x[m]), p.a.nl.hv * va[ji + T * m]),
+                                         rotate_half_angle(line_b(x[m]), p.a.nl.hv * va[N + ji + T * m]));
                 }
             } else { // P_X_POISSON
-                fft_pair<N, +1, false>(a, c, jf, p.a.tw, sm);
+                fft_pair<N, +1, false>(x, jf, p.a.tw, sm);
                 const float2 ka = __ldg(p.a.dko + line0 + 2 * g), kb = __ldg(p.a.dko + line0 + 2 * g + 1);
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 kx = __ldg(p.a.ksq2 + jf + T * m);
-                    const float ga = helmholtz_mult(ka, kx, p.a.pscale, p.a.lap), gb = helmholtz_mult(kb, kx, p.a.pscale, p.a.lap);
-                    a[m].x *= ga; a[m].y *= ga; c[m].x *= gb; c[m].y *= gb;
+                    x[m] = cscale(x[m], helmholtz_mult(ka, kx, p.a.pscale, p.a.lap), helmholtz_mult(kb, kx, p.a.pscale, p.a.lap));
                 }
-                fft_pair<N, -1, false>(a, c, ji, p.a.tw, sm);
+                fft_pair<N, -1, false>(x, ji, p.a.tw, sm);
             }
             sm.sync(); // exchange layout (float4 per position) != line layout: whole group must be done reading
 #pragma unroll
             for (int m = 0; m < P; m++) {
-                la[ji + T * m] = a[m];
-                lb[ji + T * m] = c[m];
+                la[ji + T * m] = line_a(x[m]);
+                lb[ji + T * m] = line_b(x[m]);
             }
         }
         warp_arrive_done(done + b);

@@ -110,29 +110,39 @@ def test_potential_matches_oracle(mods, dims, C, state):
     got, want = sim.debug_potential(), orc.potential()
     sim.close()
     orc.close()
-    assert rel(got, want) < 2e-6 and maxrel(got, want) < 2e-5, (rel(got, want), maxrel(got, want))
+    # white noise: rho has a mean as large as its fluctuations, and the fp32 rounding of that mean through the
+    # butterflies (6e-8 x sum rho) lands on the lowest modes, which 1/k^2 then weights up -- a few 1e-6 on 2^21 cells
+    # C > 0 a relative 1.4e-3 away from a grid mode (7.7 vs k^2 = 7.711): that mode is amplified 700x over its neighbours
+    tol = (2e-6 if C <= 0 else 5e-6) if state == "blobs" else 1e-5
+    assert rel(got, want) < tol and maxrel(got, want) < 10 * tol, (rel(got, want), maxrel(got, want))
 
 
-@pytest.mark.parametrize("dims", [(64, 128), (64, 64, 64), (512, 64), (96, 64)])
+@pytest.mark.parametrize("dims", [(64, 128), (64, 64, 64), (512, 64), (96, 64), (64, 512, 64), (64, 64, 512)])
 def test_potential_spectrum_bin_by_bin(mods, dims):
-    """Every Fourier bin of phi against D rho^/(C - k^2) of the oracle for white-noise psi (C = 0: the flat
-    spectrum of |psi|^2 is divided by k^2, so a rel-L2 over phi is dominated by the lowest modes; here each bin
-    counts relative to its own magnitude ... within the fp32 floor of the whole transform)."""
+    """Every Fourier bin of phi against the oracle's for white-noise psi.  A rel-L2 over phi with C = 0 is blind to the
+    high wavenumbers (1/k^2 suppresses the Nyquist row by 1/N^2), so: (i) C = -300 ~ -k_max^2, where D/(C - k^2) varies
+    by less than 5x over the spectrum and every bin -- row N/2 of the half spectrum, the mirrored rows of the packed
+    real transforms -- carries the same weight: tight bound per bin; (ii) C = 0 with the bins re-weighted by k^2: only
+    as tight as the float32 rounding of phi itself allows (a white 6e-8 max|phi| floor against a signal that falls as
+    1/k^2), still 100x below what one wrong row would give (sqrt(1/N0) ~ 0.05)."""
     snref, Oracle, inputs, sn = mods
     psi0 = inputs.white_noise(dims, seed=22)
-    sim = sn.Simulation(dims, 16.0, -0.5, 1.0, 0.0, 0.9, (), 1e-3)
-    sim.set_state(psi0)
-    orc = Oracle(dims, 16.0, -0.5, 1.0, 0.0, 0.9, (), 1e-3)
-    orc.set_state(psi0.astype(np.complex128))
-    got, want = sim.debug_potential(), orc.potential()
-    sim.close()
-    orc.close()
-    G, W = snref.fftn(got.astype(np.complex128), +1), snref.fftn(want.astype(np.complex128), +1)
-    # weight k^2: undoes the 1/k^2 of eq. (2), so every bin of the density spectrum is compared at equal weight
     k2 = sum(np.square(2 * np.pi / 16.0 * np.fft.fftfreq(n, 1.0 / n)).reshape([-1 if i == a else 1 for i in range(len(dims))])
              for a, n in enumerate(dims))
-    assert rel(G * k2, W * k2) < 2e-6
-    assert np.max(np.abs((G - W) * k2)) < 3e-5 * np.max(np.abs(W * k2))
+    for C, w, tol in ((-300.0, 1.0, 3e-6), (0.0, k2, 2e-4)):
+        sim = sn.Simulation(dims, 16.0, -0.5, 1.0, C, 0.9, (), 1e-3)
+        sim.set_state(psi0)
+        orc = Oracle(dims, 16.0, -0.5, 1.0, C, 0.9, (), 1e-3)
+        orc.set_state(psi0.astype(np.complex128))
+        got, want = sim.debug_potential(), orc.potential()
+        sim.close()
+        orc.close()
+        G, W = snref.fftn(got.astype(np.complex128), +1), snref.fftn(want.astype(np.complex128), +1)
+        if C != 0:                      # the k = 0 bin holds D rho_mean/C, ~sqrt(cells) above the rest: compare it on its own
+            assert abs(G.flat[0] - W.flat[0]) < 1e-6 * abs(W.flat[0])
+            G.flat[0] = W.flat[0] = 0.0
+        assert rel(G * w, W * w) < tol, (C, rel(G * w, W * w))
+        assert np.max(np.abs((G - W) * w)) < 10 * tol * np.max(np.abs(W * w)), C
 
 
 def test_single_mode_poisson_closed_form(mods):
