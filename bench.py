@@ -199,6 +199,9 @@ def main():
                     help="NEXT-1 row: also run with the pressure potential 0.02 ln(rho) (eq. (16)) and the "
                          "phi_C table of eq. (11) as external potential and the beta, gamma tables of eq. (12) "
                          "(DESIGN.md section 8)")
+    ap.add_argument("--dtype", default="c64", choices=["c64", "c128"],
+                    help="c64: complex64 (BASELINE.json's metric); c128: the complex128 path (SURVEY.md 8(f) item 3, the "
+                         "precision the paper benchmarked): same step, 16 B per cell of state, float64 arithmetic")
     ap.add_argument("--repeats", type=int, default=5,
                     help="timed repetitions of the K-step call (SURVEY.md 8(d): median of >= 5); value = median")
     args = ap.parse_args()
@@ -256,11 +259,15 @@ def main():
     nd = len(cfg.dims)
     K, W = args.steps, args.warmup
     psi0 = cfg.initial_state()                          # seeded synthetic state, complex64
+    f64 = args.dtype == "c128"
+    esz = 16 if f64 else 8                              # bytes per complex value
+    if f64:
+        psi0 = psi0.astype(np.complex128)               # same rounded recipe state, carried in double
     if args.batch:
         rng = np.random.default_rng(1)
         mem = [np.roll(psi0, tuple(int(rng.integers(n)) for n in cfg.dims), axis=tuple(range(nd))) *
                np.complex64(0.8 + 0.4 * b / args.batch) for b in range(args.batch)]
-        psi0 = np.ascontiguousarray(np.stack(mem, axis=1).astype(np.complex64))   # storage layout [n0][batch][...]
+        psi0 = np.ascontiguousarray(np.stack(mem, axis=1).astype(psi0.dtype))   # storage layout [n0][batch][...]
         del mem
     host_in = torch.from_numpy(psi0).pin_memory()
     host_out = torch.empty_like(host_in).pin_memory()
@@ -268,7 +275,8 @@ def main():
 
     stream = torch.cuda.current_stream()
     sim = sn.Simulation.from_config(cfg, device=dev, stream=stream, batch=args.batch or None,
-                                    features=(sn.FEAT_VEXT | sn.FEAT_SOURCE) if args.extras else 0)
+                                    features=(sn.FEAT_VEXT | sn.FEAT_SOURCE) if args.extras else 0,
+                                    dtype="complex128" if f64 else "complex64")
     if args.extras:
         # eq. (16) n = 1: V_pressure = w ln(rho), w = 0.02; eq. (11): phi_C = ln[1 - (r0/(r + r0))^lambda], lambda = 1,
         # r0 = 2, radius softened to sqrt(r^2 + 1) (the grid has a point at r = 0)
@@ -336,6 +344,9 @@ def main():
         hs_frac = (cfg.dims[0] // 2 + 1) / (cfg.dims[0] / 2)   # exact half-spectrum factor on the 4-byte terms
         def bytes_per_cell(kind):
             """algorithmic bytes per cell of the full grid for one launch of this pass kind"""
+            return bytes_per_cell_c64(kind) * (esz / 8.0)   # complex128: every array is twice as wide
+
+        def bytes_per_cell_c64(kind):
             if kind == "H_NLKIN":
                 return 16.0 + 4.0 * hs_frac
             if kind == "H_R2C":
@@ -352,14 +363,14 @@ def main():
         bpc = bytes_per_cell(dom)
         achieved = bpc * cells / (dom_ms * 1e-3) / 1e9
         out = {
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "metric": METRIC if not f64 else "split-step cell-updates/sec (complex128)", "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
+            "dtype": "complex128 (f64 arithmetic)" if f64 else "complex64 (f32 arithmetic)", "data": "synthetic",
             "config": {"workload": f"{cfg.name}{' x%d ensemble' % args.batch if args.batch else ''}{'+next1(0.02 ln rho, phi_C, beta/gamma tables of eq. (12))' if args.extras else ''}: {'x'.join(map(str, cfg.dims))} periodic, L={cfg.L}, A={cfg.A}, "
                                    f"B={cfg.B}, C={cfg.C}, D={cfg.D:.6g}, g={list(cfg.g)}, dtau={cfg.dtau}",
                        "dims": list(cfg.dims), "parallelism": "replicas only" if world > 1 else "single GPU",
-                       "l2": "state 8 B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
-                           cells, cells * 8 / 2 ** 20) if cells * 8 > 126e6 else
+                       "l2": "state %d B/cell x %d cells = %.0f MiB > 126 MB L2, no flush needed" % (
+                           esz, cells, cells * esz / 2 ** 20) if cells * esz > 126e6 else
                        "state fits L2: launch/L2-bound regime, HBM fraction is an effective figure only",
                        "timed_call": f"one {'sn_step_order4' if args.order4 else 'sn_step'}({K}) (merged half kinetics) per "
                                      f"repetition; value = median of {len(reps)} repetitions"},
@@ -370,7 +381,7 @@ def main():
             "roofline": {
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
-                "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras else None,
+                "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras and not f64 and not args.batch else None,
                 "traffic_source": "ncu --set full dram bytes per launch, profiles/r01c_ncu_full_C5_512.md (re-captured at round end, same values: r01g)",
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
@@ -379,18 +390,18 @@ def main():
                                  "achieved_GBps": bytes_per_cell(k) * cells / (v[0] / v[1] * 1e-3) / 1e9,
                                  "frac_of_measured_peak": bytes_per_cell(k) * cells / (v[0] / v[1] * 1e-3) / 1e9 / peak}
                              for k, v in sorted(prof.items())},
-                "step": {"b_min_bytes_per_cell_update": B_MIN[nd],
-                         "achieved_GBps_over_b_min": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9,
-                         "frac_of_measured_peak": B_MIN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak,
-                         "frac_of_8TBps_nominal": B_MIN[nd] * cells * K / (ms * 1e-3) / 8e12,
-                         "own_bytes_per_cell_update": B_OWN[nd],
-                         "achieved_GBps_over_own_bytes": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9,
-                         "own_frac_of_measured_peak": B_OWN[nd] * cells * K / (ms * 1e-3) / 1e9 / peak},
+                "step": {"b_min_bytes_per_cell_update": B_MIN[nd] * (esz / 8.0),
+                         "achieved_GBps_over_b_min": B_MIN[nd] * (esz / 8.0) * cells * K / (ms * 1e-3) / 1e9,
+                         "frac_of_measured_peak": B_MIN[nd] * (esz / 8.0) * cells * K / (ms * 1e-3) / 1e9 / peak,
+                         "frac_of_8TBps_nominal": B_MIN[nd] * (esz / 8.0) * cells * K / (ms * 1e-3) / 8e12,
+                         "own_bytes_per_cell_update": B_OWN[nd] * (esz / 8.0),
+                         "achieved_GBps_over_own_bytes": B_OWN[nd] * (esz / 8.0) * cells * K / (ms * 1e-3) / 1e9,
+                         "own_frac_of_measured_peak": B_OWN[nd] * (esz / 8.0) * cells * K / (ms * 1e-3) / 1e9 / peak},
             },
             "e2e": {"value": replicas.whole_job_rate(cells, K, world, e2e_ms), "unit": UNIT,
-                    "h2d_bytes_per_step": cells * 8 / K, "d2h_bytes_per_step": (cells * 8 + 40) / K,
+                    "h2d_bytes_per_step": cells * esz / K, "d2h_bytes_per_step": (cells * esz + 40) / K,
                     "call": f"sn_set_state(pinned host) + sn_step({K}) + sn_get_state(pinned host) + sn_diagnostics",
-                    "h2d_bytes_per_call": cells * 8, "d2h_bytes_per_call": cells * 8 + 40, "ms_per_call": e2e_ms},
+                    "h2d_bytes_per_call": cells * esz, "d2h_bytes_per_call": cells * esz + 40, "ms_per_call": e2e_ms},
             "checks": {"norm_after_timed_steps": norm_after, "norm_after_e2e": d["norm"]},
         }
         if world == 1 and not args.no_cpu_baseline:

@@ -72,8 +72,17 @@ typedef struct {
     size_t struct_size;  /* sizeof(sn_options), filled in by the caller (a mismatch is SN_ERR_PARAM) */
     int64_t batch;       /* ensemble members, >= 1 (see sn_create_batch) */
     uint32_t features;   /* SN_FEAT_* bits */
-    uint32_t reserved;   /* 0 */
+    uint32_t dtype;      /* SN_DTYPE_C64 (default) or SN_DTYPE_C128 */
 } sn_options;
+
+/* Precision of the state and of all arithmetic.  SN_DTYPE_C64: complex64 / float32 (BASELINE.json's metric).
+ * SN_DTYPE_C128: complex128 / float64, the precision the paper benchmarked: psi passed to
+ * sn_set_state / sn_get_state is complex128 (16 B per cell), sn_debug_potential writes float64, the workspace is
+ * about twice as large.  The complex128 path runs eq. (1),(2) with the polynomial G (Strang and order-4 steps,
+ * ensembles, diagnostics, test hooks); the NEXT-1 terms (sn_set_local_terms, _external_potential, _source_tables,
+ * _bohm) return SN_ERR_FEATURE there and features must be 0. */
+#define SN_DTYPE_C64 0u
+#define SN_DTYPE_C128 1u
 
 /* Supported axis lengths: powers of two with 32 <= N <= 4096, and 3*2^a with 96 <= N <= 3072 (96, 192, 384, 768,
  * 1536, 3072: radix-4 stages, a leading radix-2 stage where needed, and one radix-6 stage; the grid-size sweep's 384^3).  Any other length: sn_workspace_bytes

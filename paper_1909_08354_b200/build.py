@@ -69,6 +69,8 @@ def _build_locked(force: bool) -> str:
             for n in LENGTHS_FIRST + LENGTHS + LENGTHS3]
     jobs += [(os.path.join(CSRC, "sn_pipe.cu"), os.path.join(OBJ, f"sn_pipe_{n}.o"), [f"-DSN_LEN={n}"])
              for n in LENGTHS + LENGTHS3]
+    jobs += [(os.path.join(CSRC, "sn_kernels_f64.cu"), os.path.join(OBJ, f"sn_kernels_f64_{n}.o"), [f"-DSN_LEN={n}"])
+             for n in LENGTHS_FIRST + LENGTHS + LENGTHS3]     # complex128 path
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(_compile, jobs))

@@ -73,18 +73,25 @@ struct Layout {
     int64_t n[3];
     int64_t cells, cols0, nx, hs_lines, hs_elems;
     unsigned features; // SN_FEAT_*: which optional regions exist
+    unsigned dtype;    // SN_DTYPE_*
+    size_t esz;        // bytes of a complex value: 8 (complex64) or 16 (complex128)
     size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_ksq2[3], off_kother[2],
         off_diag, total;
 };
 
-bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, unsigned features = 0)
+bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, unsigned features = 0,
+                 unsigned dtype = SN_DTYPE_C64)
 {
     if (!dims || (ndim != 2 && ndim != 3)) return false;
     if (batch < 1 || batch > (1 << 20)) return false;
     if (features & ~SN_FEAT_ALL) return false;
+    if (dtype != SN_DTYPE_C64 && dtype != SN_DTYPE_C128) return false;
+    if (dtype == SN_DTYPE_C128 && features != 0) return false; // the NEXT-1 terms are complex64 only
     L.ndim = ndim;
     L.batch = batch;
     L.features = features;
+    L.dtype = dtype;
+    L.esz = dtype == SN_DTYPE_C128 ? 16 : 8;
     L.pcells = 1;
     for (int d = 0; d < ndim; d++) {
         if (!len_ok(dims[d])) return false;
@@ -100,12 +107,14 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, un
     // the kernels index columns, lines and outer blocks with 32-bit ints: reject ensembles that do not fit
     if (L.cols0 > INT_MAX || L.cells / L.nx > INT_MAX || L.hs_lines > INT_MAX || L.n[0] * batch > INT_MAX) return false;
     size_t o = 0;
-    L.off_psi = o; o = align256(o + (size_t)L.cells * 8);
-    L.off_hs = o; o = align256(o + (size_t)L.hs_elems * 8);
+    L.off_psi = o; o = align256(o + (size_t)L.cells * L.esz);
+    L.off_hs = o; o = align256(o + (size_t)L.hs_elems * L.esz);
+    // table entries have the same size in both precisions: twiddle / phase = float4 (hi + lo) or double2 (16 B),
+    // + the plain float2 twiddle copy; k^2 = float + float2 (hi + lo) or double; denominators float2 or double (8 B)
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 24); // float4 hi/lo table + float2 plain copy
         for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
-        L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 4);
+        L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 8);
         L.off_ksq2[d] = o; o = align256(o + (size_t)L.n[d] * 8);
     }
     for (int i = 0; i < 2; i++) { L.off_kother[i] = o; o = align256(o + (size_t)L.hs_lines * 8); }
@@ -135,6 +144,21 @@ inline f2 split_real(double v)
     f2 r;
     r.x = (float)v;
     r.y = (float)(v - (double)r.x);
+    return r;
+}
+
+// complex128 contexts keep the same table slots (16 and 8 bytes per entry) filled with doubles
+inline f4 as_double2(double re, double im)
+{
+    f4 r;
+    const double v[2] = {re, im};
+    std::memcpy(&r, v, 16);
+    return r;
+}
+inline f2 as_double(double v)
+{
+    f2 r;
+    std::memcpy(&r, &v, 8);
     return r;
 }
 
@@ -188,6 +212,8 @@ struct sn_ctx {
     float *phi;
     const float4 *tw[3], *ph[5][3]; // kinetic phase tables per slot (PH_*) and axis
     snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
+    bool f64;                       // SN_DTYPE_C128: every array and table below holds double2 / double instead
+    snk::NLParamsD nlvd[3];
     const float *ksq[3];
     const float2 *ksq2[3];                  // k_a^2 as hi + lo (Helmholtz denominator, evaluated without cancellation)
     const float2 *kother[2];                // per half-spectrum line: [0] C - k_other^2, [1] -k_other^2 (Laplacian), hi + lo
@@ -343,9 +369,55 @@ int run_pass(sn_ctx *c, int N, PassArgs &a)
     return SN_OK;
 }
 
+// complex128 context: the same pass descriptor, pointers reinterpreted (the scheduler only handles addresses), the
+// scalars rebuilt in double from the context
+int run_pass_f64(sn_ctx *c, int N, const PassArgs &a)
+{
+    snk::PassArgsD d;
+    std::memset(&d, 0, sizeof(d));
+    d.kind = a.kind; d.dir = a.dir;
+    d.data = reinterpret_cast<double2 *>(a.data);
+    d.hs = reinterpret_cast<double2 *>(a.hs);
+    d.row_stride = a.row_stride; d.outer_stride = a.outer_stride;
+    d.ncols = a.ncols; d.n_outer = a.n_outer; d.axis = a.axis; d.nlines = a.nlines;
+    d.tw = reinterpret_cast<const double2 *>(a.tw);
+    d.phase = reinterpret_cast<const double2 *>(a.phase);
+    d.ksq = reinterpret_cast<const double *>(a.kind == snk::P_X_POISSON ? (const void *)a.ksq2 : (const void *)a.ksq);
+    d.dko = reinterpret_cast<const double *>(a.dko);
+    d.scale = a.scale == 1.f ? 1.0 : 1.0 / (double)N; // the only scales the scheduler uses: 1 and 1/N (sn_debug_fft inverse)
+    d.lap = a.lap;
+    d.pscale = (a.lap ? 1.0 : c->D) * 0.5 / (double)c->lay.pcells;
+    d.nl = c->nlvd[a.kind == snk::P_H_NLKIN ? a.nl_slot : NL_MAIN];
+    d.phi_out = reinterpret_cast<double *>(a.phi_out);
+    d.diag = a.diag;
+    d.stream = c->stream;
+    int rc;
+    switch (N) {
+    case 96: rc = snk::launch_pass_d<96>(d); break;
+    case 384: rc = snk::launch_pass_d<384>(d); break;
+    case 1536: rc = snk::launch_pass_d<1536>(d); break;
+    case 192: rc = snk::launch_pass_d<192>(d); break;
+    case 768: rc = snk::launch_pass_d<768>(d); break;
+    case 3072: rc = snk::launch_pass_d<3072>(d); break;
+    case 32: rc = snk::launch_pass_d<32>(d); break;
+    case 64: rc = snk::launch_pass_d<64>(d); break;
+    case 128: rc = snk::launch_pass_d<128>(d); break;
+    case 256: rc = snk::launch_pass_d<256>(d); break;
+    case 512: rc = snk::launch_pass_d<512>(d); break;
+    case 1024: rc = snk::launch_pass_d<1024>(d); break;
+    case 2048: rc = snk::launch_pass_d<2048>(d); break;
+    case 4096: rc = snk::launch_pass_d<4096>(d); break;
+    default: return SN_ERR_DIMS;
+    }
+    if (rc != 0) return cuda_fail((cudaError_t)rc);
+    c->launches++;
+    return SN_OK;
+}
+
 int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
 {
     a.stream = c->stream;
+    if (c->f64) return run_pass_f64(c, N, a);
     int rc;
     if (c->use_pipe) {
         const bool strided = a.kind == snk::P_S_FFT || a.kind == snk::P_S_KIN;
@@ -428,12 +500,17 @@ int upload_phase_tables(sn_ctx *c)
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
         const int64_t n = l.n[d];
-        std::vector<f4> tab(n);
+        std::vector<f4> tab(n); // 16 bytes per entry: (re hi, im hi, re lo, im lo) floats, or (re, im) doubles
         for (int sl = 0; sl < PH_SLOTS; sl++) {
             for (int64_t k = 0; k < n; k++) {
                 const double kk = kval(k, n, c->L[d]);
                 const double th = c->A * kk * kk * c->dtau * PH_LEN[sl];
-                tab[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
+                if (c->f64) {
+                    const double v[2] = {std::cos(th) / (double)n, std::sin(th) / (double)n};
+                    std::memcpy(&tab[k], v, 16);
+                } else {
+                    tab[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
+                }
             }
             SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph[sl][d], tab.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
             SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vector is rewritten in the next iteration
@@ -451,9 +528,13 @@ int upload_phase_tables(sn_ctx *c)
         nl.hv = (float)h;
         nl.flog = (float)c->g_log;
         nl.fpow = (float)(c->g_pow / (c->p_pow + 1.0));
+        snk::NLParamsD &nd = c->nlvd[sl];
+        nd.hb = 2.0 * h * c->B; // full angle: theta = -s (B phi + G)
         for (int j = 0; j < 4; j++) {
             nl.hg[j] = j < c->n_g ? (float)(h * c->g[j]) : 0.f;
             nl.fg[j] = j < c->n_g ? (float)(c->g[j] / (double)(j + 2)) : 0.f;
+            nd.hg[j] = j < c->n_g ? 2.0 * h * c->g[j] : 0.0;
+            nd.fg[j] = j < c->n_g ? c->g[j] / (double)(j + 2) : 0.0;
         }
     }
     c->nl = c->nlv[NL_MAIN];
@@ -474,22 +555,23 @@ int upload_static_tables(sn_ctx *c)
                 for (int q = 1; q < r; q++)
                     for (int kp = 0; kp < ns; kp++) {
                         const double th = -2.0 * M_PI * (double)((q * kp) % (ns * r)) / (double)(ns * r);
-                        tw.push_back(split_hilo(std::cos(th), std::sin(th)));
+                        tw.push_back(c->f64 ? as_double2(std::cos(th), std::sin(th)) : split_hilo(std::cos(th), std::sin(th)));
                     }
             ns *= r;
         }
         std::vector<float> ksq(N);
-        std::vector<f2> ksq2(N);
+        std::vector<f2> ksq2(N); // complex128: k^2 as double, in the slot of the float table too
         for (int k = 0; k < N; k++) {
             const double kk = kval(k, N, c->L[d]);
             ksq[k] = (float)(kk * kk);
-            ksq2[k] = split_real(kk * kk);
+            ksq2[k] = c->f64 ? as_double(kk * kk) : split_real(kk * kk);
         }
         std::vector<f2> twp(tw.size()); // the same entries, hi part only (stages / transforms that apply them plainly)
         for (size_t i = 0; i < tw.size(); i++) twp[i] = f2{tw[i].x, tw[i].y};
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d], tw.data(), tw.size() * 16, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_tw[d] + tw.size() * 16, twp.data(), twp.size() * 8, cudaMemcpyHostToDevice, c->stream));
-        SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq.data(), (size_t)N * 4, cudaMemcpyHostToDevice, c->stream));
+        if (c->f64) SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq2.data(), (size_t)N * 8, cudaMemcpyHostToDevice, c->stream));
+        else SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq[d], ksq.data(), (size_t)N * 4, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ksq2[d], ksq2.data(), (size_t)N * 8, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
@@ -502,16 +584,17 @@ int upload_static_tables(sn_ctx *c)
     const int64_t h0 = l.n[0] / 2 + 1;
     for (int tab = 0; tab < 2; tab++) {
         const double c0 = tab == 0 ? c->C : 0.0;
-        std::fill(ko.begin(), ko.end(), split_real(tab == 0 && c->C != 0.0 ? c->C : -1.0)); // padding line: any finite non-zero value
+        auto enc = [&](double v) { return c->f64 ? as_double(v) : split_real(v); };
+        std::fill(ko.begin(), ko.end(), enc(tab == 0 && c->C != 0.0 ? c->C : -1.0)); // padding line: any finite non-zero value
         for (int64_t k0 = 0; k0 < h0; k0++) {
             const double a = kval(k0, l.n[0], c->L[0]);
             for (int64_t b = 0; b < l.batch; b++) {
                 if (l.ndim == 2) {
-                    ko[k0 * l.batch + b] = split_real(c0 - a * a);
+                    ko[k0 * l.batch + b] = enc(c0 - a * a);
                 } else {
                     for (int64_t k1 = 0; k1 < l.n[1]; k1++) {
                         const double q = kval(k1, l.n[1], c->L[1]);
-                        ko[(k0 * l.batch + b) * l.n[1] + k1] = split_real(c0 - (a * a + q * q));
+                        ko[(k0 * l.batch + b) * l.n[1] + k1] = enc(c0 - (a * a + q * q));
                     }
                 }
             }
@@ -519,7 +602,7 @@ int upload_static_tables(sn_ctx *c)
         SN_CUDA(cudaMemcpyAsync(c->ws + l.off_kother[tab], ko.data(), ko.size() * 8, cudaMemcpyHostToDevice, c->stream));
         SN_CUDA(cudaStreamSynchronize(c->stream));
     }
-    SN_CUDA(cudaMemsetAsync(c->ws + l.off_hs, 0, (size_t)l.hs_elems * 8, c->stream));
+    SN_CUDA(cudaMemsetAsync(c->ws + l.off_hs, 0, (size_t)l.hs_elems * l.esz, c->stream));
     SN_CUDA(cudaStreamSynchronize(c->stream));
     return SN_OK;
 }
@@ -564,6 +647,7 @@ int kinetic_sweep(sn_ctx *c, int ph_slot, bool with_nl, bool before_n, int nl_sl
         a.tw = c->tw[d];
         a.phase = c->ph[ph_slot][d];
         a.nl = c->nlv[nl_slot];
+        a.nl_slot = nl_slot;
         if (c->v_in_xkin) a.nl.flags &= ~2; // the axis-0 pass leaves V to the contiguous pass
         a.vext = nullptr;
         if (d == l.ndim - 1) {
@@ -703,7 +787,7 @@ void drop_step_graph(sn_ctx *c)
 
 extern "C" {
 
-static bool options_ok(const sn_options *opt) { return opt && opt->struct_size == sizeof(sn_options) && opt->reserved == 0; }
+static bool options_ok(const sn_options *opt) { return opt && opt->struct_size == sizeof(sn_options); }
 
 size_t sn_workspace_bytes(int ndim, const int64_t *dims)
 {
@@ -721,12 +805,12 @@ size_t sn_workspace_bytes_opt(int ndim, const int64_t *dims, const sn_options *o
 {
     Layout l;
     if (!options_ok(opt)) return 0;
-    return make_layout(ndim, dims, l, opt->batch, opt->features) ? l.total : 0;
+    return make_layout(ndim, dims, l, opt->batch, opt->features, opt->dtype) ? l.total : 0;
 }
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features);
+                       int64_t batch, unsigned features, unsigned dtype = SN_DTYPE_C64);
 
 int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
               const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
@@ -748,8 +832,10 @@ int sn_create_opt(sn_ctx **out, int ndim, const int64_t *dims, const double *L, 
     if (!opt) return SN_ERR_NULL;
     if (!options_ok(opt)) return SN_ERR_PARAM;
     if (opt->features & ~SN_FEAT_ALL) return SN_ERR_PARAM;
+    if (opt->dtype != SN_DTYPE_C64 && opt->dtype != SN_DTYPE_C128) return SN_ERR_PARAM;
+    if (opt->dtype == SN_DTYPE_C128 && opt->features != 0) return SN_ERR_PARAM;
     return create_impl(out, ndim, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, opt->batch,
-                       opt->features);
+                       opt->features, opt->dtype);
 }
 
 // reading Q5: C > 0 within 1e-12 (relative) of k^2 of a grid mode makes eq. (2) unsolvable.  Per axis: the distinct
@@ -783,11 +869,11 @@ static bool helmholtz_singular(const Layout &l, const double *L, double C)
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features)
+                       int64_t batch, unsigned features, unsigned dtype)
 {
     if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
     Layout l;
-    if (!make_layout(ndim, dims, l, batch, features)) return SN_ERR_DIMS;
+    if (!make_layout(ndim, dims, l, batch, features, dtype)) return SN_ERR_DIMS;
     if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
     if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
         return SN_ERR_PARAM;
@@ -821,8 +907,9 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     for (int i = 0; i < 2; i++) c->kother[i] = reinterpret_cast<const float2 *>(c->ws + l.off_kother[i]);
     c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
     c->sched = reinterpret_cast<int *>(c->ws + l.off_diag + 128); // inside the 256-byte block of the diagnostics
+    c->f64 = dtype == SN_DTYPE_C128;
     c->use_graph = l.cells <= ((int64_t)1 << 24);
-    c->use_pipe = true;
+    c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
     int rc = SN_OK;
@@ -843,7 +930,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
         if (rc == SN_OK) {
             if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->sm_count < 1)
                 rc = cuda_fail(cudaGetLastError());
-            else
+            else if (c->use_pipe)
                 rc = make_tensor_maps(c);
         }
     }
@@ -871,8 +958,8 @@ int sn_set_option(sn_ctx *c, int option, int value)
     if (option == SN_OPT_GRAPH) {
         c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24);
     } else {
-        c->use_pipe = value != 1;
-        c->pipe_all = value == 2;
+        c->use_pipe = value != 1 && !c->f64;
+        c->pipe_all = value == 2 && !c->f64;
         c->v_in_xkin = c->has_vext && c->use_pipe && c->lay.nx % 3 != 0 && c->lay.nx >= 64;
         return upload_phase_tables(c); // the external-potential flag of the nonlinear coefficients follows v_in_xkin
     }
@@ -916,6 +1003,7 @@ int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, 
     if (!std::isfinite(g_log) || !std::isfinite(rho_floor) || !std::isfinite(g_pow) || !std::isfinite(p_pow))
         return SN_ERR_PARAM;
     if (rho_floor <= 0.0 || p_pow == -1.0) return SN_ERR_PARAM;
+    if (c->f64 && (g_log != 0.0 || g_pow != 0.0)) return SN_ERR_FEATURE; // NEXT-1 terms: complex64 contexts only
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     c->g_log = g_log; c->rho_floor = rho_floor; c->g_pow = g_pow; c->p_pow = p_pow;
@@ -944,6 +1032,7 @@ int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
     if (!std::isfinite(c_bohm) || !std::isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SN_ERR_PARAM;
+    if (c->f64 && c_bohm != 0.0) return SN_ERR_FEATURE;
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     c->c_bohm = c_bohm;
@@ -984,7 +1073,7 @@ int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)
 {
     if (!c || !psi) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * 8,
+    SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * c->lay.esz,
                             src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!src_on_device) SN_CUDA(cudaStreamSynchronize(c->stream)); // caller may reuse its host buffer
     c->has_state = true;
@@ -996,7 +1085,7 @@ int sn_get_state(sn_ctx *c, void *psi_out, int dst_on_device)
     if (!c || !psi_out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
-    SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * 8,
+    SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * c->lay.esz,
                             dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
     if (!dst_on_device) SN_CUDA(cudaStreamSynchronize(c->stream));
     return SN_OK;

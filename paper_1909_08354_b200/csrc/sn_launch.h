@@ -63,6 +63,7 @@ struct PassArgs {
     int sqrt_rho;           // P_H_R2C: transform sqrt(rho) instead of rho (Bohm term)
     float hbohm, sfloor;    // P_H_BOHM: half angle = hbohm * W / max(sqrt(rho), sfloor), hbohm = -s c_B/4; floor of sqrt(rho)
     double *diag;           // DEVICE: accumulators
+    int nl_slot;            // which nonlinear sub-step the coefficients in `nl` belong to (scheduler bookkeeping)
     cudaStream_t stream;
 };
 
@@ -132,6 +133,34 @@ inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 
 template <int N>
 int launch_pipe(const PipeArgs &a);
+
+// ---- complex128 path (sn_kernels_f64.cu; the precision the paper benchmarked) ----
+// Same pass kinds and geometry fields as PassArgs; a double2 point is one complex128 value.
+struct NLParamsD {
+    double hb;     // -s B: theta = hb phi + rho (hg[0] + rho (hg[1] + ...)), psi *= exp(i theta)
+    double hg[4];  // -s g_j
+    double fg[4];  // g_j/(j+2)   (diagnostics: F(rho) = rho^2 (fg[0] + rho (fg[1] + ...)))
+};
+struct PassArgsD {
+    int kind, dir;
+    double2 *data;          // DEVICE: array transformed in place (psi, or the half spectrum)
+    double2 *hs;            // DEVICE: half-spectrum buffer (P_H_* kinds)
+    long long row_stride, outer_stride;
+    int ncols, n_outer, axis, nlines;
+    const double2 *tw;      // DEVICE: twiddles exp(-2 pi i r kp/(NS R)), table layout of the complex64 engine
+    const double2 *phase;   // DEVICE: kinetic phase exp(i A k^2 s)/N per index of this axis
+    const double *ksq;      // DEVICE: k_a^2 per index of this axis
+    const double *dko;      // DEVICE: P_X_POISSON: per line, C - (other axes' k^2) (lap: -(other axes' k^2))
+    double scale;           // P_*_FFT: output scale (1/N on inverse)
+    double pscale;          // P_X_POISSON: D * 0.5 / prod(N)
+    int lap;
+    NLParamsD nl;
+    double *phi_out;        // DEVICE: P_H_POT
+    double *diag;           // DEVICE: accumulators
+    cudaStream_t stream;
+};
+template <int N>
+int launch_pass_d(const PassArgsD &a);
 
 // setup helper (not part of a step): bg[i] = (beta[i], gamma[i])
 int launch_interleave(const float *beta, const float *gamma, float2 *bg, long long n, cudaStream_t stream);

@@ -43,11 +43,15 @@ class SnDiag(ctypes.Structure):
 
 class SnOptions(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_size_t), ("batch", ctypes.c_int64), ("features", ctypes.c_uint32),
-                ("reserved", ctypes.c_uint32)]
+                ("dtype", ctypes.c_uint32)]
 
 
-def _options(batch: int, features: int) -> SnOptions:
-    return SnOptions(ctypes.sizeof(SnOptions), int(batch), int(features), 0)
+DTYPE_C64, DTYPE_C128 = 0, 1
+_DTYPES = {"complex64": DTYPE_C64, "c64": DTYPE_C64, "complex128": DTYPE_C128, "c128": DTYPE_C128}
+
+
+def _options(batch: int, features: int, dtype: int = DTYPE_C64) -> SnOptions:
+    return SnOptions(ctypes.sizeof(SnOptions), int(batch), int(features), int(dtype))
 
 
 class SnError(RuntimeError):
@@ -112,9 +116,9 @@ def _chk(rc: int, what: str) -> None:
         raise SnError(rc, what, lib().sn_strerror(rc).decode())
 
 
-def workspace_bytes(dims: Sequence[int], batch: int = 1, features: int = 0) -> int:
+def workspace_bytes(dims: Sequence[int], batch: int = 1, features: int = 0, dtype: str = "complex64") -> int:
     d = (ctypes.c_int64 * len(dims))(*[int(n) for n in dims])
-    opt = _options(batch, features)
+    opt = _options(batch, features, _DTYPES[dtype])
     return int(lib().sn_workspace_bytes_opt(len(dims), d, ctypes.byref(opt)))
 
 
@@ -122,10 +126,12 @@ class Simulation:
     """One sn_ctx plus the torch tensor that backs its workspace."""
 
     def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float, g: Sequence[float],
-                 dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None, features: int = 0):
+                 dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None, features: int = 0,
+                 dtype: str = "complex64"):
         """batch=None: one 2D/3D system of shape dims.  batch=B: an ensemble of B systems; every array then has the
         STORAGE shape (dims[0], B, dims[1][, dims[2]]) (member b at [:, b, ...]).  features: FEAT_* bits, the optional
-        workspace regions (external potential table, source tables, host staging); 0 = the stepper alone, ~12 B/cell."""
+        workspace regions (external potential table, source tables, host staging); 0 = the stepper alone, ~12 B/cell.
+        dtype: "complex64" (default) or "complex128" -- the precision of the state and of all arithmetic."""
         import torch
 
         if not torch.cuda.is_available():
@@ -134,10 +140,12 @@ class Simulation:
         nd = len(pd)
         self.dims = pd if batch is None else (pd[0], int(batch)) + pd[1:]   # storage shape of every array
         self.features = int(features)
+        self.dtype = np.dtype(np.complex128 if _DTYPES[dtype] == DTYPE_C128 else np.complex64)
+        self.real_dtype = np.dtype(np.float64 if _DTYPES[dtype] == DTYPE_C128 else np.float32)
         Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
         g = [float(v) for v in g]
         self.device = torch.device(device)
-        opt = _options(1 if batch is None else int(batch), features)
+        opt = _options(1 if batch is None else int(batch), features, _DTYPES[dtype])
         c_dims = (ctypes.c_int64 * nd)(*pd)
         nbytes = int(lib().sn_workspace_bytes_opt(nd, c_dims, ctypes.byref(opt)))
         if nbytes == 0:
@@ -175,26 +183,23 @@ class Simulation:
 
     # -- state ------------------------------------------------------------------------------
     def set_state(self, psi) -> None:
-        """psi: numpy complex64 array (host) or torch complex64 CUDA tensor, shape == dims."""
+        """psi: numpy array (host) or torch CUDA / host tensor of the context's complex dtype, shape == dims."""
         if isinstance(psi, np.ndarray):
-            a = np.ascontiguousarray(psi, dtype=np.complex64)
+            a = np.ascontiguousarray(psi, dtype=self.dtype)
             assert a.shape == self.dims, (a.shape, self.dims)
             _chk(lib().sn_set_state(self._h, ctypes.c_void_p(a.ctypes.data), 0), "sn_set_state")
         else:
             import torch
-            if psi.is_cuda:
-                assert psi.dtype == torch.complex64 and psi.is_contiguous() and tuple(psi.shape) == self.dims
-                _chk(lib().sn_set_state(self._h, ctypes.c_void_p(psi.data_ptr()), 1), "sn_set_state")
-            else:  # host torch tensor (e.g. pinned)
-                assert psi.dtype == torch.complex64 and psi.is_contiguous() and tuple(psi.shape) == self.dims
-                _chk(lib().sn_set_state(self._h, ctypes.c_void_p(psi.data_ptr()), 0), "sn_set_state")
+            tdt = torch.complex128 if self.dtype == np.complex128 else torch.complex64
+            assert psi.dtype == tdt and psi.is_contiguous() and tuple(psi.shape) == self.dims
+            _chk(lib().sn_set_state(self._h, ctypes.c_void_p(psi.data_ptr()), 1 if psi.is_cuda else 0), "sn_set_state")
 
     def get_state(self, out=None):
-        """Return the state as a numpy complex64 array, or fill `out` (numpy / torch host or CUDA tensor)."""
+        """Return the state as a numpy array of the context's dtype, or fill `out` (numpy / torch host or CUDA tensor)."""
         if out is None:
-            out = np.empty(self.dims, dtype=np.complex64)
+            out = np.empty(self.dims, dtype=self.dtype)
         if isinstance(out, np.ndarray):
-            assert out.dtype == np.complex64 and out.flags.c_contiguous and out.shape == self.dims
+            assert out.dtype == self.dtype and out.flags.c_contiguous and out.shape == self.dims
             _chk(lib().sn_get_state(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_get_state")
         else:
             _chk(lib().sn_get_state(self._h, ctypes.c_void_p(out.data_ptr()), 1 if out.is_cuda else 0),
@@ -300,11 +305,12 @@ class Simulation:
         """phi of eq. (2) for the current state, as a numpy float32 array (written to a device tensor by the library,
         copied to the host by torch; with FEAT_STAGING the library copies it itself)."""
         if self.features & FEAT_STAGING:
-            out = np.empty(self.dims, dtype=np.float32)
+            out = np.empty(self.dims, dtype=self.real_dtype)
             _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(out.ctypes.data), 0), "sn_debug_potential")
             return out
         import torch
         with torch.cuda.device(self.device), torch.cuda.stream(self._stream):
-            dev = torch.empty(self.dims, dtype=torch.float32, device=self.device)
+            dev = torch.empty(self.dims, dtype=torch.float64 if self.real_dtype == np.float64 else torch.float32,
+                              device=self.device)
             _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(dev.data_ptr()), 1), "sn_debug_potential")
             return dev.cpu().numpy()
