@@ -585,3 +585,195 @@ void snref_set_num_threads(int n)
     (void)n;
 #endif
 }
+
+/* ================================================================== NEXT-4b: coupled wave functions
+ *
+ * PAPER.md:46 (section II): "Equations (1) and (2) can be further generalized if one considers multiple wave
+ * functions coupled through the different nonlinearities of the system".  The paper does not write the generalized
+ * system down; reading Q18 of DESIGN.md -- M components psi_c, each with its own kinetic and nonlocal constants, coupled
+ * through (i) the local (Kerr-type) nonlinearity, a matrix g_cc' acting on the component densities, and (ii) the
+ * nonlocal field, sourced by the weighted total density:
+ *      i dpsi_c/dtau = A_c lap psi_c + B_c phi psi_c + (sum_c' g_cc' |psi_c'|^2) psi_c          (1')
+ *      lap phi + C phi = D sum_c w_c |psi_c|^2                                                   (2')
+ * Strang step, same readings as the one-component path (Q1-Q4):
+ *      K(s):  psi_c^ *= exp(+i A_c k^2 s) for every c
+ *      N(s):  rho_c = |psi_c|^2;  phi from (2') (phi^(0) = 0 when C == 0);
+ *             psi_c *= exp(-i s (B_c phi + sum_c' g_cc' rho_c'))   -- exact for the N sub-flow: every rho_c is invariant
+ *      step:  K(dtau/2) N(dtau) K(dtau/2)
+ * State layout: [M][cells], component-major.  Reuses fftn / kval of this file; everything else is written out here.
+ * Pins (tests/test_oracle_pins_mc.py): two plane waves (exact for any dtau), decoupled limit against snref_step,
+ * equal split of a one-component state, per-component norm conservation, order 2 under dtau halving. */
+
+#define SNREF_MC_MAX 4
+
+typedef struct snref_mc_ctx {
+    int ndim, M;
+    int64_t n[3];
+    double L[3];
+    double A[SNREF_MC_MAX], B[SNREF_MC_MAX], w[SNREF_MC_MAX], g[SNREF_MC_MAX][SNREF_MC_MAX];
+    double C, D, dtau;
+    int64_t cells;
+    cplx *psi;  /* [M][cells] */
+    cplx *work; /* cells */
+    int has_state;
+} snref_mc_ctx;
+
+static double mc_ksq_at(const snref_mc_ctx *c, int64_t idx)
+{
+    double k2 = 0.0;
+    for (int d = c->ndim - 1; d >= 0; d--) {
+        int64_t j = idx % c->n[d];
+        idx /= c->n[d];
+        double k = kval(j, c->n[d], c->L[d]);
+        k2 += k * k;
+    }
+    return k2;
+}
+
+int snref_mc_create(snref_mc_ctx **out, int ndim, const int64_t *dims, const double *L, int M, const double *A,
+                    const double *B, double C, double D, const double *w, const double *g /* [M][M] row-major */,
+                    double dtau)
+{
+    if (!out || !dims || !L || !A || !B || !w || !g) return SNREF_ERR_NULL;
+    if (ndim != 2 && ndim != 3) return SNREF_ERR_DIMS;
+    if (M < 1 || M > SNREF_MC_MAX) return SNREF_ERR_PARAM;
+    snref_mc_ctx *c = (snref_mc_ctx *)calloc(1, sizeof(*c));
+    if (!c) return SNREF_ERR_NOMEM;
+    c->ndim = ndim;
+    c->M = M;
+    c->cells = 1;
+    for (int d = 0; d < ndim; d++) {
+        if (!fft_len_ok(dims[d]) || !(L[d] > 0.0)) { free(c); return SNREF_ERR_DIMS; }
+        c->n[d] = dims[d];
+        c->L[d] = L[d];
+        c->cells *= dims[d];
+    }
+    for (int a = 0; a < M; a++) {
+        c->A[a] = A[a]; c->B[a] = B[a]; c->w[a] = w[a];
+        for (int b = 0; b < M; b++) c->g[a][b] = g[a * M + b];
+    }
+    c->C = C; c->D = D; c->dtau = dtau;
+    c->psi = (cplx *)malloc(sizeof(cplx) * (size_t)c->cells * (size_t)M);
+    c->work = (cplx *)malloc(sizeof(cplx) * (size_t)c->cells);
+    if (!c->psi || !c->work) { free(c->psi); free(c->work); free(c); return SNREF_ERR_NOMEM; }
+    *out = c;
+    return SNREF_OK;
+}
+
+int snref_mc_destroy(snref_mc_ctx *c)
+{
+    if (!c) return SNREF_ERR_NULL;
+    free(c->psi);
+    free(c->work);
+    free(c);
+    return SNREF_OK;
+}
+
+int snref_mc_set_dtau(snref_mc_ctx *c, double dtau)
+{
+    if (!c) return SNREF_ERR_NULL;
+    c->dtau = dtau;
+    return SNREF_OK;
+}
+
+int snref_mc_set_state(snref_mc_ctx *c, const cplx *psi)
+{
+    if (!c || !psi) return SNREF_ERR_NULL;
+    memcpy(c->psi, psi, sizeof(cplx) * (size_t)c->cells * (size_t)c->M);
+    c->has_state = 1;
+    return SNREF_OK;
+}
+
+int snref_mc_get_state(snref_mc_ctx *c, cplx *out)
+{
+    if (!c || !out) return SNREF_ERR_NULL;
+    if (!c->has_state) return SNREF_ERR_STATE;
+    memcpy(out, c->psi, sizeof(cplx) * (size_t)c->cells * (size_t)c->M);
+    return SNREF_OK;
+}
+
+/* K(s) of (1'): component by component */
+static int mc_kinetic(snref_mc_ctx *c, double s)
+{
+    for (int a = 0; a < c->M; a++) {
+        cplx *p = c->psi + (size_t)a * (size_t)c->cells;
+        int rc = fftn(p, c->ndim, c->n, +1);
+        if (rc) return rc;
+#pragma omp parallel for schedule(static)
+        for (int64_t i = 0; i < c->cells; i++) {
+            double th = c->A[a] * mc_ksq_at(c, i) * s;
+            p[i] *= cos(th) + I * sin(th);
+        }
+        if ((rc = fftn(p, c->ndim, c->n, -1))) return rc;
+    }
+    return SNREF_OK;
+}
+
+/* N(s) of (1'),(2') */
+static int mc_nonlinear(snref_mc_ctx *c, double s)
+{
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) {
+        double src = 0.0;
+        for (int a = 0; a < c->M; a++) {
+            cplx v = c->psi[(size_t)a * (size_t)c->cells + (size_t)i];
+            src += c->w[a] * (creal(v) * creal(v) + cimag(v) * cimag(v));
+        }
+        c->work[i] = src;
+    }
+    int rc = fftn(c->work, c->ndim, c->n, +1);
+    if (rc) return rc;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) {
+        if (c->C == 0.0 && i == 0) { c->work[i] = 0.0; continue; }
+        c->work[i] = c->D * c->work[i] / (c->C - mc_ksq_at(c, i));
+    }
+    if ((rc = fftn(c->work, c->ndim, c->n, -1))) return rc;
+#pragma omp parallel for schedule(static)
+    for (int64_t i = 0; i < c->cells; i++) {
+        double rho[SNREF_MC_MAX];
+        for (int a = 0; a < c->M; a++) {
+            cplx v = c->psi[(size_t)a * (size_t)c->cells + (size_t)i];
+            rho[a] = creal(v) * creal(v) + cimag(v) * cimag(v);
+        }
+        double phi = creal(c->work[i]);
+        for (int a = 0; a < c->M; a++) {
+            double loc = 0.0;
+            for (int b = 0; b < c->M; b++) loc += c->g[a][b] * rho[b];
+            double th = -s * (c->B[a] * phi + loc);
+            c->psi[(size_t)a * (size_t)c->cells + (size_t)i] *= cos(th) + I * sin(th);
+        }
+    }
+    return SNREF_OK;
+}
+
+int snref_mc_step(snref_mc_ctx *c, int64_t nsteps)
+{
+    if (!c) return SNREF_ERR_NULL;
+    if (!c->has_state) return SNREF_ERR_STATE;
+    if (nsteps < 0) return SNREF_ERR_PARAM;
+    for (int64_t s = 0; s < nsteps; s++) {
+        int rc;
+        if ((rc = mc_kinetic(c, 0.5 * c->dtau))) return rc;
+        if ((rc = mc_nonlinear(c, c->dtau))) return rc;
+        if ((rc = mc_kinetic(c, 0.5 * c->dtau))) return rc;
+    }
+    return SNREF_OK;
+}
+
+/* norms[a] = sum |psi_a|^2 dV */
+int snref_mc_norms(snref_mc_ctx *c, double *norms)
+{
+    if (!c || !norms) return SNREF_ERR_NULL;
+    if (!c->has_state) return SNREF_ERR_STATE;
+    double dV = 1.0;
+    for (int d = 0; d < c->ndim; d++) dV *= c->L[d] / (double)c->n[d];
+    for (int a = 0; a < c->M; a++) {
+        const cplx *p = c->psi + (size_t)a * (size_t)c->cells;
+        double s = 0.0;
+#pragma omp parallel for schedule(static) reduction(+ : s)
+        for (int64_t i = 0; i < c->cells; i++) s += creal(p[i]) * creal(p[i]) + cimag(p[i]) * cimag(p[i]);
+        norms[a] = s * dV;
+    }
+    return SNREF_OK;
+}

@@ -54,6 +54,14 @@ def lib() -> ctypes.CDLL:
         L.snref_set_source_tables.argtypes = [vp, vp, vp]
         L.snref_set_bohm.argtypes = [vp, ctypes.c_double, ctypes.c_double]
         L.snref_bohm_potential.argtypes = [vp, vp]
+        L.snref_mc_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_int, dp, dp, ctypes.c_double,
+                                      ctypes.c_double, dp, dp, ctypes.c_double]
+        L.snref_mc_destroy.argtypes = [vp]
+        L.snref_mc_set_dtau.argtypes = [vp, ctypes.c_double]
+        L.snref_mc_set_state.argtypes = [vp, vp]
+        L.snref_mc_get_state.argtypes = [vp, vp]
+        L.snref_mc_step.argtypes = [vp, ctypes.c_int64]
+        L.snref_mc_norms.argtypes = [vp, dp]
         L.snref_num_threads.restype = ctypes.c_int
         L.snref_set_num_threads.argtypes = [ctypes.c_int]
         _lib = L
@@ -185,3 +193,52 @@ class Oracle:
         d = SnrefDiag()
         _chk(lib().snref_diagnostics(self._h, ctypes.byref(d)), "snref_diagnostics")
         return {k: getattr(d, k) for k, _ in SnrefDiag._fields_}
+
+
+class OracleMC:
+    """Coupled wave functions (NEXT-4b, reading Q18): state shape (M,) + dims, complex128."""
+
+    def __init__(self, dims: Sequence[int], L, A: Sequence[float], B: Sequence[float], C: float, D: float,
+                 w: Sequence[float], g, dtau: float):
+        self.dims = tuple(int(n) for n in dims)
+        nd = len(self.dims)
+        self.M = len(A)
+        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
+        gm = np.ascontiguousarray(g, dtype=np.float64)
+        assert gm.shape == (self.M, self.M) and len(B) == self.M and len(w) == self.M
+        self._h = ctypes.c_void_p()
+        arr = lambda v: (ctypes.c_double * len(v))(*[float(x) for x in v])
+        _chk(lib().snref_mc_create(ctypes.byref(self._h), nd, (ctypes.c_int64 * nd)(*self.dims), arr(Ls), self.M,
+                                   arr(A), arr(B), C, D, arr(w), arr(gm.ravel()), dtau), "snref_mc_create")
+
+    def close(self) -> None:
+        if self._h:
+            lib().snref_mc_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_state(self, psi: np.ndarray) -> None:
+        a = np.ascontiguousarray(psi, dtype=np.complex128)
+        assert a.shape == (self.M,) + self.dims, a.shape
+        _chk(lib().snref_mc_set_state(self._h, a.ctypes.data), "snref_mc_set_state")
+
+    def get_state(self) -> np.ndarray:
+        out = np.empty((self.M,) + self.dims, dtype=np.complex128)
+        _chk(lib().snref_mc_get_state(self._h, out.ctypes.data), "snref_mc_get_state")
+        return out
+
+    def step(self, n: int) -> None:
+        _chk(lib().snref_mc_step(self._h, int(n)), "snref_mc_step")
+
+    def set_dtau(self, dtau: float) -> None:
+        _chk(lib().snref_mc_set_dtau(self._h, float(dtau)), "snref_mc_set_dtau")
+
+    def norms(self) -> np.ndarray:
+        out = (ctypes.c_double * self.M)()
+        _chk(lib().snref_mc_norms(self._h, out), "snref_mc_norms")
+        return np.array(out[:])
