@@ -166,6 +166,23 @@ int sn_set_local_terms(sn_ctx *ctx, double g_log, double rho_floor, double g_pow
 int sn_set_source_tables(sn_ctx *ctx, const float *beta, const float *gamma, int src_on_device);
 int sn_set_external_potential(sn_ctx *ctx, const float *v, int src_on_device);
 
+/* ---- NEXT-4b: coupled wave functions ("Equations (1) and (2) can be further generalized if one considers
+ * multiple wave functions coupled through the different nonlinearities of the system"; the paper does not write the
+ * system down -- reading Q18 of DESIGN.md) ----
+ *      i dpsi_c/dtau = A_c lap psi_c + B_c phi psi_c + (sum_c' g_cc' |psi_c'|^2) psi_c,   c = 0..n_comp-1
+ *      lap phi + C phi = D sum_c w_c |psi_c|^2
+ * advanced by the same Strang step: K(s) acts on every component with its own A_c; N(s) is exact for its sub-flow
+ * (every |psi_c|^2 is invariant under it).  1 <= n_comp <= 4; A, B, w: n_comp values; g: n_comp x n_comp, row-major
+ * (g[c * n_comp + c'] multiplies |psi_c'|^2 in the equation of component c); all host pointers.  complex64.
+ * State layout for sn_set_state / sn_get_state: [n_comp][dims...] (component-major).  Calls that work on such a
+ * context: sn_set_state, sn_step, sn_get_state, sn_set_dtau, sn_mc_norms, sn_set_option, sn_profile*, sn_destroy;
+ * the others return SN_ERR_FEATURE.  sn_mc_norms: norms[c] = sum |psi_c|^2 dV (each conserved); host, n_comp doubles. */
+size_t sn_workspace_bytes_mc(int ndim, const int64_t *dims /* host */, int n_comp);
+int sn_create_mc(sn_ctx **out, int ndim, const int64_t *dims, const double *L, int n_comp, const double *A,
+                 const double *B, double C, double D, const double *w, const double *g, double dtau,
+                 void *d_workspace, size_t workspace_bytes, void *cuda_stream);
+int sn_mc_norms(sn_ctx *ctx, double *norms);
+
 int sn_destroy(sn_ctx *ctx);
 
 /* Text for an error code; for SN_ERR_CUDA the last CUDA error string seen by this thread. */
@@ -184,10 +201,11 @@ int64_t sn_launch_count(const sn_ctx *ctx);
  *   6 H_DIAG axis-0 c2r + energy sums              7 X_FFT  contiguous-axis plain transform
  *   8 X_KIN  contiguous-axis forward-phase-inverse 9 X_POISSON contiguous-axis forward-D/(C-k^2)-inverse
  *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12))
- *  12 H_BOHM axis-0 Bohm phase (eq. (15)) */
-#define SN_NUM_PASS_KINDS 13
+ *  12 H_BOHM axis-0 Bohm phase (eq. (15))       13 H_R2C_MC weighted density of coupled components + packed r2c
+ *  14 H_NL_MC axis-0 c2r + nonlinear phases of coupled components */
+#define SN_NUM_PASS_KINDS 15
 int sn_profile(sn_ctx *ctx, int enable);
-int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 13 */, int64_t *launches_by_kind /* host, 13 */,
+int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 15 */, int64_t *launches_by_kind /* host, 15 */,
                     int reset);
 
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */

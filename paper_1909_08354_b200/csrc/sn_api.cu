@@ -75,13 +75,16 @@ struct Layout {
     unsigned features; // SN_FEAT_*: which optional regions exist
     unsigned dtype;    // SN_DTYPE_*
     size_t esz;        // bytes of a complex value: 8 (complex64) or 16 (complex128)
+    int ncomp;         // coupled wave functions (sn_create_mc): psi holds ncomp arrays one after the other; else 1
     size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_ksq2[3], off_kother[2],
         off_diag, total;
 };
 
 bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, unsigned features = 0,
-                 unsigned dtype = SN_DTYPE_C64)
+                 unsigned dtype = SN_DTYPE_C64, int ncomp = 1)
 {
+    if (ncomp < 1 || ncomp > 4) return false;
+    L.ncomp = ncomp;
     if (!dims || (ndim != 2 && ndim != 3)) return false;
     if (batch < 1 || batch > (1 << 20)) return false;
     if (features & ~SN_FEAT_ALL) return false;
@@ -107,13 +110,13 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, un
     // the kernels index columns, lines and outer blocks with 32-bit ints: reject ensembles that do not fit
     if (L.cols0 > INT_MAX || L.cells / L.nx > INT_MAX || L.hs_lines > INT_MAX || L.n[0] * batch > INT_MAX) return false;
     size_t o = 0;
-    L.off_psi = o; o = align256(o + (size_t)L.cells * L.esz);
+    L.off_psi = o; o = align256(o + (size_t)L.cells * L.esz * (size_t)ncomp);
     L.off_hs = o; o = align256(o + (size_t)L.hs_elems * L.esz);
     // table entries have the same size in both precisions: twiddle / phase = float4 (hi + lo) or double2 (16 B),
     // + the plain float2 twiddle copy; k^2 = float + float2 (hi + lo) or double; denominators float2 or double (8 B)
     for (int d = 0; d < ndim; d++) {
         L.off_tw[d] = o; o = align256(o + (size_t)twiddle_entries((int)L.n[d]) * 24); // float4 hi/lo table + float2 plain copy
-        for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16); }
+        for (int sl = 0; sl < 5; sl++) { L.off_ph[sl][d] = o; o = align256(o + (size_t)L.n[d] * 16 * (size_t)ncomp); } // one table per component
         L.off_ksq[d] = o; o = align256(o + (size_t)L.n[d] * 8);
         L.off_ksq2[d] = o; o = align256(o + (size_t)L.n[d] * 8);
     }
@@ -212,6 +215,12 @@ struct sn_ctx {
     float *phi;
     const float4 *tw[3], *ph[5][3]; // kinetic phase tables per slot (PH_*) and axis
     snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
+    // coupled wave functions (NEXT-4b; reading Q18): per-component constants; component c's state is
+    // psi + c * cells, its kinetic phase tables ph[slot][axis] + c * n[axis]
+    int ncomp;
+    bool is_mc; // created by sn_create_mc (also with ncomp == 1): sn_step runs the coupled scheduler
+    double Ac[4], Bc[4], wc[4], gc[4][4];
+    CUtensorMap m_psi_mc[4][2];
     bool f64;                       // SN_DTYPE_C128: every array and table below holds double2 / double instead
     snk::NLParamsD nlvd[3];
     const float *ksq[3];
@@ -338,6 +347,12 @@ int make_tensor_maps(sn_ctx *c)
         if ((rc = make_map(&c->m_bg, c->bg, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         c->m_ok[0] = true;
     }
+    for (int k = 1; k < l.ncomp; k++) { // coupled components: their own views of psi_k (same geometry)
+        float2 *pk = c->psi + (size_t)k * l.cells;
+        if (c->m_ok[0] && (rc = make_map(&c->m_psi_mc[k][0], pk, 1, (int)l.n[0], l.cols0, snk::pipe_box_rows((int)l.n[0]), snk::pipe_cpw((int)l.n[0])))) return rc;
+        if (l.ndim == 3 && l.n[1] >= 64 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0 &&
+            (rc = make_map(&c->m_psi_mc[k][1], pk, l.n[0] * l.batch, (int)l.n[1], l.n[2], snk::pipe_box_rows((int)l.n[1]), snk::pipe_cpw((int)l.n[1])))) return rc;
+    }
     if (l.ndim == 3 && l.n[1] >= 64 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
         const int n1 = (int)l.n[1], cpw = snk::pipe_cpw(n1);
         if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0] * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
@@ -436,7 +451,8 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
             pa.a = a;
             pa.sched = c->sched;
             if (strided) {
-                pa.m_data = axis == 1 ? (a.data == c->hs ? c->m_hs1 : c->m_psi[1]) : c->m_psi[0];
+                const int comp = (a.data == c->hs || c->ncomp <= 1) ? 0 : (int)((a.data - c->psi) / c->lay.cells);
+                pa.m_data = a.data == c->hs ? c->m_hs1 : (comp ? c->m_psi_mc[comp][axis] : c->m_psi[axis]);
                 pa.tiles_per_outer = a.ncols / (2 * snk::pipe_groups(N));
                 pa.n_tiles = pa.tiles_per_outer * a.n_outer;
             } else if (haxis) {
@@ -500,19 +516,21 @@ int upload_phase_tables(sn_ctx *c)
     const Layout &l = c->lay;
     for (int d = 0; d < l.ndim; d++) {
         const int64_t n = l.n[d];
-        std::vector<f4> tab(n); // 16 bytes per entry: (re hi, im hi, re lo, im lo) floats, or (re, im) doubles
+        std::vector<f4> tab(n * l.ncomp); // 16 bytes per entry: (re hi, im hi, re lo, im lo) floats, or (re, im) doubles
         for (int sl = 0; sl < PH_SLOTS; sl++) {
-            for (int64_t k = 0; k < n; k++) {
+            for (int64_t kc = 0; kc < n * l.ncomp; kc++) {
+                const int64_t k = kc % n;
+                const double Acomp = c->is_mc ? c->Ac[kc / n] : c->A;
                 const double kk = kval(k, n, c->L[d]);
-                const double th = c->A * kk * kk * c->dtau * PH_LEN[sl];
+                const double th = Acomp * kk * kk * c->dtau * PH_LEN[sl];
                 if (c->f64) {
                     const double v[2] = {std::cos(th) / (double)n, std::sin(th) / (double)n};
-                    std::memcpy(&tab[k], v, 16);
+                    std::memcpy(&tab[kc], v, 16);
                 } else {
-                    tab[k] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
+                    tab[kc] = split_hilo(std::cos(th) / (double)n, std::sin(th) / (double)n);
                 }
             }
-            SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph[sl][d], tab.data(), n * 16, cudaMemcpyHostToDevice, c->stream));
+            SN_CUDA(cudaMemcpyAsync(c->ws + l.off_ph[sl][d], tab.data(), tab.size() * 16, cudaMemcpyHostToDevice, c->stream));
             SN_CUDA(cudaStreamSynchronize(c->stream)); // the host vector is rewritten in the next iteration
         }
     }
@@ -746,6 +764,60 @@ int prepare_n(sn_ctx *c, int nl_slot)
     return potential_spectrum(c);
 }
 
+// ---- coupled wave functions (NEXT-4b, reading Q18 of DESIGN.md) ----
+// K(s): every component on its own, one forward -> phase -> inverse pass per axis with the component's phase tables
+int kinetic_sweep_mc(sn_ctx *c, int ph_slot)
+{
+    const Layout &l = c->lay;
+    int rc;
+    for (int k = 0; k < l.ncomp; k++)
+        for (int d = 0; d < l.ndim; d++) {
+            PassArgs a = base_args(c);
+            a.data = c->psi + (size_t)k * l.cells;
+            a.tw = c->tw[d];
+            a.phase = c->ph[ph_slot][d] + (size_t)k * l.n[d];
+            a.vext = nullptr;
+            if (d == l.ndim - 1) {
+                a.kind = snk::P_X_KIN;
+                a.nlines = (int)(l.cells / l.nx);
+            } else {
+                a.kind = snk::P_S_KIN;
+                set_axis_geometry(c, a, d, l.n[0]);
+            }
+            if ((rc = run_pass(c, (int)l.n[d], a))) return rc;
+        }
+    return SN_OK;
+}
+
+snk::MCParams mc_params(const sn_ctx *c, double s)
+{
+    snk::MCParams m;
+    std::memset(&m, 0, sizeof(m));
+    m.ncomp = c->lay.ncomp;
+    m.comp_stride = c->lay.cells;
+    for (int a = 0; a < m.ncomp; a++) {
+        m.w[a] = (float)c->wc[a];
+        m.hb[a] = (float)(-0.5 * s * c->Bc[a]);
+        for (int b = 0; b < m.ncomp; b++) m.hg[a][b] = (float)(-0.5 * s * c->gc[a][b]);
+    }
+    return m;
+}
+
+// N(s): rho = sum_c w_c |psi_c|^2 -> phi^ (same half-spectrum chain as one component) -> every component's phase
+int nonlinear_mc(sn_ctx *c, double s)
+{
+    const Layout &l = c->lay;
+    int rc;
+    PassArgs a = base_args(c);
+    a.kind = snk::P_H_R2C_MC; a.data = c->psi; a.hs = c->hs; a.tw = c->tw[0];
+    a.mc = mc_params(c, s);
+    set_axis_geometry(c, a, 0, l.n[0]);
+    if ((rc = run_pass(c, (int)l.n[0], a))) return rc;
+    if ((rc = spectrum_chain(c, /*lap=*/false))) return rc;
+    a.kind = snk::P_H_NL_MC;
+    return run_pass(c, (int)l.n[0], a);
+}
+
 // capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
 int build_step_graph(sn_ctx *c)
 {
@@ -787,6 +859,11 @@ void drop_step_graph(sn_ctx *c)
 
 extern "C" {
 
+struct MCInit { // constants of the coupled-component system handed from sn_create_mc to create_impl
+    int n;
+    const double *A, *B, *w, *g;
+};
+
 static bool options_ok(const sn_options *opt) { return opt && opt->struct_size == sizeof(sn_options); }
 
 size_t sn_workspace_bytes(int ndim, const int64_t *dims)
@@ -810,7 +887,7 @@ size_t sn_workspace_bytes_opt(int ndim, const int64_t *dims, const sn_options *o
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features, unsigned dtype = SN_DTYPE_C64);
+                       int64_t batch, unsigned features, unsigned dtype = SN_DTYPE_C64, const MCInit *mc = nullptr);
 
 int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
               const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
@@ -869,11 +946,11 @@ static bool helmholtz_singular(const Layout &l, const double *L, double C)
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features, unsigned dtype)
+                       int64_t batch, unsigned features, unsigned dtype, const MCInit *mc)
 {
     if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
     Layout l;
-    if (!make_layout(ndim, dims, l, batch, features, dtype)) return SN_ERR_DIMS;
+    if (!make_layout(ndim, dims, l, batch, features, dtype, mc ? mc->n : 1)) return SN_ERR_DIMS;
     if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
     if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
         return SN_ERR_PARAM;
@@ -908,7 +985,14 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->diag = reinterpret_cast<double *>(c->ws + l.off_diag);
     c->sched = reinterpret_cast<int *>(c->ws + l.off_diag + 128); // inside the 256-byte block of the diagnostics
     c->f64 = dtype == SN_DTYPE_C128;
-    c->use_graph = l.cells <= ((int64_t)1 << 24);
+    c->ncomp = l.ncomp;
+    c->is_mc = mc != nullptr;
+    if (mc)
+        for (int a = 0; a < mc->n; a++) {
+            c->Ac[a] = mc->A[a]; c->Bc[a] = mc->B[a]; c->wc[a] = mc->w[a];
+            for (int b = 0; b < mc->n; b++) c->gc[a][b] = mc->g[a * mc->n + b];
+        }
+    c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc;
     c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
@@ -942,6 +1026,50 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     return SN_OK;
 }
 
+size_t sn_workspace_bytes_mc(int ndim, const int64_t *dims, int n_comp)
+{
+    Layout l;
+    return make_layout(ndim, dims, l, 1, 0, SN_DTYPE_C64, n_comp) ? l.total : 0;
+}
+
+int sn_create_mc(sn_ctx **out, int ndim, const int64_t *dims, const double *L, int n_comp, const double *A, const double *B,
+                 double C, double D, const double *w, const double *g, double dtau, void *d_workspace,
+                 size_t workspace_bytes, void *cuda_stream)
+{
+    if (!A || !B || !w || !g) return SN_ERR_NULL;
+    if (n_comp < 1 || n_comp > 4) return SN_ERR_PARAM;
+    for (int a = 0; a < n_comp; a++) {
+        if (!std::isfinite(A[a]) || !std::isfinite(B[a]) || !std::isfinite(w[a])) return SN_ERR_PARAM;
+        for (int b = 0; b < n_comp; b++)
+            if (!std::isfinite(g[a * n_comp + b])) return SN_ERR_PARAM;
+    }
+    MCInit mc;
+    mc.n = n_comp; mc.A = A; mc.B = B; mc.w = w; mc.g = g;
+    return create_impl(out, ndim, dims, L, A[0], B[0], C, D, nullptr, 0, dtau, d_workspace, workspace_bytes, cuda_stream, 1, 0,
+                       SN_DTYPE_C64, &mc);
+}
+
+int sn_mc_norms(sn_ctx *c, double *norms)
+{
+    if (!c || !norms) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    DeviceGuard guard(c->device);
+    const Layout &l = c->lay;
+    SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));
+    for (int k = 0; k < l.ncomp; k++) {
+        const int rc = snk::launch_norm(c->psi + (size_t)k * l.cells, l.cells, c->diag + k, c->stream);
+        if (rc != 0) return cuda_fail((cudaError_t)rc);
+        c->launches++;
+    }
+    double h[4];
+    SN_CUDA(cudaMemcpyAsync(h, c->diag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    double dV = 1.0;
+    for (int d = 0; d < l.ndim; d++) dV *= c->L[d] / (double)l.n[d];
+    for (int k = 0; k < l.ncomp; k++) norms[k] = h[k] * dV;
+    return SN_OK;
+}
+
 int sn_set_option(sn_ctx *c, int option, int value)
 {
     if (!c) return SN_ERR_NULL;
@@ -956,7 +1084,7 @@ int sn_set_option(sn_ctx *c, int option, int value)
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     if (option == SN_OPT_GRAPH) {
-        c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24);
+        c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24) && !c->is_mc;
     } else {
         c->use_pipe = value != 1 && !c->f64;
         c->pipe_all = value == 2 && !c->f64;
@@ -1000,6 +1128,7 @@ int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, 
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!std::isfinite(g_log) || !std::isfinite(rho_floor) || !std::isfinite(g_pow) || !std::isfinite(p_pow))
         return SN_ERR_PARAM;
     if (rho_floor <= 0.0 || p_pow == -1.0) return SN_ERR_PARAM;
@@ -1014,6 +1143,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (v && !c->vext) return SN_ERR_FEATURE; // SN_FEAT_VEXT not requested at create
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
@@ -1031,6 +1161,7 @@ int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!std::isfinite(c_bohm) || !std::isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SN_ERR_PARAM;
     if (c->f64 && c_bohm != 0.0) return SN_ERR_FEATURE;
     SN_CUDA(cudaStreamSynchronize(c->stream));
@@ -1044,6 +1175,7 @@ int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int s
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if ((beta == nullptr) != (gamma == nullptr)) return SN_ERR_NULL;
     if (beta && (!c->bg || (!src_on_device && !c->phi))) return SN_ERR_FEATURE; // SN_FEAT_SOURCE (+ SN_FEAT_STAGING for host tables)
     SN_CUDA(cudaStreamSynchronize(c->stream));
@@ -1073,7 +1205,7 @@ int sn_set_state(sn_ctx *c, const void *psi, int src_on_device)
 {
     if (!c || !psi) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * c->lay.esz,
+    SN_CUDA(cudaMemcpyAsync(c->psi, psi, (size_t)c->lay.cells * c->lay.esz * (size_t)c->lay.ncomp,
                             src_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
     if (!src_on_device) SN_CUDA(cudaStreamSynchronize(c->stream)); // caller may reuse its host buffer
     c->has_state = true;
@@ -1085,7 +1217,7 @@ int sn_get_state(sn_ctx *c, void *psi_out, int dst_on_device)
     if (!c || !psi_out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
-    SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * c->lay.esz,
+    SN_CUDA(cudaMemcpyAsync(psi_out, c->psi, (size_t)c->lay.cells * c->lay.esz * (size_t)c->lay.ncomp,
                             dst_on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
     if (!dst_on_device) SN_CUDA(cudaStreamSynchronize(c->stream));
     return SN_OK;
@@ -1098,6 +1230,14 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
+    if (c->is_mc) { // coupled components: same merged schedule, component-wise sweeps
+        int rc = kinetic_sweep_mc(c, PH_HALF);
+        for (int64_t i = 1; rc == SN_OK && i <= nsteps; i++) {
+            rc = nonlinear_mc(c, c->dtau);
+            if (rc == SN_OK) rc = kinetic_sweep_mc(c, i == nsteps ? PH_HALF : PH_FULL);
+        }
+        return rc;
+    }
     // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
     int rc = kinetic_sweep(c, PH_HALF, /*with_nl=*/false, /*before_n=*/true);
     int64_t i = 1;
@@ -1119,6 +1259,7 @@ int sn_step_order4(sn_ctx *c, int64_t nsteps)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
@@ -1140,6 +1281,7 @@ int sn_debug_fft(sn_ctx *c, int direction)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (direction != 1 && direction != -1) return SN_ERR_PARAM;
     const Layout &l = c->lay;
@@ -1164,6 +1306,7 @@ int sn_debug_potential(sn_ctx *c, float *phi_out, int dst_on_device)
 {
     if (!c || !phi_out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (!dst_on_device && !c->phi) return SN_ERR_FEATURE; // a host destination is staged through the SN_FEAT_STAGING scratch
     int rc = potential_spectrum(c);
@@ -1184,6 +1327,7 @@ int sn_diagnostics(sn_ctx *c, sn_diag *out)
 {
     if (!c || !out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
+    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     const Layout &l = c->lay;
     SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));

@@ -199,8 +199,78 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
         return;
     }
 
+    if (MODE == P_H_R2C_MC) {
+        // coupled components (reading Q18): the source of eq. (2') is sum_c w_c |psi_c|^2
+        float2 a[P], b[P];
+        const long long cs4 = p.mc.comp_stride / 2;
+#pragma unroll
+        for (int m = 0; m < P; m++) {
+            a[m] = make_float2(0.f, 0.f);
+            b[m] = make_float2(0.f, 0.f);
+            for (int c = 0; c < p.mc.ncomp; c++) {
+                const float4 u = psi4[c * cs4 + (long long)(j + T * m) * rs4 + t];
+                const float4 v = psi4[c * cs4 + (long long)(j + T * m) * rs4 + CP + t];
+                const float w = p.mc.w[c];
+                a[m] = make_float2(fmaf(w, abs2(lo2(u)), a[m].x), fmaf(w, abs2(hi2(u)), a[m].y));
+                b[m] = make_float2(fmaf(w, abs2(lo2(v)), b[m].x), fmaf(w, abs2(hi2(v)), b[m].y));
+            }
+        }
+        fft_pair<N, +1, false>(a, b, j, p.tw, sm);
+        sm.sync();
+#pragma unroll
+        for (int m = 0; m < P; m++) sm.st(j + T * m, a[m], b[m]);
+        sm.sync();
+#pragma unroll
+        for (int m = 0; m <= P / 2; m++) {
+            if (m < P / 2 || j == 0) {
+                const int k = j + T * m;
+                float2 ya, yb;
+                sm.ld((N - k) % N, ya, yb);
+                hs4[(long long)k * rs4 + t] = make_float4(a[m].x + ya.x, a[m].y - ya.y, a[m].y + ya.y, ya.x - a[m].x);
+                hs4[(long long)k * rs4 + CP + t] =
+                    make_float4(b[m].x + yb.x, b[m].y - yb.y, b[m].y + yb.y, yb.x - b[m].x);
+            }
+        }
+        return;
+    }
+
     float2 fa[P], fb[P];
     c2r_potential<N, CP>(p, hs4, rs4, t, j, fa, fb, sm);
+
+    if (MODE == P_H_NL_MC) {
+        // psi_c *= exp(-i s (B_c phi + sum_c' g_cc' rho_c')): every rho_c is read before any component is rewritten
+        const long long cs4 = p.mc.comp_stride / 2;
+        const int M = p.mc.ncomp;
+#pragma unroll
+        for (int half = 0; half < 2; half++) {
+#pragma unroll
+            for (int m = 0; m < P; m++) {
+                float4 *g4 = psi4 + half * CP + t + (long long)(j + T * m) * rs4;
+                const float2 ph = half == 0 ? fa[m] : fb[m];
+                float4 v[4];
+                float2 rho[4];
+#pragma unroll
+                for (int c = 0; c < 4; c++)
+                    if (c < M) {
+                        v[c] = g4[c * cs4];
+                        rho[c] = make_float2(abs2(lo2(v[c])), abs2(hi2(v[c])));
+                    }
+#pragma unroll
+                for (int c = 0; c < 4; c++)
+                    if (c < M) {
+                        float tx = p.mc.hb[c] * ph.x, ty = p.mc.hb[c] * ph.y;
+#pragma unroll
+                        for (int d = 0; d < 4; d++)
+                            if (d < M) {
+                                tx = fmaf(p.mc.hg[c][d], rho[d].x, tx);
+                                ty = fmaf(p.mc.hg[c][d], rho[d].y, ty);
+                            }
+                        g4[c * cs4] = pack4(rotate_half_angle(lo2(v[c]), tx), rotate_half_angle(hi2(v[c]), ty));
+                    }
+            }
+        }
+        return;
+    }
 
     if (MODE == P_H_POT) {
         float2 *out = reinterpret_cast<float2 *>(p.phi_out) + col4;
@@ -406,8 +476,12 @@ int launch_pass(const PassArgs &a)
     case P_H_POT:
     case P_H_SRC:
     case P_H_BOHM:
+    case P_H_R2C_MC:
+    case P_H_NL_MC:
     case P_H_DIAG: {
         const unsigned grid = (unsigned)(a.ncols / (4 * CP));
+        if (a.kind == P_H_R2C_MC) return launch_kernel(k_haxis<N, CP, P_H_R2C_MC>, grid, ST, SSMEM, a);
+        if (a.kind == P_H_NL_MC) return launch_kernel(k_haxis<N, CP, P_H_NL_MC>, grid, ST, SSMEM, a);
         if (a.kind == P_H_NLKIN) return launch_kernel(k_haxis<N, CP, P_H_NLKIN>, grid, ST, SSMEM, a);
         if (a.kind == P_H_R2C) return launch_kernel(k_haxis<N, CP, P_H_R2C>, grid, ST, SSMEM, a);
         if (a.kind == P_H_POT) return launch_kernel(k_haxis<N, CP, P_H_POT>, grid, ST, SSMEM, a);
@@ -444,6 +518,20 @@ __global__ void k_interleave(const float *__restrict__ beta, const float *__rest
 int launch_interleave(const float *beta, const float *gamma, float2 *bg, long long n, cudaStream_t stream)
 {
     k_interleave<<<1184, 256, 0, stream>>>(beta, gamma, bg, n);
+    return (int)cudaGetLastError();
+}
+
+// per-component norms of the coupled-field path (sn_mc_norms): fp32 squares, fp64 accumulation
+__global__ void k_norm(const float2 *__restrict__ psi, long long n, double *out)
+{
+    double v[1] = {0.0};
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        v[0] += (double)abs2(psi[i]);
+    block_accumulate<1>(v, out);
+}
+int launch_norm(const float2 *psi, long long n, double *out, cudaStream_t stream)
+{
+    k_norm<<<1184, 256, 0, stream>>>(psi, n, out);
     return (int)cudaGetLastError();
 }
 #endif

@@ -19,7 +19,19 @@ enum PassKind {
     P_X_POISSON,   // contiguous axis of the half spectrum: forward -> D/(C-k^2) -> inverse (S5-S7)
     P_X_KDIAG,     // contiguous axis: forward, accumulate sum k_x^2 |psi^|^2
     P_H_SRC,       // axis 0: c2r of F[lap rho] -> s = gamma rho + beta lap rho -> packed r2c   (eq. (12), NEXT-1)
-    P_H_BOHM       // axis 0: c2r of F[lap sqrt(rho)] -> psi *= exp(-i s c_B lap sqrt(rho)/(2 sqrt(rho)))  (eq. (15))
+    P_H_BOHM,      // axis 0: c2r of F[lap sqrt(rho)] -> psi *= exp(-i s c_B lap sqrt(rho)/(2 sqrt(rho)))  (eq. (15))
+    P_H_R2C_MC,    // axis 0, coupled components: rho = sum_c w_c |psi_c|^2 -> packed r2c
+    P_H_NL_MC      // axis 0, coupled components: c2r of phi^ -> psi_c *= exp(-i s (B_c phi + sum_c' g_cc' rho_c')) for every c
+};
+
+// Coupled wave functions (NEXT-4b; reading Q18 of DESIGN.md): up to 4 components, stored one after the other
+// (component c at data + c * comp_stride); half-angle coefficients like NLParams.
+struct MCParams {
+    int ncomp;
+    long long comp_stride; // complex elements between components
+    float w[4];            // source weights of eq. (2')
+    float hb[4];           // -s/2 * B_c
+    float hg[4][4];        // -s/2 * g_cc'
 };
 
 // Nonlinear phase psi *= exp(-i dtau (B phi + sum_j g_j rho^j)), stored as HALF-angle
@@ -64,6 +76,7 @@ struct PassArgs {
     float hbohm, sfloor;    // P_H_BOHM: half angle = hbohm * W / max(sqrt(rho), sfloor), hbohm = -s c_B/4; floor of sqrt(rho)
     double *diag;           // DEVICE: accumulators
     int nl_slot;            // which nonlinear sub-step the coefficients in `nl` belong to (scheduler bookkeeping)
+    MCParams mc;            // P_H_R2C_MC / P_H_NL_MC
     cudaStream_t stream;
 };
 
@@ -161,6 +174,9 @@ struct PassArgsD {
 };
 template <int N>
 int launch_pass_d(const PassArgsD &a);
+
+// sum |psi|^2 over n complex64 values, accumulated in double into *out (sn_mc_norms)
+int launch_norm(const float2 *psi, long long n, double *out, cudaStream_t stream);
 
 // setup helper (not part of a step): bg[i] = (beta[i], gamma[i])
 int launch_interleave(const float *beta, const float *gamma, float2 *bg, long long n, cudaStream_t stream);

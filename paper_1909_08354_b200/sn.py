@@ -30,10 +30,10 @@ DISPATCH_DEFAULT, DISPATCH_FIRST_PATH, DISPATCH_PIPELINED = 0, 1, 2
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
            "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm", "sn_workspace_bytes_opt",
-           "sn_create_opt", "sn_set_option")
+           "sn_create_opt", "sn_set_option", "sn_workspace_bytes_mc", "sn_create_mc", "sn_mc_norms")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
-              "X_KDIAG", "H_SRC", "H_BOHM")
+              "X_KDIAG", "H_SRC", "H_BOHM", "H_R2C_MC", "H_NL_MC")
 
 
 class SnDiag(ctypes.Structure):
@@ -88,6 +88,11 @@ def lib() -> ctypes.CDLL:
                                     ctypes.c_double, ctypes.c_double, dp, ctypes.c_int, ctypes.c_double, vp,
                                     ctypes.c_size_t, vp, ctypes.POINTER(SnOptions)]
         L.sn_set_option.argtypes = [vp, ctypes.c_int, ctypes.c_int]
+        L.sn_workspace_bytes_mc.argtypes = [ctypes.c_int, i64p, ctypes.c_int]
+        L.sn_workspace_bytes_mc.restype = ctypes.c_size_t
+        L.sn_create_mc.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_int, dp, dp, ctypes.c_double,
+                                   ctypes.c_double, dp, dp, ctypes.c_double, vp, ctypes.c_size_t, vp]
+        L.sn_mc_norms.argtypes = [vp, dp]
         L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_step.argtypes = [vp, ctypes.c_int64]
         L.sn_step_order4.argtypes = [vp, ctypes.c_int64]
@@ -314,3 +319,41 @@ class Simulation:
                               device=self.device)
             _chk(lib().sn_debug_potential(self._h, ctypes.c_void_p(dev.data_ptr()), 1), "sn_debug_potential")
             return dev.cpu().numpy()
+
+
+class CoupledSimulation(Simulation):
+    """Coupled wave functions (sn_create_mc, reading Q18 of DESIGN.md): state shape (M,) + dims, complex64.
+    i dpsi_c/dtau = A_c lap psi_c + B_c phi psi_c + (sum_c' g[c][c'] |psi_c'|^2) psi_c; lap phi + C phi = D sum_c w_c |psi_c|^2."""
+
+    def __init__(self, dims: Sequence[int], L, A: Sequence[float], B: Sequence[float], C: float, D: float,
+                 w: Sequence[float], g, dtau: float, device: str = "cuda:0", stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1909_08354_b200 needs a CUDA device (no CPU fallback)")
+        pd = tuple(int(n) for n in dims)
+        nd, M = len(pd), len(A)
+        gm = np.ascontiguousarray(g, dtype=np.float64)
+        assert gm.shape == (M, M) and len(B) == M and len(w) == M
+        self.dims = (M,) + pd
+        self.features = 0
+        self.dtype, self.real_dtype = np.dtype(np.complex64), np.dtype(np.float32)
+        Ls = [float(L)] * nd if np.isscalar(L) else [float(v) for v in L]
+        self.device = torch.device(device)
+        c_dims = (ctypes.c_int64 * nd)(*pd)
+        nbytes = int(lib().sn_workspace_bytes_mc(nd, c_dims, M))
+        if nbytes == 0:
+            raise SnError(-2, "sn_workspace_bytes_mc", lib().sn_strerror(-2).decode())
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._h = ctypes.c_void_p()
+        arr = lambda v: (ctypes.c_double * len(v))(*[float(x) for x in v])
+        _chk(lib().sn_create_mc(ctypes.byref(self._h), nd, c_dims, arr(Ls), M, arr(A), arr(B), C, D, arr(w),
+                                arr(gm.ravel()), dtau, ctypes.c_void_p(self._ws.data_ptr()), nbytes,
+                                ctypes.c_void_p(self._stream.cuda_stream)), "sn_create_mc")
+
+    def norms(self) -> np.ndarray:
+        out = (ctypes.c_double * self.dims[0])()
+        _chk(lib().sn_mc_norms(self._h, out), "sn_mc_norms")
+        return np.array(out[:])
