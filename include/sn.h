@@ -183,6 +183,47 @@ int sn_create_mc(sn_ctx **out, int ndim, const int64_t *dims, const double *L, i
                  void *d_workspace, size_t workspace_bytes, void *cuda_stream);
 int sn_mc_norms(sn_ctx *ctx, double *norms);
 
+/* ---- NEXT-2: slab-decomposed step for R ranks (the paper's solver is single-device,
+ * PAPER.md:113) ----
+ * 3D, complex64, eq. (1),(2) with the polynomial G.  The grid dims[0] x dims[1] x dims[2] is split over nranks
+ * ranks; rank r owns the z-slab rows [r dims[0]/R, (r+1) dims[0]/R) of axis 0 ("view A", [dims[0]/R][dims[1]][dims[2]]:
+ * the layout of sn_set_state / sn_get_state on such a context).  Lines along axes 1 and 2 are whole in view A; for
+ * the passes along axis 0 the data is moved to the y-slab view B = [dims[0]][dims[1]/R][dims[2]] by an all-to-all,
+ * and back: 4 exchanges per step (psi twice, 8 B/cell; the half spectrum twice, 4 B/cell).  The library runs the LOCAL
+ * passes (sn_slab_stage) and the pack/unpack copies; the exchange itself belongs to the caller: sn_slab_exchange_local
+ * for R contexts on ONE device and stream (virtual ranks: how the path is validated on one GPU), or, one process per
+ * GPU, any all-to-all over the buffers of sn_slab_buffer (paper_1909_08354_b200/slab.py uses torch.distributed, i.e.
+ * NCCL over NVLink; not measured on hardware in this build).  Requirements: dims[0], dims[1] and dims[0]/2 divisible
+ * by nranks; (dims[1]/nranks) * dims[2] a multiple of 32.  The half-spectrum rows 0..dims[0]/2 are dealt out
+ * (dims[0]/2)/nranks per rank, the Nyquist row to the last rank.
+ * One call of n steps, psi starting and ending in view A (half_phase = 1 on the first and last kinetic sweep):
+ *   KIN_A(half) | psi A->B | KIN0_B(half)
+ *   n times: R2C_B | hs B->A | CHAIN_A | hs A->B | NLKIN_B(half on the last step) | psi B->A | KIN_A(same) | psi A->B
+ *   (the last psi A->B is dropped)
+ * Exchange buffers: view-B buffers hold the block for / from rank r contiguously (rows r dims[0]/R ... of psi_B, rows
+ * h_lo(r) ... of hs_B); sn_slab_pack gathers the blocks of a view-A buffer into the staging buffer in rank order
+ * (unpack = 0) or scatters them back (unpack = 1).  sn_step and the other whole-grid calls return SN_ERR_FEATURE on a
+ * slab context; sn_set_state, sn_get_state, sn_set_dtau, sn_destroy, sn_profile*, sn_launch_count work. */
+#define SN_SLAB_KIN_A 0    /* stages of sn_slab_stage */
+#define SN_SLAB_KIN0_B 1
+#define SN_SLAB_R2C_B 2
+#define SN_SLAB_CHAIN_A 3
+#define SN_SLAB_NLKIN_B 4
+#define SN_SLAB_PSI_A 0    /* buffers of sn_slab_buffer; PSI_A / HS_A also name WHAT an exchange or a pack moves */
+#define SN_SLAB_PSI_B 1
+#define SN_SLAB_HS_A 2
+#define SN_SLAB_HS_B 3
+#define SN_SLAB_STAGING 4
+size_t sn_slab_workspace_bytes(const int64_t *dims /* host, 3 */, int nranks, int rank);
+int sn_slab_create(sn_ctx **out, const int64_t *dims, const double *L, double A, double B, double C, double D,
+                   const double *g, int n_g, double dtau, int nranks, int rank, void *d_workspace,
+                   size_t workspace_bytes, void *cuda_stream);
+int sn_slab_stage(sn_ctx *ctx, int stage, int half_phase);
+int sn_slab_buffer(sn_ctx *ctx, int which, void **ptr /* host; receives a DEVICE pointer */, int64_t *elems /* complex64 */);
+int sn_slab_pack(sn_ctx *ctx, int what /* SN_SLAB_PSI_A or SN_SLAB_HS_A */, int unpack);
+int sn_slab_exchange_local(sn_ctx **ctxs /* host, nranks contexts in rank order */, int nranks, int what, int to_a);
+int sn_slab_local_norm(sn_ctx *ctx, double *sum_abs2_dv /* host: this rank's part of the norm */);
+
 int sn_destroy(sn_ctx *ctx);
 
 /* Text for an error code; for SN_ERR_CUDA the last CUDA error string seen by this thread. */

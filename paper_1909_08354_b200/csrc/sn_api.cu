@@ -76,15 +76,35 @@ struct Layout {
     unsigned dtype;    // SN_DTYPE_*
     size_t esz;        // bytes of a complex value: 8 (complex64) or 16 (complex128)
     int ncomp;         // coupled wave functions (sn_create_mc): psi holds ncomp arrays one after the other; else 1
+    // slab decomposition (sn_slab_create; 3D, complex64): rank `rank` of R.  n[] stay the GLOBAL dims (pcells too);
+    // cells = the LOCAL cell count; "A" = the z-slab view [n0/R][n1][n2] (axis-1/2 passes; psi = psi_A, hs = hs_A with
+    // h_cnt of the n0/2+1 half-spectrum rows, starting at h_lo), "B" = the y-slab view [n0][n1/R][n2] (axis-0 passes;
+    // cols0 = (n1/R) n2 is its column count)
+    int R, rank;
+    int64_t rowsA, n1B, h_lo, h_cnt, hsB_elems;
+    size_t off_psiB, off_hsB, off_stage;
     size_t off_psi, off_hs, off_phi, off_vext, off_bg, off_tw[3], off_ph[5][3], off_ksq[3], off_ksq2[3], off_kother[2],
         off_diag, total;
 };
 
+// rows [lo, lo + cnt) of the n0/2+1 half-spectrum rows owned by rank r of R in the z-slab view: (n0/2)/R each, the
+// Nyquist row n0/2 goes to the last rank
+inline void slab_hs_rows(int64_t n0, int R, int r, int64_t &lo, int64_t &cnt)
+{
+    const int64_t per = (n0 / 2) / R;
+    lo = per * r;
+    cnt = per + (r == R - 1 ? 1 : 0);
+}
+
 bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, unsigned features = 0,
-                 unsigned dtype = SN_DTYPE_C64, int ncomp = 1)
+                 unsigned dtype = SN_DTYPE_C64, int ncomp = 1, int R = 1, int rank = 0)
 {
     if (ncomp < 1 || ncomp > 4) return false;
     L.ncomp = ncomp;
+    if (R < 1 || rank < 0 || rank >= R) return false;
+    if (R > 1 && (ndim != 3 || batch != 1 || features != 0 || dtype != SN_DTYPE_C64 || ncomp != 1)) return false;
+    L.R = R;
+    L.rank = rank;
     if (!dims || (ndim != 2 && ndim != 3)) return false;
     if (batch < 1 || batch > (1 << 20)) return false;
     if (features & ~SN_FEAT_ALL) return false;
@@ -107,6 +127,20 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, un
     L.hs_lines = (L.n[0] / 2 + 1) * L.cols0 / L.nx;
     if (L.hs_lines & 1) L.hs_lines++; // line pairs: one dummy line (2D)
     L.hs_elems = L.hs_lines * L.nx;
+    L.rowsA = L.n[0]; L.n1B = L.n[1]; L.h_lo = 0; L.h_cnt = L.n[0] / 2 + 1; L.hsB_elems = 0;
+    if (R > 1) {
+        // every rank needs whole tiles in both views: n0/R rows and n1/R columns per rank, (n0/2)/R spectrum rows
+        if (L.n[0] % R || L.n[1] % R || (L.n[0] / 2) % R) return false;
+        L.rowsA = L.n[0] / R;
+        L.n1B = L.n[1] / R;
+        if ((L.n1B * L.n[2]) % 32) return false; // axis-0 tiles are up to 32 columns wide
+        slab_hs_rows(L.n[0], R, rank, L.h_lo, L.h_cnt);
+        L.cells = L.rowsA * L.n[1] * L.n[2];
+        L.cols0 = L.n1B * L.n[2];
+        L.hs_lines = L.h_cnt * L.n[1];              // lines of hs_A
+        L.hs_elems = L.hs_lines * L.nx;
+        L.hsB_elems = (L.n[0] / 2 + 1) * L.cols0;   // hs_B
+    }
     // the kernels index columns, lines and outer blocks with 32-bit ints: reject ensembles that do not fit
     if (L.cols0 > INT_MAX || L.cells / L.nx > INT_MAX || L.hs_lines > INT_MAX || L.n[0] * batch > INT_MAX) return false;
     size_t o = 0;
@@ -126,6 +160,12 @@ bool make_layout(int ndim, const int64_t *dims, Layout &L, int64_t batch = 1, un
     L.off_phi = o; if (features & SN_FEAT_STAGING) o = align256(o + (size_t)L.cells * 4);
     L.off_vext = o; if (features & SN_FEAT_VEXT) o = align256(o + (size_t)L.cells * 4);
     L.off_bg = o; if (features & SN_FEAT_SOURCE) o = align256(o + (size_t)L.cells * 8);
+    L.off_psiB = L.off_hsB = L.off_stage = o;
+    if (R > 1) {
+        L.off_psiB = o; o = align256(o + (size_t)L.cells * 8);
+        L.off_hsB = o; o = align256(o + (size_t)L.hsB_elems * 8);
+        L.off_stage = o; o = align256(o + (size_t)L.cells * 8); // pack/unpack staging of the distributed exchange
+    }
     L.total = o;
     return true;
 }
@@ -217,6 +257,7 @@ struct sn_ctx {
     snk::NLParams nlv[3];           // nonlinear coefficients per slot (NL_*)
     // coupled wave functions (NEXT-4b; reading Q18): per-component constants; component c's state is
     // psi + c * cells, its kinetic phase tables ph[slot][axis] + c * n[axis]
+    float2 *psiB, *hsB, *stage;             // slab contexts: the y-slab view buffers and the exchange staging
     int ncomp;
     bool is_mc; // created by sn_create_mc (also with ncomp == 1): sn_step runs the coupled scheduler
     double Ac[4], Bc[4], wc[4], gc[4][4];
@@ -339,12 +380,14 @@ int make_tensor_maps(sn_ctx *c)
     const Layout &l = c->lay;
     int rc;
     c->m_ok[0] = c->m_ok[1] = false;
+    // axis-0 views (slab contexts: the y-slab buffers psi_B / hs_B, n0 rows x (n1/R) n2 columns)
+    float2 *p0 = l.R > 1 ? c->psiB : c->psi, *h0 = l.R > 1 ? c->hsB : c->hs;
     if (l.n[0] >= 64 && l.cols0 % (2 * snk::pipe_groups((int)l.n[0])) == 0) {
         const int n0 = (int)l.n[0], cpw = snk::pipe_cpw(n0);
-        if ((rc = make_map(&c->m_psi[0], c->psi, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
-        if ((rc = make_map(&c->m_hs0, c->hs, 1, n0 / 2 + 1, l.cols0, snk::pipe_box_rows(n0 / 2), cpw))) return rc;
-        if ((rc = make_map(&c->m_hs0_row, c->hs, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
-        if ((rc = make_map(&c->m_bg, c->bg, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
+        if ((rc = make_map(&c->m_psi[0], p0, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs0, h0, 1, n0 / 2 + 1, l.cols0, snk::pipe_box_rows(n0 / 2), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs0_row, h0, 1, n0 / 2 + 1, l.cols0, 1, cpw))) return rc;
+        if (c->bg && (rc = make_map(&c->m_bg, c->bg, 1, n0, l.cols0, snk::pipe_box_rows(n0), cpw))) return rc;
         c->m_ok[0] = true;
     }
     for (int k = 1; k < l.ncomp; k++) { // coupled components: their own views of psi_k (same geometry)
@@ -355,8 +398,9 @@ int make_tensor_maps(sn_ctx *c)
     }
     if (l.ndim == 3 && l.n[1] >= 64 && l.n[2] % (2 * snk::pipe_groups((int)l.n[1])) == 0) {
         const int n1 = (int)l.n[1], cpw = snk::pipe_cpw(n1);
-        if ((rc = make_map(&c->m_psi[1], c->psi, l.n[0] * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
-        if ((rc = make_map(&c->m_hs1, c->hs, (l.n[0] / 2 + 1) * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
+        // axis-1 views (slab contexts: the z-slab buffers, rowsA rows of psi and h_cnt rows of the half spectrum)
+        if ((rc = make_map(&c->m_psi[1], c->psi, l.rowsA * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
+        if ((rc = make_map(&c->m_hs1, c->hs, l.h_cnt * l.batch, n1, l.n[2], snk::pipe_box_rows(n1), cpw))) return rc;
         c->m_ok[1] = true;
     }
     return SN_OK;
@@ -599,13 +643,13 @@ int upload_static_tables(sn_ctx *c)
     // nearly cancels k^2 (a plain float C - k^2 has an absolute error of 1e-7 k^2 there).
     // Lines of the half spectrum are indexed (k0, member[, k1]); the member index carries no wavenumber.
     std::vector<f2> ko(l.hs_lines);
-    const int64_t h0 = l.n[0] / 2 + 1;
+    const int64_t h0 = l.h_cnt; // slab contexts: the rows h_lo .. h_lo + h_cnt of the half spectrum
     for (int tab = 0; tab < 2; tab++) {
         const double c0 = tab == 0 ? c->C : 0.0;
         auto enc = [&](double v) { return c->f64 ? as_double(v) : split_real(v); };
         std::fill(ko.begin(), ko.end(), enc(tab == 0 && c->C != 0.0 ? c->C : -1.0)); // padding line: any finite non-zero value
         for (int64_t k0 = 0; k0 < h0; k0++) {
-            const double a = kval(k0, l.n[0], c->L[0]);
+            const double a = kval(l.h_lo + k0, l.n[0], c->L[0]);
             for (int64_t b = 0; b < l.batch; b++) {
                 if (l.ndim == 2) {
                     ko[k0 * l.batch + b] = enc(c0 - a * a);
@@ -818,6 +862,87 @@ int nonlinear_mc(sn_ctx *c, double s)
     return run_pass(c, (int)l.n[0], a);
 }
 
+// ---- slab-decomposed step (NEXT-2): the LOCAL passes of rank `rank` of R ----
+// Lines along axis 0 are whole in the y-slab view B = [n0][n1/R][n2], lines along axes 1 and 2 in the z-slab view
+// A = [n0/R][n1][n2]; between the stages below the caller moves psi (8 B/cell) or the half spectrum (4 B/cell) from
+// one view to the other with an all-to-all (sn_slab_exchange_local for R contexts on one device; pack / all_to_all /
+// unpack for one process per GPU).  The kernels are the ones of the single-GPU step, on the local geometry.
+void slab_axis1(const sn_ctx *c, PassArgs &a, int64_t rows)
+{
+    const Layout &l = c->lay;
+    a.axis = 1; a.n_outer = (int)rows; a.outer_stride = l.n[1] * l.n[2]; a.ncols = (int)l.n[2]; a.row_stride = l.n[2];
+}
+void slab_axis0(const sn_ctx *c, PassArgs &a)
+{
+    const Layout &l = c->lay;
+    a.axis = 0; a.n_outer = 1; a.outer_stride = 0; a.ncols = (int)l.cols0; a.row_stride = l.cols0;
+}
+
+int slab_stage(sn_ctx *c, int stage, int ph_slot)
+{
+    const Layout &l = c->lay;
+    int rc;
+    switch (stage) {
+    case SN_SLAB_KIN_A: { // kinetic passes along axes 1 and 2 on psi_A
+        PassArgs a = base_args(c);
+        a.kind = snk::P_S_KIN; a.data = c->psi; a.tw = c->tw[1]; a.phase = c->ph[ph_slot][1]; a.vext = nullptr;
+        slab_axis1(c, a, l.rowsA);
+        if ((rc = run_pass(c, (int)l.n[1], a))) return rc;
+        PassArgs b = base_args(c);
+        b.kind = snk::P_X_KIN; b.data = c->psi; b.tw = c->tw[2]; b.phase = c->ph[ph_slot][2]; b.vext = nullptr;
+        b.nlines = (int)(l.cells / l.nx);
+        return run_pass(c, (int)l.n[2], b);
+    }
+    case SN_SLAB_KIN0_B: { // kinetic pass along axis 0 on psi_B, no nonlinear phase (opening sweep of a call)
+        PassArgs a = base_args(c);
+        a.kind = snk::P_S_KIN; a.data = c->psiB; a.tw = c->tw[0]; a.phase = c->ph[ph_slot][0]; a.vext = nullptr;
+        slab_axis0(c, a);
+        return run_pass(c, (int)l.n[0], a);
+    }
+    case SN_SLAB_R2C_B: { // rho = |psi_B|^2 -> packed r2c along axis 0 -> hs_B
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_R2C; a.data = c->psiB; a.hs = c->hsB; a.tw = c->tw[0];
+        slab_axis0(c, a);
+        return run_pass(c, (int)l.n[0], a);
+    }
+    case SN_SLAB_CHAIN_A: { // hs_A: forward along axis 1 -> forward, D/(C - k^2), inverse along axis 2 -> inverse along axis 1
+        PassArgs a = base_args(c);
+        a.kind = snk::P_S_FFT; a.dir = +1; a.hilo = 0; a.data = c->hs; a.tw = c->tw[1];
+        slab_axis1(c, a, l.h_cnt);
+        if ((rc = run_pass(c, (int)l.n[1], a))) return rc;
+        PassArgs x = base_args(c);
+        x.kind = snk::P_X_POISSON; x.data = c->hs; x.tw = c->tw[2]; x.ksq2 = c->ksq2[2]; x.dko = c->kother[0];
+        x.nlines = (int)l.hs_lines;
+        x.pscale = (float)(c->D * 0.5 / (double)l.pcells);
+        if ((rc = run_pass(c, (int)l.n[2], x))) return rc;
+        a.dir = -1;
+        return run_pass(c, (int)l.n[1], a);
+    }
+    case SN_SLAB_NLKIN_B: { // c2r of hs_B -> nonlinear phase -> kinetic pass along axis 0, on psi_B
+        PassArgs a = base_args(c);
+        a.kind = snk::P_H_NLKIN; a.data = c->psiB; a.hs = c->hsB; a.tw = c->tw[0]; a.phase = c->ph[ph_slot][0];
+        a.nl = c->nlv[NL_MAIN]; a.nl_slot = NL_MAIN; a.vext = nullptr;
+        slab_axis0(c, a);
+        return run_pass(c, (int)l.n[0], a);
+    }
+    default:
+        return SN_ERR_PARAM;
+    }
+}
+
+// block of the exchange between the y-slab buffer of rank s and the z-slab buffer of rank r: rows [lo, lo + cnt) of
+// s's B array (contiguous there), columns s (n1/R) n2 ... of r's A array (pitch n1 n2)
+int slab_copy_block(const Layout &l, float2 *A_r, float2 *B_s, int64_t lo, int64_t cnt, int s, bool b2a, cudaStream_t st)
+{
+    const size_t width = (size_t)l.cols0 * 8;                       // bytes of one row of a block
+    float2 *bp = B_s + (size_t)lo * l.cols0;                        // contiguous in B
+    float2 *ap = A_r + (size_t)s * l.cols0;                         // strided in A
+    const size_t apitch = (size_t)l.n[1] * l.n[2] * 8;
+    const cudaError_t e = b2a ? cudaMemcpy2DAsync(ap, apitch, bp, width, width, (size_t)cnt, cudaMemcpyDeviceToDevice, st)
+                              : cudaMemcpy2DAsync(bp, width, ap, apitch, width, (size_t)cnt, cudaMemcpyDeviceToDevice, st);
+    return e == cudaSuccess ? SN_OK : cuda_fail(e);
+}
+
 // capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
 int build_step_graph(sn_ctx *c)
 {
@@ -887,7 +1012,8 @@ size_t sn_workspace_bytes_opt(int ndim, const int64_t *dims, const sn_options *o
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features, unsigned dtype = SN_DTYPE_C64, const MCInit *mc = nullptr);
+                       int64_t batch, unsigned features, unsigned dtype = SN_DTYPE_C64, const MCInit *mc = nullptr, int R = 1,
+                       int rank = 0);
 
 int sn_create(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
               const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream)
@@ -946,11 +1072,11 @@ static bool helmholtz_singular(const Layout &l, const double *L, double C)
 
 static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double *L, double A, double B, double C, double D,
                        const double *g, int n_g, double dtau, void *d_workspace, size_t workspace_bytes, void *cuda_stream,
-                       int64_t batch, unsigned features, unsigned dtype, const MCInit *mc)
+                       int64_t batch, unsigned features, unsigned dtype, const MCInit *mc, int R, int rank)
 {
     if (!out || !dims || !L || !d_workspace || (n_g > 0 && !g)) return SN_ERR_NULL;
     Layout l;
-    if (!make_layout(ndim, dims, l, batch, features, dtype, mc ? mc->n : 1)) return SN_ERR_DIMS;
+    if (!make_layout(ndim, dims, l, batch, features, dtype, mc ? mc->n : 1, R, rank)) return SN_ERR_DIMS;
     if (n_g < 0 || n_g > 4) return SN_ERR_PARAM;
     if (!std::isfinite(A) || !std::isfinite(B) || !std::isfinite(C) || !std::isfinite(D) || !std::isfinite(dtau))
         return SN_ERR_PARAM;
@@ -974,6 +1100,10 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->phi = (features & SN_FEAT_STAGING) ? reinterpret_cast<float *>(c->ws + l.off_phi) : nullptr;
     c->vext = (features & SN_FEAT_VEXT) ? reinterpret_cast<float *>(c->ws + l.off_vext) : nullptr;
     c->bg = (features & SN_FEAT_SOURCE) ? reinterpret_cast<float2 *>(c->ws + l.off_bg) : nullptr;
+    // one rank: the two views coincide
+    c->psiB = l.R > 1 ? reinterpret_cast<float2 *>(c->ws + l.off_psiB) : c->psi;
+    c->hsB = l.R > 1 ? reinterpret_cast<float2 *>(c->ws + l.off_hsB) : c->hs;
+    c->stage = l.R > 1 ? reinterpret_cast<float2 *>(c->ws + l.off_stage) : nullptr;
     c->rho_floor = 1e-30; c->p_pow = 1.0; c->sqrt_floor = 1e-30;
     for (int d = 0; d < ndim; d++) {
         c->tw[d] = reinterpret_cast<const float4 *>(c->ws + l.off_tw[d]);
@@ -992,7 +1122,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
             c->Ac[a] = mc->A[a]; c->Bc[a] = mc->B[a]; c->wc[a] = mc->w[a];
             for (int b = 0; b < mc->n; b++) c->gc[a][b] = mc->g[a * mc->n + b];
         }
-    c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc;
+    c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc && l.R == 1;
     c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
@@ -1070,6 +1200,106 @@ int sn_mc_norms(sn_ctx *c, double *norms)
     return SN_OK;
 }
 
+size_t sn_slab_workspace_bytes(const int64_t *dims, int nranks, int rank)
+{
+    Layout l;
+    return make_layout(3, dims, l, 1, 0, SN_DTYPE_C64, 1, nranks, rank) ? l.total : 0;
+}
+
+int sn_slab_create(sn_ctx **out, const int64_t *dims, const double *L, double A, double B, double C, double D,
+                   const double *g, int n_g, double dtau, int nranks, int rank, void *d_workspace, size_t workspace_bytes,
+                   void *cuda_stream)
+{
+    if (nranks < 1 || rank < 0 || rank >= nranks) return SN_ERR_PARAM;
+    return create_impl(out, 3, dims, L, A, B, C, D, g, n_g, dtau, d_workspace, workspace_bytes, cuda_stream, 1, 0,
+                       SN_DTYPE_C64, nullptr, nranks, rank);
+}
+
+int sn_slab_stage(sn_ctx *c, int stage, int half_phase)
+{
+    if (!c) return SN_ERR_NULL;
+    if (c->lay.R < 1 || c->lay.ndim != 3 || c->is_mc || c->f64 || c->lay.batch != 1) return SN_ERR_FEATURE;
+    if (!c->has_state) return SN_ERR_STATE;
+    DeviceGuard guard(c->device);
+    return slab_stage(c, stage, half_phase ? PH_HALF : PH_FULL);
+}
+
+int sn_slab_buffer(sn_ctx *c, int which, void **ptr, int64_t *elems)
+{
+    if (!c || !ptr || !elems) return SN_ERR_NULL;
+    const Layout &l = c->lay;
+    if (l.ndim != 3 || c->is_mc || c->f64 || l.batch != 1) return SN_ERR_FEATURE;
+    switch (which) {
+    case SN_SLAB_PSI_A: *ptr = c->psi; *elems = l.cells; break;
+    case SN_SLAB_PSI_B: *ptr = c->psiB; *elems = l.cells; break;
+    case SN_SLAB_HS_A: *ptr = c->hs; *elems = l.hs_elems; break;
+    case SN_SLAB_HS_B: *ptr = c->hsB; *elems = l.R > 1 ? l.hsB_elems : l.hs_elems; break;
+    case SN_SLAB_STAGING: *ptr = c->stage; *elems = l.cells; break;
+    default: return SN_ERR_PARAM;
+    }
+    return SN_OK;
+}
+
+// staging <-> z-slab view: staging holds, for each peer s, the block (rows of this rank) x (columns of s) contiguously
+int sn_slab_pack(sn_ctx *c, int what, int unpack)
+{
+    if (!c) return SN_ERR_NULL;
+    const Layout &l = c->lay;
+    if (what != SN_SLAB_PSI_A && what != SN_SLAB_HS_A) return SN_ERR_PARAM;
+    if (l.R <= 1) return SN_OK; // one rank: view A is view B
+    DeviceGuard guard(c->device);
+    float2 *A = what == SN_SLAB_PSI_A ? c->psi : c->hs;
+    const int64_t rows = what == SN_SLAB_PSI_A ? l.rowsA : l.h_cnt;
+    for (int s = 0; s < l.R; s++) {
+        // the staging area seen as a B-like array of R blocks of `rows` rows: block s starts at row s * rows
+        const int rc = slab_copy_block(l, A, c->stage, (int64_t)s * rows, rows, s, /*b2a=*/unpack != 0, c->stream);
+        if (rc) return rc;
+    }
+    return SN_OK;
+}
+
+int sn_slab_exchange_local(sn_ctx **ctxs, int nranks, int what, int to_a)
+{
+    if (!ctxs) return SN_ERR_NULL;
+    if (what != SN_SLAB_PSI_A && what != SN_SLAB_HS_A) return SN_ERR_PARAM;
+    for (int r = 0; r < nranks; r++)
+        if (!ctxs[r] || ctxs[r]->lay.R != nranks || ctxs[r]->lay.rank != r || ctxs[r]->device != ctxs[0]->device ||
+            ctxs[r]->stream != ctxs[0]->stream)
+            return SN_ERR_PARAM; // R contexts of one decomposition, on one device and one stream
+    if (nranks == 1) return SN_OK;
+    DeviceGuard guard(ctxs[0]->device);
+    for (int r = 0; r < nranks; r++)     // destination (to_a) / source (!to_a) of the z-slab side
+        for (int s = 0; s < nranks; s++) {
+            const Layout &lr = ctxs[r]->lay;
+            int64_t lo = (int64_t)r * lr.rowsA, cnt = lr.rowsA;
+            if (what == SN_SLAB_HS_A) { lo = lr.h_lo; cnt = lr.h_cnt; }
+            float2 *A_r = what == SN_SLAB_PSI_A ? ctxs[r]->psi : ctxs[r]->hs;
+            float2 *B_s = what == SN_SLAB_PSI_A ? ctxs[s]->psiB : ctxs[s]->hsB;
+            const int rc = slab_copy_block(lr, A_r, B_s, lo, cnt, s, to_a != 0, ctxs[0]->stream);
+            if (rc) return rc;
+        }
+    return SN_OK;
+}
+
+int sn_slab_local_norm(sn_ctx *c, double *sum_abs2_dv)
+{
+    if (!c || !sum_abs2_dv) return SN_ERR_NULL;
+    if (!c->has_state) return SN_ERR_STATE;
+    DeviceGuard guard(c->device);
+    const Layout &l = c->lay;
+    SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));
+    const int rc = snk::launch_norm(c->psi, l.cells, c->diag, c->stream);
+    if (rc != 0) return cuda_fail((cudaError_t)rc);
+    c->launches++;
+    double h = 0.0;
+    SN_CUDA(cudaMemcpyAsync(&h, c->diag, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    SN_CUDA(cudaStreamSynchronize(c->stream));
+    double dV = 1.0;
+    for (int d = 0; d < l.ndim; d++) dV *= c->L[d] / (double)l.n[d];
+    *sum_abs2_dv = h * dV;
+    return SN_OK;
+}
+
 int sn_set_option(sn_ctx *c, int option, int value)
 {
     if (!c) return SN_ERR_NULL;
@@ -1084,7 +1314,7 @@ int sn_set_option(sn_ctx *c, int option, int value)
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     if (option == SN_OPT_GRAPH) {
-        c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24) && !c->is_mc;
+        c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24) && !c->is_mc && c->lay.R == 1;
     } else {
         c->use_pipe = value != 1 && !c->f64;
         c->pipe_all = value == 2 && !c->f64;
@@ -1128,7 +1358,7 @@ int sn_set_local_terms(sn_ctx *c, double g_log, double rho_floor, double g_pow, 
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!std::isfinite(g_log) || !std::isfinite(rho_floor) || !std::isfinite(g_pow) || !std::isfinite(p_pow))
         return SN_ERR_PARAM;
     if (rho_floor <= 0.0 || p_pow == -1.0) return SN_ERR_PARAM;
@@ -1143,7 +1373,7 @@ int sn_set_external_potential(sn_ctx *c, const float *v, int src_on_device)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (v && !c->vext) return SN_ERR_FEATURE; // SN_FEAT_VEXT not requested at create
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
@@ -1161,7 +1391,7 @@ int sn_set_bohm(sn_ctx *c, double c_bohm, double sqrt_floor)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!std::isfinite(c_bohm) || !std::isfinite(sqrt_floor) || sqrt_floor <= 0.0) return SN_ERR_PARAM;
     if (c->f64 && c_bohm != 0.0) return SN_ERR_FEATURE;
     SN_CUDA(cudaStreamSynchronize(c->stream));
@@ -1175,7 +1405,7 @@ int sn_set_source_tables(sn_ctx *c, const float *beta, const float *gamma, int s
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if ((beta == nullptr) != (gamma == nullptr)) return SN_ERR_NULL;
     if (beta && (!c->bg || (!src_on_device && !c->phi))) return SN_ERR_FEATURE; // SN_FEAT_SOURCE (+ SN_FEAT_STAGING for host tables)
     SN_CUDA(cudaStreamSynchronize(c->stream));
@@ -1229,6 +1459,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     DeviceGuard guard(c->device);
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
+    if (c->lay.R > 1) return SN_ERR_FEATURE; // a slab context advances through sn_slab_stage + the caller's exchanges
     if (nsteps == 0) return SN_OK;
     if (c->is_mc) { // coupled components: same merged schedule, component-wise sweeps
         int rc = kinetic_sweep_mc(c, PH_HALF);
@@ -1259,7 +1490,7 @@ int sn_step_order4(sn_ctx *c, int64_t nsteps)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
@@ -1281,7 +1512,7 @@ int sn_debug_fft(sn_ctx *c, int direction)
 {
     if (!c) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (direction != 1 && direction != -1) return SN_ERR_PARAM;
     const Layout &l = c->lay;
@@ -1306,7 +1537,7 @@ int sn_debug_potential(sn_ctx *c, float *phi_out, int dst_on_device)
 {
     if (!c || !phi_out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     if (!dst_on_device && !c->phi) return SN_ERR_FEATURE; // a host destination is staged through the SN_FEAT_STAGING scratch
     int rc = potential_spectrum(c);
@@ -1327,7 +1558,7 @@ int sn_diagnostics(sn_ctx *c, sn_diag *out)
 {
     if (!c || !out) return SN_ERR_NULL;
     DeviceGuard guard(c->device);
-    if (c->is_mc) return SN_ERR_FEATURE; // coupled-component contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
+    if (c->is_mc || c->lay.R > 1) return SN_ERR_FEATURE; // coupled-component / slab contexts: sn_step, state copies, sn_mc_norms, sn_set_dtau
     if (!c->has_state) return SN_ERR_STATE;
     const Layout &l = c->lay;
     SN_CUDA(cudaMemsetAsync(c->diag, 0, 8 * sizeof(double), c->stream));

@@ -30,7 +30,9 @@ DISPATCH_DEFAULT, DISPATCH_FIRST_PATH, DISPATCH_PIPELINED = 0, 1, 2
 EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get_state", "sn_diagnostics",
            "sn_set_dtau", "sn_destroy", "sn_strerror", "sn_launch_count", "sn_profile", "sn_profile_read",
            "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm", "sn_workspace_bytes_opt",
-           "sn_create_opt", "sn_set_option", "sn_workspace_bytes_mc", "sn_create_mc", "sn_mc_norms")
+           "sn_create_opt", "sn_set_option", "sn_workspace_bytes_mc", "sn_create_mc", "sn_mc_norms",
+           "sn_slab_workspace_bytes", "sn_slab_create", "sn_slab_stage", "sn_slab_buffer", "sn_slab_pack",
+           "sn_slab_exchange_local", "sn_slab_local_norm")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG", "H_SRC", "H_BOHM", "H_R2C_MC", "H_NL_MC")
