@@ -97,7 +97,11 @@ struct SmemSub {
 };
 
 // Exchange accessor for ONE line (float2 per position) living in the first N/2 slots of a group's
-// column pair: position pos -> row q ^ ((q >> 2) & 7), q = pos >> 1, half (pos ^ (pos >> 6)) & 1.
+// column pair: position pos -> row q ^ ((q >> 2) & 7) ^ (4 if q bit 5), q = pos >> 1, half (pos ^ (pos >> 6)) & 1.
+// A 64-bit access is served per half-warp, so 16 lanes must land on 16 different 8-byte bank pairs: position bit 6
+// (lane bit 3 in the stores after the NS = 8 stage) has to reach the row bits as well as the half bit -- without the
+// "^ 4" term those stores were 2-way conflicted (ncu source page, profiles/r02g: 8 STS.64 per transform at twice
+// their ideal wavefronts, 10 % of the r2c kernel's shared-memory wavefronts).
 template <int T, int CPW>
 struct SmemSubOne {
     float2 *sub2; // the sub-tile as float2
@@ -105,7 +109,7 @@ struct SmemSubOne {
     static constexpr int TMASK = (CPW - 1) << 1;
     __host__ __device__ static constexpr int lin(int pos)
     {
-        const int q = pos >> 1, r = q ^ ((q >> 2) & 7);
+        const int q = pos >> 1, r = q ^ ((q >> 2) & 7) ^ (((q >> 5) & 1) << 2);
         return (((r * CPW) | swz<CPW>(r)) << 1) | ((pos ^ (pos >> 6)) & 1);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ (t << 1); }
