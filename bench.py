@@ -179,6 +179,43 @@ def run_reference(args, inputs):
         "gpu_launches": 0}))
 
 
+def run_slab(args, cfg, psi0, dev, barrier):
+    """--slab R: the decomposed step on one GPU (R contexts, one stream); one JSON line, no per-pass roofline."""
+    import torch
+    from paper_1909_08354_b200 import slab
+    R, K = args.slab, args.steps
+    grp = slab.LocalSlabGroup(cfg.dims, cfg.L, cfg.A, cfg.B, cfg.C, cfg.D, cfg.g, cfg.dtau, R, device=dev)
+    grp.set_state(psi0)
+    n0 = grp.norm()
+    grp.step(args.warmup)
+    stream = torch.cuda.current_stream()
+    reps = []
+    for r in range(args.repeats):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        l0, x0 = grp.launch_count(), grp.exchanged_elems
+        barrier()
+        e0.record(stream)
+        grp.step(K)
+        e1.record(stream)
+        barrier()
+        launches, moved = grp.launch_count() - l0, (grp.exchanged_elems - x0) * 8
+        reps.append(e0.elapsed_time(e1))
+    n1 = grp.norm()
+    grp.close()
+    ms = statistics.median(reps)
+    print(json.dumps({
+        "metric": METRIC, "value": cfg.cells * K / (ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms / K, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+        "dtype": "complex64 (f32 arithmetic)", "data": "synthetic",
+        "config": {"workload": f"{cfg.name}: {'x'.join(map(str, cfg.dims))}", "dims": list(cfg.dims),
+                   "parallelism": f"slab decomposition, {R} virtual ranks on ONE GPU (sn_slab_exchange_local: device-to-device "
+                                  f"block copies stand in for the all-to-all; not a multi-GPU measurement)"},
+        "gpu_launches": launches, "exchange_bytes_per_step": moved / K,
+        "exchange_bytes_per_cell_update": moved / K / cfg.cells,
+        "repeats": {"n": len(reps), "ms_per_step_min": min(reps) / K, "ms_per_step_max": max(reps) / K},
+        "checks": {"norm_before": n0, "norm_after": n1}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -202,6 +239,9 @@ def main():
     ap.add_argument("--dtype", default="c64", choices=["c64", "c128"],
                     help="c64: complex64 (BASELINE.json's metric); c128: the complex128 path (SURVEY.md 8(f) item 3, the "
                          "precision the paper benchmarked): same step, 16 B per cell of state, float64 arithmetic")
+    ap.add_argument("--slab", type=int, default=0,
+                    help="time the slab-decomposed step (NEXT-2, DESIGN.md section 7) as this many virtual ranks on ONE GPU: "
+                         "the local passes of every rank plus the all-to-all exchanges done as device-to-device copies")
     ap.add_argument("--repeats", type=int, default=5,
                     help="timed repetitions of the K-step call (SURVEY.md 8(d): median of >= 5); value = median")
     args = ap.parse_args()
@@ -272,6 +312,10 @@ def main():
     host_in = torch.from_numpy(psi0).pin_memory()
     host_out = torch.empty_like(host_in).pin_memory()
     dev_in = host_in.to(dev, non_blocking=True)
+
+    if args.slab:
+        run_slab(args, cfg, psi0, dev, barrier)
+        return
 
     stream = torch.cuda.current_stream()
     sim = sn.Simulation.from_config(cfg, device=dev, stream=stream, batch=args.batch or None,

@@ -52,15 +52,24 @@ __device__ __forceinline__ void block_accumulate(double (&v)[NV], double *out)
     }
 }
 
-// columns per CTA tile of the strided kernels: 128-byte rows up to N = 512, then as many as 512 threads carry
-__host__ __device__ constexpr int cpd_for(int N) { return N <= 512 ? 8 : (N <= 1024 ? 4 : (N <= 2048 ? 2 : 1)); }
+// columns per CTA tile of the strided kernels: 256-thread CTAs (two or three resident per SM: the loads of one overlap
+// the butterflies of another -- with one 512-thread CTA per SM the 512^3 passes ran at 22-34 % of DRAM throughput,
+// profiles/r02g) with rows of 128 bytes up to N = 256, 64 bytes at 512, 32 bytes (one sector) at 1024 and 2048
+#ifndef SN_F64_CP512
+#define SN_F64_CP512 4
+#endif
+__host__ __device__ constexpr int cpd_for(int N)
+{
+    return N <= 384 ? 8 : (N <= 768 ? SN_F64_CP512 : (N <= 2048 ? 2 : 1));
+}
 __host__ __device__ constexpr int sthreads(int N) { return cpd_for(N) * (N / ppt_for(N)); }
+__host__ __device__ constexpr int sblocks(int N) { return sthreads(N) <= 256 ? 2 : 1; }
 
 // ---------------------------------------------------------------------------- strided axis
 // Tile: N rows (points of the line, row_stride elements apart) x CP adjacent columns; thread (t, j): column t,
 // points j + T*m.  8 adjacent lanes read/write one 128-byte row segment.
 template <int N, int CP, int MODE, int DIR>
-__global__ void __launch_bounds__(sthreads(N)) kd_strided(const PassArgsD p)
+__global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_strided(const PassArgsD p)
 {
     extern __shared__ double2 smem_d[];
     constexpr int P = ppt_for(N), T = N / P;
@@ -104,7 +113,7 @@ __global__ void __launch_bounds__(sthreads(N)) kd_strided(const PassArgsD p)
 // the factor 1/2 is folded into the Poisson multiplier (PassArgsD::pscale).  The half spectrum stores X[k] in column
 // 2t and Y[k] in column 2t+1 of row k.
 template <int N, int CP, int MODE>
-__global__ void __launch_bounds__(sthreads(N)) kd_haxis(const PassArgsD p)
+__global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassArgsD p)
 {
     extern __shared__ double2 smem_d[];
     constexpr int P = ppt_for(N), T = N / P;

@@ -134,11 +134,13 @@ class Simulation:
 
     def __init__(self, dims: Sequence[int], L, A: float, B: float, C: float, D: float, g: Sequence[float],
                  dtau: float, device: str = "cuda:0", stream=None, batch: Optional[int] = None, features: int = 0,
-                 dtype: str = "complex64"):
+                 dtype: str = "complex64", workspace=None):
         """batch=None: one 2D/3D system of shape dims.  batch=B: an ensemble of B systems; every array then has the
         STORAGE shape (dims[0], B, dims[1][, dims[2]]) (member b at [:, b, ...]).  features: FEAT_* bits, the optional
         workspace regions (external potential table, source tables, host staging); 0 = the stepper alone, ~12 B/cell.
-        dtype: "complex64" (default) or "complex128" -- the precision of the state and of all arithmetic."""
+        dtype: "complex64" (default) or "complex128" -- the precision of the state and of all arithmetic.
+        workspace: a caller-owned, 256-byte aligned torch uint8 CUDA tensor of at least workspace_bytes(...) bytes to
+        use instead of allocating one (the tests hand in the middle of a larger, poisoned buffer)."""
         import torch
 
         if not torch.cuda.is_available():
@@ -158,7 +160,7 @@ class Simulation:
         if nbytes == 0:
             raise SnError(-2, "sn_workspace_bytes_opt", lib().sn_strerror(-2).decode())
         with torch.cuda.device(self.device):
-            self._ws = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+            self._ws = workspace if workspace is not None else torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self._h = ctypes.c_void_p()
         c_L = (ctypes.c_double * nd)(*Ls)
