@@ -346,8 +346,15 @@ __device__ __forceinline__ void fft_single(float2 (&a)[P], int j, const float4 *
 // Multiplications by -i / +i are register renames plus sign flips that fold into operand modifiers.
 // Rounding is identical to the scalar engine (same operations in the same order, lane by lane).
 #ifndef SN_PACKED
-#define SN_PACKED 1
+#define SN_PACKED 1 // 0: scalar engine everywhere (A/B builds)
 #endif
+#ifndef SN_PACKED_3
+// packed engine for the 3*2^a lengths too?  No: measured at 384^3 (12 points per thread, radix-4/6 stages, ~195
+// registers) the packed form is SLOWER -- pipelined H_NLKIN 0.611 -> 0.877 ms, first-path S_KIN 0.314 -> 0.345 ms
+// (the 64-bit register pairs cost that kernel the freedom it needs at its register budget); profiles/r02o.
+#define SN_PACKED_3 0
+#endif
+__host__ __device__ constexpr bool packed_for(int N) { return SN_PACKED && (N % 3 != 0 || SN_PACKED_3); }
 
 struct cp2 {
     float2 r, i;
@@ -541,29 +548,41 @@ template <int N, int DIR, bool HILO, class SM, int P>
 __device__ __forceinline__ void fft_pair(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
     static_assert(P == ppt_for(N), "points per thread");
-    constexpr int R = radix_for(N, 1);
-    const float4 none[(P / R) * (R - 1)] = {};
-    stage_compute<N, R, 1, DIR, HILO>(x, none);
-    if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, SM>(x, j, tw, sm);
+    if constexpr (packed_for(N)) {
+        constexpr int R = radix_for(N, 1);
+        const float4 none[(P / R) * (R - 1)] = {};
+        stage_compute<N, R, 1, DIR, HILO>(x, none);
+        if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, SM>(x, j, tw, sm);
+    } else { // scalar engine on the same registers (the repacking is register naming)
+        float2 a[P], b[P];
+#pragma unroll
+        for (int m = 0; m < P; m++) {
+            a[m] = line_a(x[m]);
+            b[m] = line_b(x[m]);
+        }
+        fft_pair_scalar<N, DIR, HILO>(a, b, j, tw, sm);
+#pragma unroll
+        for (int m = 0; m < P; m++) x[m] = pack_pair(a[m], b[m]);
+    }
 }
 
 // Line pair given as two complex arrays: through the packed engine (the repacking is register naming).
 template <int N, int DIR, bool HILO, class SM, int P>
 __device__ __forceinline__ void fft_pair(float2 (&a)[P], float2 (&b)[P], int j, const float4 *__restrict__ tw, SM &sm)
 {
-#if SN_PACKED
-    cp2 x[P];
+    if constexpr (packed_for(N)) {
+        cp2 x[P];
 #pragma unroll
-    for (int m = 0; m < P; m++) x[m] = pack_pair(a[m], b[m]);
-    fft_pair<N, DIR, HILO>(x, j, tw, sm);
+        for (int m = 0; m < P; m++) x[m] = pack_pair(a[m], b[m]);
+        fft_pair<N, DIR, HILO>(x, j, tw, sm);
 #pragma unroll
-    for (int m = 0; m < P; m++) {
-        a[m] = line_a(x[m]);
-        b[m] = line_b(x[m]);
+        for (int m = 0; m < P; m++) {
+            a[m] = line_a(x[m]);
+            b[m] = line_b(x[m]);
+        }
+    } else {
+        fft_pair_scalar<N, DIR, HILO>(a, b, j, tw, sm);
     }
-#else
-    fft_pair_scalar<N, DIR, HILO>(a, b, j, tw, sm);
-#endif
 }
 
 // ---- shared-memory accessors -------------------------------------------------------------

@@ -109,7 +109,10 @@ struct SmemSubOne {
     static constexpr int TMASK = (CPW - 1) << 1;
     __host__ __device__ static constexpr int lin(int pos)
     {
-        const int q = pos >> 1, r = q ^ ((q >> 2) & 7) ^ (((q >> 5) & 1) << 2);
+#ifndef SN_SUBONE_BIT6
+#define SN_SUBONE_BIT6 1
+#endif
+        const int q = pos >> 1, r = q ^ ((q >> 2) & 7) ^ (SN_SUBONE_BIT6 ? ((q >> 5) & 1) << 2 : 0);
         return (((r * CPW) | swz<CPW>(r)) << 1) | ((pos ^ (pos >> 6)) & 1);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ (t << 1); }
