@@ -529,30 +529,73 @@ __device__ __forceinline__ void exchange_load(cp2 (&x)[P], int j, SM &sm)
     for (int m = 0; m < P; m++) sm.ld_i(comb<SM>(tbr, T * m, T - 1), x[m].r, x[m].i);
 }
 
+// ---- resident last-stage twiddles ----
+// The twiddles of the LAST stage depend on the thread (kp = (j + T q) mod NS) but not on the tile, and the forward and
+// the inverse transform use the same values (conjugated).  A persistent pass kernel can load them once per CTA
+// lifetime and keep them in registers (7 float4 at N = 512): per 64 KB tile and warp that removes 2 x 7 warp-wide
+// 128-bit loads = 56 of the ~420 L1 wavefronts of a kinetic pass -- and L1/shared-memory wavefronts are what bounds
+// these kernels.
+__host__ __device__ constexpr int last_stage_ns(int N)
+{
+    int ns = 1;
+    while (ns * radix_for(N, ns) < N) ns *= radix_for(N, ns);
+    return ns;
+}
+__host__ __device__ constexpr int last_stage_off(int N)
+{
+    int ns = 1, off = 0;
+    while (ns * radix_for(N, ns) < N) {
+        if (ns > 1) off += ns * (radix_for(N, ns) - 1);
+        ns *= radix_for(N, ns);
+    }
+    return off;
+}
+template <int N>
+struct LastTw {
+    static constexpr int P = ppt_for(N), NS = last_stage_ns(N), R = radix_for(N, NS), OFF = last_stage_off(N);
+    static constexpr int COUNT = (P / R) * (R - 1);
+    float4 w[COUNT];
+    template <bool HILO>
+    __device__ __forceinline__ void load(int j, const float4 *__restrict__ tw)
+    {
+        load_twiddles<N, R, NS, OFF, HILO, P>(w, j, tw);
+    }
+};
+
 template <int N, int NSP, int RP, int OFF, int DIR, bool HILO, class SM, int P>
-__device__ __forceinline__ void fft_next(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm)
+__device__ __forceinline__ void fft_next(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm,
+                                         const LastTw<N> *res = nullptr)
 {
     constexpr int NS = NSP * RP, R = radix_for(N, NS);
     constexpr bool H = stage_hilo<HILO, NS>();
+    if constexpr (NS * R == N) {
+        if (res != nullptr) { // last stage with resident twiddles (res is a compile-time-known pointer after inlining)
+            exchange_store<N, RP, NSP>(x, j, sm);
+            exchange_load<N>(x, j, sm);
+            stage_compute<N, R, NS, DIR, H>(x, res->w);
+            return;
+        }
+    }
     float4 w[(P / R) * (R - 1)];
     exchange_store<N, RP, NSP>(x, j, sm);
     if (SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
     exchange_load<N>(x, j, sm);
     if (!SN_TW_PREFETCH) load_twiddles<N, R, NS, OFF, H, P>(w, j, tw);
     stage_compute<N, R, NS, DIR, H>(x, w);
-    if constexpr (NS * R < N) fft_next<N, NS, R, OFF + NS * (R - 1), DIR, HILO, SM>(x, j, tw, sm);
+    if constexpr (NS * R < N) fft_next<N, NS, R, OFF + NS * (R - 1), DIR, HILO, SM>(x, j, tw, sm, res);
 }
 
 // Unscaled DFT of a packed line pair; same contract as fft_pair.
 template <int N, int DIR, bool HILO, class SM, int P>
-__device__ __forceinline__ void fft_pair(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm)
+__device__ __forceinline__ void fft_pair(cp2 (&x)[P], int j, const float4 *__restrict__ tw, SM &sm,
+                                         const LastTw<N> *res = nullptr)
 {
     static_assert(P == ppt_for(N), "points per thread");
     if constexpr (packed_for(N)) {
         constexpr int R = radix_for(N, 1);
         const float4 none[(P / R) * (R - 1)] = {};
         stage_compute<N, R, 1, DIR, HILO>(x, none);
-        if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, SM>(x, j, tw, sm);
+        if constexpr (R < N) fft_next<N, 1, R, 0, DIR, HILO, SM>(x, j, tw, sm, res);
     } else { // scalar engine on the same registers (the repacking is register naming)
         float2 a[P], b[P];
 #pragma unroll

@@ -32,6 +32,11 @@
 
 namespace snk {
 
+// keep the last stage's hi/lo twiddles of the psi transforms in registers across tiles (sn_fft_core.cuh, LastTw)?
+#ifndef SN_RES_TW
+#define SN_RES_TW 1
+#endif
+__host__ __device__ constexpr bool res_tw_for(int N) { return SN_RES_TW && packed_for(N) && N == 512; }
 
 template <int N>
 struct Geo {
@@ -156,6 +161,18 @@ __device__ __forceinline__ void apply_phase(cp2 (&x)[P], int j, const float4 *__
     for (int m = 0; m < P; m++) x[m] = twmul<+1, true>(x[m], __ldg(phase + j + T * m));
 }
 
+// the same with the first NR of the thread's P phase values already in registers (they do not depend on the tile
+// either; all P of them would not fit the 128-register budget: measured, 92 bytes of spills)
+#ifndef SN_RES_PH
+#define SN_RES_PH 0
+#endif
+template <int T, int P, int NR>
+__device__ __forceinline__ void apply_phase(cp2 (&x)[P], int j, const float4 *__restrict__ phase, const float4 (&ph)[NR])
+{
+#pragma unroll
+    for (int m = 0; m < P; m++) x[m] = twmul<+1, true>(x[m], m < NR ? ph[m] : __ldg(phase + j + T * m));
+}
+
 // ---------------------------------------------------------------------------- strided axis
 // P_S_KIN: forward -> kinetic phase -> inverse along a strided axis; P_S_FFT: plain transform.
 // 3-stage ring.  Thread 0 is the issuer: at the end of tile k it waits until every warp has
@@ -202,6 +219,15 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
         if (nk > 0) issue_load(0);
         if (nk > 1) issue_load(1);
     }
+    LastTw<N> wres;
+    constexpr bool RES = MODE == P_S_KIN && res_tw_for(N);
+    if (RES) wres.template load<true>(j, p.a.tw);
+    const LastTw<N> *res = RES ? &wres : nullptr;
+    float4 phres[SN_RES_PH > 0 ? SN_RES_PH : 1];
+    if (RES && SN_RES_PH) {
+#pragma unroll
+        for (int m = 0; m < SN_RES_PH; m++) phres[m] = __ldg(p.a.phase + j + T * m);
+    }
 
     for (int k = 0; k < nk; k++) {
         const int b = k % NST;
@@ -223,9 +249,10 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
                 for (int m = 0; m < P; m++) x[m] = cscale(x[m], sc);
             }
         } else { // P_S_KIN
-            fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
-            apply_phase<T, P>(x, jf, p.a.phase);
-            fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
+            fft_pair<N, +1, true>(x, jf, p.a.tw, sm, res);
+            if (RES && SN_RES_PH) apply_phase<T, P>(x, jf, p.a.phase, phres);
+            else apply_phase<T, P>(x, jf, p.a.phase);
+            fft_pair<N, -1, true>(x, ji, p.a.tw, sm, res);
         }
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
         __syncwarp();
@@ -326,6 +353,10 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
         issue_load(0);
         if (more) issue_load(1);
     }
+    LastTw<N> wres; // the last stage's hi/lo twiddles of the psi transforms stay in registers across tiles
+    constexpr bool RES = MODE == P_H_NLKIN && res_tw_for(N);
+    if (RES) wres.template load<true>(j, p.a.tw);
+    const LastTw<N> *res = RES ? &wres : nullptr;
 
     for (int k = 0;; k++) {
         const int b = k % NST;
@@ -375,9 +406,9 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
                     const float4 v = mine[CPW * T * m];
                     x[m] = pack_pair(nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl), nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl));
                 }
-                fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
+                fft_pair<N, +1, true>(x, jf, p.a.tw, sm, res);
                 apply_phase<T, P>(x, jf, p.a.phase);
-                fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
+                fft_pair<N, -1, true>(x, ji, p.a.tw, sm, res);
                 __syncwarp();
 #pragma unroll
                 for (int m = 0; m < P; m++) mine[CPW * T * m] = pack4(x[m]);
@@ -716,6 +747,10 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
         if (nk > 0) issue_load(0);
         if (nk > 1) issue_load(1);
     }
+    LastTw<N> wres; // the last stage's twiddles stay in registers across tiles (sn_fft_core.cuh)
+    constexpr bool RES = res_tw_for(N);
+    if (RES) wres.template load<MODE == P_X_KIN>(j, p.a.tw);
+    const LastTw<N> *res = RES ? &wres : nullptr;
 
     for (int k = 0; k < nk; k++) {
         const int b = k % NST;
@@ -733,13 +768,13 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
 #pragma unroll
             for (int m = 0; m < P; m++) x[m] = pack_pair(la[jf + T * m], lb[jf + T * m]);
             if (MODE == P_X_KIN) {
-                fft_pair<N, +1, true>(x, jf, p.a.tw, sm);
+                fft_pair<N, +1, true>(x, jf, p.a.tw, sm, res);
                 if (NST == 2 && tid == 0 && k >= 1 && k + 1 < nk) { // reload the stage tile k-1 was stored from
                     bulk_wait_read<0>();
                     issue_load(k + 1);
                 }
                 apply_phase<T, P>(x, jf, p.a.phase);
-                fft_pair<N, -1, true>(x, ji, p.a.tw, sm);
+                fft_pair<N, -1, true>(x, ji, p.a.tw, sm, res);
                 if (VEXT) {
                     const float *va = reinterpret_cast<const float *>(base + b * STAGE_BYTES + TILE_BYTES) + 2 * g * N;
 #pragma unroll
@@ -748,14 +783,14 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_contig(const __grid
                                          rotate_half_angle(line_b(x[m]), p.a.nl.hv * va[N + ji + T * m]));
                 }
             } else { // P_X_POISSON
-                fft_pair<N, +1, false>(x, jf, p.a.tw, sm);
+                fft_pair<N, +1, false>(x, jf, p.a.tw, sm, res);
                 const float2 ka = __ldg(p.a.dko + line0 + 2 * g), kb = __ldg(p.a.dko + line0 + 2 * g + 1);
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 kx = __ldg(p.a.ksq2 + jf + T * m);
                     x[m] = cscale(x[m], helmholtz_mult(ka, kx, p.a.pscale, p.a.lap), helmholtz_mult(kb, kx, p.a.pscale, p.a.lap));
                 }
-                fft_pair<N, -1, false>(x, ji, p.a.tw, sm);
+                fft_pair<N, -1, false>(x, ji, p.a.tw, sm, res);
             }
             sm.sync(); // exchange layout (float4 per position) != line layout: whole group must be done reading
 #pragma unroll
