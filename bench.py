@@ -239,6 +239,8 @@ def main():
     ap.add_argument("--dtype", default="c64", choices=["c64", "c128"],
                     help="c64: complex64 (BASELINE.json's metric); c128: the complex128 path (SURVEY.md 8(f) item 3, the "
                          "precision the paper benchmarked): same step, 16 B per cell of state, float64 arithmetic")
+    ap.add_argument("--dispatch", type=int, default=0, choices=[0, 1, 2],
+                    help="sn_set_option(SN_OPT_DISPATCH): 0 default, 1 first-path kernels only, 2 pipelined wherever instantiated")
     ap.add_argument("--slab", type=int, default=0,
                     help="time the slab-decomposed step (NEXT-2, DESIGN.md section 7) as this many virtual ranks on ONE GPU: "
                          "the local passes of every rank plus the all-to-all exchanges done as device-to-device copies")
@@ -335,6 +337,8 @@ def main():
         if args.bohm:
             sim.set_bohm(args.bohm, 1e-4)               # eq. (15): + nu^2 V_B
         del rs, f, r2
+    if args.dispatch:
+        sim.set_option(sn.OPT_DISPATCH, args.dispatch)
     step = sim.step_order4 if args.order4 else sim.step
     sim.set_state(dev_in)
     step(W)                                             # untimed warm-up steps

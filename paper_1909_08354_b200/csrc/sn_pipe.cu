@@ -221,8 +221,8 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
         if (nk > 1) issue_load(1);
     }
     LastTw<N> wres;
-    constexpr bool RES = MODE == P_S_KIN && res_tw_for(N);
-    if (RES) wres.template load<true>(j, p.a.tw);
+    constexpr bool RES = res_tw_for(N);
+    if (RES) wres.template load<MODE == P_S_KIN || HILO>(j, p.a.tw);
     const LastTw<N> *res = RES ? &wres : nullptr;
     float4 phres[SN_RES_PH > 0 ? SN_RES_PH : 1];
     if (RES && SN_RES_PH) {
@@ -243,7 +243,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
 #pragma unroll
         for (int m = 0; m < P; m++) x[m] = unpack4(mine[CPW * T * m]);
         if (MODE == P_S_FFT) {
-            fft_pair<N, DIR, HILO>(x, jf, p.a.tw, sm);
+            fft_pair<N, DIR, HILO>(x, jf, p.a.tw, sm, res);
             if (DIR < 0) {
                 const float sc = p.a.scale;
 #pragma unroll
