@@ -51,9 +51,10 @@ PASS_BYTES_PER_CELL = {
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
 B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update
-# ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, C5_512, from profiles/r01c_ncu_full_C5_512.md
-NCU_TRAFFIC_C5_512 = {"H_NLKIN": 2.633e9, "S_KIN": 2.089e9, "X_KIN": 2.088e9, "H_R2C": 1.577e9, "S_FFT": 1.019e9,
-                      "X_POISSON": 1.019e9}
+# ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, C5_512, from profiles/r02g_ncu_full_C5_512.md
+# (capture of commit 163e14c "NEXT-4b on the GPU"; later commits changed twiddle loads and shared-memory layout, not DRAM traffic)
+NCU_TRAFFIC_C5_512 = {"H_NLKIN": 2.633e9, "S_KIN": 2.088e9, "X_KIN": 2.088e9, "H_R2C": 1.577e9, "S_FFT": 1.019e9,
+                      "X_POISSON": 1.022e9}
 
 
 def load_peaks():
@@ -430,7 +431,7 @@ def main():
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras and not f64 and not args.batch else None,
-                "traffic_source": "ncu --set full dram bytes per launch, profiles/r01c_ncu_full_C5_512.md (re-captured at round end, same values: r01g)",
+                "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r02g_ncu_full_C5_512.md",
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
                 "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot,

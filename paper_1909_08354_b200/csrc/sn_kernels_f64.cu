@@ -106,12 +106,17 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_strided(const Pass
 }
 
 // ---------------------------------------------------------------------------- axis 0 ("h") kernels
-// Tile: N rows x 2*CP columns; thread (t, j) owns columns 2t, 2t+1.  The two REAL columns of rho / phi travel as
-// one complex line z = x + i y (two-for-one trick):
+// Tile: N rows x 2*CP columns; thread (t, j) owns two columns of the tile, S apart.  The two REAL columns of rho / phi
+// travel as one complex line z = x + i y (two-for-one trick).  Which two columns are paired is free per kernel -- once
+// untangled, column c of the half spectrum holds the spectrum of real column c -- so each mode picks the pairing that
+// gives whole 32-byte sectors: the modes that read both psi columns at once (R2C, DIAG, POT) pair 2t with 2t+1 (S = 1,
+// 32 contiguous bytes per thread); NLKIN, which transforms one psi column after the other, pairs t with CP + t (S = CP:
+// the CP lanes of a row read CP adjacent 16-byte values in each column pass).  Measured at 512^3: NLKIN 2.68 -> 2.49 ms
+// with S = CP, R2C 0.73 -> 1.02 ms if it used S = CP too.
 //   X[k] = (Z[k] + conj Z[N-k])/2,  Y[k] = (Z[k] - conj Z[N-k])/(2i),  k = 0..N/2;
 //   inverse: Z[k] = X[k] + i Y[k] (k <= N/2), Z[N-k] = conj X[k] + i conj Y[k];
 // the factor 1/2 is folded into the Poisson multiplier (PassArgsD::pscale).  The half spectrum stores X[k] in column
-// 2t and Y[k] in column 2t+1 of row k.
+// of the first and Y[k] in the column of the second real column, row k.
 template <int N, int CP, int MODE>
 __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassArgsD p)
 {
@@ -119,7 +124,8 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
     constexpr int P = ppt_for(N), T = N / P;
     const int t = threadIdx.x % CP, j = threadIdx.x / CP;
     const long long rs = p.row_stride;
-    const long long col = (long long)blockIdx.x * 2 * CP + 2 * t;
+    constexpr int S = MODE == P_H_NLKIN ? CP : 1;              // distance between the thread's two columns
+    const long long col = (long long)blockIdx.x * 2 * CP + (S == 1 ? 2 * t : t);
     cd *psi = p.data + col;
     cd *hs = p.hs + col;
     SmemTileD<CP> sm{smem_d, t};
@@ -129,7 +135,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
 #pragma unroll
         for (int m = 0; m < P; m++) {
             const long long row = (long long)(j + T * m) * rs;
-            z[m] = make_double2(abs2(psi[row]), abs2(psi[row + 1]));
+            z[m] = make_double2(abs2(psi[row]), abs2(psi[row + S]));
         }
         fft_line<N, +1>(z, j, p.tw, sm);
         sm.sync();
@@ -142,7 +148,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
                 const int k = j + T * m;
                 const cd y = sm.ld((N - k) % N);
                 hs[(long long)k * rs] = make_double2(z[m].x + y.x, z[m].y - y.y);
-                hs[(long long)k * rs + 1] = make_double2(z[m].y + y.y, y.x - z[m].x);
+                hs[(long long)k * rs + S] = make_double2(z[m].y + y.y, y.x - z[m].x);
             }
         }
         return;
@@ -153,7 +159,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
     for (int m = 0; m < P; m++) {
         const int km = j + T * m;
         const int src = m < P / 2 ? km : N - km; // m >= P/2: km >= N/2, mirrored row in [0, N/2]
-        const cd u = hs[(long long)src * rs], v = hs[(long long)src * rs + 1];
+        const cd u = hs[(long long)src * rs], v = hs[(long long)src * rs + S];
         z[m] = m < P / 2 ? make_double2(u.x - v.y, u.y + v.x) : make_double2(u.x + v.y, v.x - u.y);
     }
     fft_line<N, -1>(z, j, p.tw, sm);
@@ -161,8 +167,10 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
     if (MODE == P_H_POT) {
         double *out = p.phi_out + col;
 #pragma unroll
-        for (int m = 0; m < P; m++)
-            *reinterpret_cast<double2 *>(out + (long long)(j + T * m) * rs) = z[m];
+        for (int m = 0; m < P; m++) {
+            out[(long long)(j + T * m) * rs] = z[m].x;
+            out[(long long)(j + T * m) * rs + S] = z[m].y;
+        }
         return;
     }
     if (MODE == P_H_DIAG) {
@@ -170,7 +178,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
 #pragma unroll
         for (int m = 0; m < P; m++) {
             const long long row = (long long)(j + T * m) * rs;
-            const double r[2] = {abs2(psi[row]), abs2(psi[row + 1])};
+            const double r[2] = {abs2(psi[row]), abs2(psi[row + S])};
             const double ph[2] = {z[m].x, z[m].y};
 #pragma unroll
             for (int c = 0; c < 2; c++) {
@@ -191,13 +199,13 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassAr
         cd x[P];
 #pragma unroll
         for (int m = 0; m < P; m++)
-            x[m] = nl_phase(psi[(long long)(j + T * m) * rs + c], c == 0 ? z[m].x : z[m].y, p.nl);
+            x[m] = nl_phase(psi[(long long)(j + T * m) * rs + c * S], c == 0 ? z[m].x : z[m].y, p.nl);
         fft_line<N, +1>(x, j, p.tw, sm);
 #pragma unroll
         for (int m = 0; m < P; m++) x[m] = cmul<+1>(x[m], __ldg(p.phase + j + T * m));
         fft_line<N, -1>(x, j, p.tw, sm);
 #pragma unroll
-        for (int m = 0; m < P; m++) psi[(long long)(j + T * m) * rs + c] = x[m];
+        for (int m = 0; m < P; m++) psi[(long long)(j + T * m) * rs + c * S] = x[m];
     }
 }
 
