@@ -162,18 +162,6 @@ __device__ __forceinline__ void apply_phase(cp2 (&x)[P], int j, const float4 *__
     for (int m = 0; m < P; m++) x[m] = twmul<+1, true>(x[m], __ldg(phase + j + T * m));
 }
 
-// the same with the first NR of the thread's P phase values already in registers (they do not depend on the tile
-// either; all P of them would not fit the 128-register budget: measured, 92 bytes of spills)
-#ifndef SN_RES_PH
-#define SN_RES_PH 0
-#endif
-template <int T, int P, int NR>
-__device__ __forceinline__ void apply_phase(cp2 (&x)[P], int j, const float4 *__restrict__ phase, const float4 (&ph)[NR])
-{
-#pragma unroll
-    for (int m = 0; m < P; m++) x[m] = twmul<+1, true>(x[m], m < NR ? ph[m] : __ldg(phase + j + T * m));
-}
-
 // ---------------------------------------------------------------------------- strided axis
 // P_S_KIN: forward -> kinetic phase -> inverse along a strided axis; P_S_FFT: plain transform.
 // 3-stage ring.  Thread 0 is the issuer: at the end of tile k it waits until every warp has
@@ -224,11 +212,6 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
     constexpr bool RES = res_tw_for(N);
     if (RES) wres.template load<MODE == P_S_KIN || HILO>(j, p.a.tw);
     const LastTw<N> *res = RES ? &wres : nullptr;
-    float4 phres[SN_RES_PH > 0 ? SN_RES_PH : 1];
-    if (RES && SN_RES_PH) {
-#pragma unroll
-        for (int m = 0; m < SN_RES_PH; m++) phres[m] = __ldg(p.a.phase + j + T * m);
-    }
 
     for (int k = 0; k < nk; k++) {
         const int b = k % NST;
@@ -251,8 +234,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_strided(const __gri
             }
         } else { // P_S_KIN
             fft_pair<N, +1, true>(x, jf, p.a.tw, sm, res);
-            if (RES && SN_RES_PH) apply_phase<T, P>(x, jf, p.a.phase, phres);
-            else apply_phase<T, P>(x, jf, p.a.phase);
+            apply_phase<T, P>(x, jf, p.a.phase);
             fft_pair<N, -1, true>(x, ji, p.a.tw, sm, res);
         }
         // the last exchange's reads and these writes can only collide inside an aligned group of 8 lanes
@@ -404,8 +386,7 @@ __global__ void __launch_bounds__(pipe_threads(N), 1) k_pipe_haxis(const __grid_
                 cp2 x[P];
 #pragma unroll
                 for (int m = 0; m < P; m++) {
-                    const float4 v = mine[CPW * T * m];
-                    x[m] = pack_pair(nl_phase<EXTRA>(lo2(v), z[m].x, p.a.nl), nl_phase<EXTRA>(hi2(v), z[m].y, p.a.nl));
+                    nl_phase_pair<EXTRA>(mine[CPW * T * m], z[m], p.a.nl, x[m].r, x[m].i);
                 }
                 fft_pair<N, +1, true>(x, jf, p.a.tw, sm, res);
                 apply_phase<T, P>(x, jf, p.a.phase);
