@@ -36,8 +36,11 @@ namespace snk {
 #ifndef SN_RES_TW
 #define SN_RES_TW 1
 #endif
+#ifndef SN_RES_TW_ALL
+#define SN_RES_TW_ALL 0
+#endif
 // (N <= 512: at 1024 and above the extra live registers spill, measured with -Xptxas -v)
-__host__ __device__ constexpr bool res_tw_for(int N) { return SN_RES_TW && packed_for(N) && N <= 512; }
+__host__ __device__ constexpr bool res_tw_for(int N) { return SN_RES_TW && packed_for(N) && (N <= 512 || SN_RES_TW_ALL); }
 
 template <int N>
 struct Geo {

@@ -203,7 +203,8 @@ class DistributedSlab:
     def norm(self) -> float:
         import torch
         import torch.distributed as dist
-        t = torch.tensor([self.ctx.local_norm()], dtype=torch.float64, device=self.ctx.device)
+        on_gpu = dist.get_backend(self.group) != "gloo"
+        t = torch.tensor([self.ctx.local_norm()], dtype=torch.float64, device=self.ctx.device if on_gpu else "cpu")
         dist.all_reduce(t, group=self.group)
         return float(t[0])
 
@@ -219,9 +220,19 @@ def all_to_all(staging, b_buf, dims, nranks, rank, what, to_a, pack, group=None)
     if staging.is_complex():                            # move (re, im) pairs as floats: every backend takes those
         staging, b_buf = torch.view_as_real(staging).reshape(-1), torch.view_as_real(b_buf).reshape(-1)
         a_split, b_split, na, nb = [2 * v for v in a_split], [2 * v for v in b_split], 2 * na, 2 * nb
+    def a2a(out, inp, out_split, in_split):
+        if inp.is_cuda and dist.get_backend(group) == "gloo":
+            # gloo moves host memory: stage through the CPU (the single-GPU validation of this driver runs two rank
+            # processes on one device this way; nccl takes the device buffers directly)
+            host_out = torch.empty(out.shape, dtype=out.dtype)
+            dist.all_to_all_single(host_out, inp.cpu(), output_split_sizes=out_split, input_split_sizes=in_split, group=group)
+            out.copy_(host_out)
+        else:
+            dist.all_to_all_single(out, inp, output_split_sizes=out_split, input_split_sizes=in_split, group=group)
+
     if to_a:                                            # view B -> view A
-        dist.all_to_all_single(staging[:na], b_buf[:nb], output_split_sizes=a_split, input_split_sizes=b_split, group=group)
+        a2a(staging[:na], b_buf[:nb], a_split, b_split)
         pack(True)
     else:                                               # view A -> view B
         pack(False)
-        dist.all_to_all_single(b_buf[:nb], staging[:na], output_split_sizes=b_split, input_split_sizes=a_split, group=group)
+        a2a(b_buf[:nb], staging[:na], b_split, a_split)

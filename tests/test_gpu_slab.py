@@ -79,3 +79,72 @@ def test_slab_contract(mods):
     assert r.buffer(slab.PSI_B).numel() == 32 * 64 * 64 and r.buffer(slab.HS_A).numel() == 17 * 64 * 64
     assert r.buffer(slab.HS_B).numel() == 33 * 32 * 64
     r.close()
+
+
+DIST_WORKER = r"""
+import json, os, sys
+sys.path.insert(0, %r)
+import numpy as np, torch, torch.distributed as dist
+from paper_1909_08354_b200 import inputs, slab
+rank, R = int(os.environ["RANK"]), int(os.environ["WORLD_SIZE"])
+dist.init_process_group("gloo", rank=rank, world_size=R)
+torch.cuda.set_device(0)
+dims, L, steps = tuple(json.loads(os.environ["SLAB_DIMS"])), float(os.environ["SLAB_L"]), int(os.environ["SLAB_STEPS"])
+cfg = inputs.scaled(inputs.CONFIGS["C4"], dims, L=L, steps=steps)
+psi0 = cfg.initial_state()
+rows = dims[0] // R
+sim = slab.DistributedSlab(dims, L, cfg.A, cfg.B, cfg.C, cfg.D, cfg.g, cfg.dtau, device="cuda:0")
+sim.ctx.set_state(np.ascontiguousarray(psi0[rank * rows:(rank + 1) * rows]))
+n0 = sim.norm()
+sim.step(steps // 2)
+sim.step(steps - steps // 2)
+n1 = sim.norm()
+np.save(os.environ["SLAB_OUT"] + ".%%d.npy" %% rank, sim.ctx.get_state())
+print(json.dumps({"rank": rank, "n0": n0, "n1": n1}))
+dist.barrier()
+sim.ctx.close()
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("dims,R,steps", [((64, 64, 64), 2, 6), ((128, 64, 128), 4, 4)])
+def test_distributed_driver_as_rank_processes_on_one_gpu(mods, tmp_path, dims, R, steps):
+    """The one-process-per-rank driver (DistributedSlab: sn_slab_pack -> all_to_all_single -> unpack) run as R rank
+    PROCESSES that share this one GPU, over the gloo backend with host staging (nccl refuses two ranks on one device).
+    No kernel waits on another process: every exchange synchronises its stream and goes through the host.  Same
+    result as the single-context step."""
+    import json
+    import os
+    import socket
+    import subprocess
+    import sys
+    Oracle, inputs, slab, sn = mods
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "worker.py"
+    script.write_text(DIST_WORKER % root)
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = str(so.getsockname()[1])
+    L = 16.0
+    procs = []
+    for r in range(R):
+        env = dict(os.environ, RANK=str(r), WORLD_SIZE=str(R), LOCAL_RANK=str(r), MASTER_ADDR="127.0.0.1", MASTER_PORT=port,
+                   SLAB_DIMS=json.dumps(list(dims)), SLAB_L=str(L), SLAB_STEPS=str(steps), SLAB_OUT=str(tmp_path / "out"))
+        procs.append(subprocess.Popen([sys.executable, str(script)], env=env, stdout=subprocess.PIPE, stderr=subprocess.PIPE,
+                                      text=True))
+    norms = []
+    for p in procs:
+        o, e = p.communicate(timeout=600)
+        assert p.returncode == 0, e[-2000:]
+        norms.append(json.loads(o.strip().splitlines()[-1]))
+    got = np.concatenate([np.load(str(tmp_path / "out") + ".%d.npy" % r) for r in range(R)], axis=0)
+    cfg = inputs.scaled(inputs.CONFIGS["C4"], dims, L=L, steps=steps)
+    one = sn.Simulation.from_config(cfg)
+    one.set_state(cfg.initial_state())
+    d0 = one.diagnostics()
+    one.step(steps)
+    want = one.get_state()
+    one.close()
+    assert rel(got, want) < 5e-6
+    for n in norms:                                   # the all-reduced norm is the global one on every rank, and conserved
+        assert abs(n["n0"] - d0["norm"]) < 1e-6 * d0["norm"] and abs(n["n1"] - n["n0"]) < TOL_NORM * n["n0"]
