@@ -99,10 +99,9 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_strided(const PassA
         for (int m = 0; m < P; m++) g4[(long long)(j + T * m) * rs4] = pack4(a[m], b[m]);
     } else { // P_S_KDIAG
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
-        float acc = 0.f;
+        double v[1] = {0.0}; // fp32 data, fp64 accumulation from the first addition on (S12)
 #pragma unroll
-        for (int m = 0; m < P; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
-        double v[1] = {(double)acc};
+        for (int m = 0; m < P; m++) v[0] += (double)__ldg(p.ksq + j + T * m) * ((double)abs2(a[m]) + (double)abs2(b[m]));
         block_accumulate<1>(v, p.diag);
     }
 }
@@ -282,7 +281,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
         return;
     }
     if (MODE == P_H_DIAG) {
-        float s_rho = 0.f, s_pr = 0.f, s_f = 0.f;
+        double s_rho = 0.0, s_pr = 0.0, s_f = 0.0; // fp32 data, fp64 accumulation from the first addition on (S12)
 #pragma unroll
         for (int m = 0; m < P; m++) {
             const float4 u = psi4[(long long)(j + T * m) * rs4 + t];
@@ -297,20 +296,20 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) k_haxis(const PassArg
             }
 #pragma unroll
             for (int c = 0; c < 4; c++) {
-                s_rho += r[c];
-                s_pr = fmaf(ph[c], r[c], s_pr);
+                s_rho += (double)r[c];
+                s_pr += (double)ph[c] * (double)r[c];
                 const float f = fmaf(r[c], fmaf(r[c], fmaf(r[c], p.nl.fg[3], p.nl.fg[2]), p.nl.fg[1]), p.nl.fg[0]);
-                s_f = fmaf(r[c] * r[c], f, s_f);
+                s_f += (double)(r[c] * r[c]) * (double)f;
                 if (p.nl.flags) { // F_log = g_log (rho ln rho_f - rho), F_pow = g_pow rho rho_f^p/(p+1), V rho
                     const float rf = fmaxf(r[c], p.nl.floor_);
                     float e = ve[c];
                     if (p.nl.flog != 0.f) e += p.nl.flog * (logf(rf) - 1.f);
                     if (p.nl.fpow != 0.f) e = fmaf(p.nl.fpow, powf(rf, p.nl.ppow), e);
-                    s_f = fmaf(r[c], e, s_f);
+                    s_f += (double)r[c] * (double)e;
                 }
             }
         }
-        double v[3] = {(double)s_rho, (double)s_pr, (double)s_f};
+        double v[3] = {s_rho, s_pr, s_f};
         block_accumulate<3>(v, p.diag);
         return;
     }
@@ -427,10 +426,10 @@ __global__ void __launch_bounds__(xthreads(N), xthreads(N) <= 256 ? 2 : 1) k_con
         }
     } else { // P_X_KDIAG
         fft_pair<N, +1, true>(a, b, j, p.tw, sm);
-        float acc = 0.f;
+        double v[1] = {0.0};
 #pragma unroll
-        for (int m = 0; m < P; m++) acc = fmaf(__ldg(p.ksq + j + T * m), abs2(a[m]) + abs2(b[m]), acc);
-        double v[1] = {active ? (double)acc : 0.0};
+        for (int m = 0; m < P; m++) v[0] += (double)__ldg(p.ksq + j + T * m) * ((double)abs2(a[m]) + (double)abs2(b[m]));
+        if (!active) v[0] = 0.0;
         block_accumulate<1>(v, p.diag);
     }
 }

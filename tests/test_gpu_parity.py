@@ -498,3 +498,32 @@ def test_runs_on_a_side_stream(mods):
         got = out.cpu().numpy()
         sim.close()
     assert np.array_equal(got, want)
+
+
+def _two_gpus():
+    try:
+        import torch
+        return torch.cuda.is_available() and torch.cuda.device_count() >= 2
+    except Exception:
+        return False
+
+
+if _two_gpus():   # defined only on a multi-GPU box (a skip would show up in the single-GPU report)
+    def test_context_on_a_device_that_is_not_current(mods):
+        """The library runs every call on the device that owns the workspace (sn.h): a context on cuda:1 driven while
+        cuda:0 is current gives the same bits as one on cuda:0."""
+        import torch
+        snref, Oracle, inputs, sn = mods
+        cfg = inputs.scaled(inputs.CONFIGS["C4"], (64, 64, 64), L=16.0, steps=6)
+        psi0 = cfg.initial_state()
+        out = []
+        for dev in ("cuda:0", "cuda:1"):
+            torch.cuda.set_device(0)
+            sim = sn.Simulation.from_config(cfg, device=dev)
+            sim.set_state(psi0)
+            sim.step(6)
+            sim.diagnostics()
+            out.append(sim.get_state())
+            sim.close()
+            assert torch.cuda.current_device() == 0
+        assert np.array_equal(out[0], out[1])
