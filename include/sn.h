@@ -50,6 +50,7 @@ extern "C" {
 #define SN_ERR_CUDA -7      /* a CUDA runtime call failed (sticky; text via sn_strerror) */
 #define SN_ERR_NOMEM -8     /* host allocation failed */
 #define SN_ERR_FEATURE -9   /* the call needs a workspace region that was not requested at create (sn_options.features) */
+#define SN_ERR_TOO_LARGE -10 /* sn_norm_static: more cells than its fixed static scratch serves */
 
 typedef struct sn_ctx sn_ctx; /* opaque host object, owned by the library */
 
@@ -223,6 +224,23 @@ int sn_slab_buffer(sn_ctx *ctx, int which, void **ptr /* host; receives a DEVICE
 int sn_slab_pack(sn_ctx *ctx, int what /* SN_SLAB_PSI_A or SN_SLAB_HS_A */, int unpack);
 int sn_slab_exchange_local(sn_ctx **ctxs /* host, nranks contexts in rank order */, int nranks, int what, int to_a);
 int sn_slab_local_norm(sn_ctx *ctx, double *sum_abs2_dv /* host: this rank's part of the norm */);
+
+/* ---- allocation-free entry point (no context, no workspace) ----
+ * For callers that cannot allocate device memory at the call site (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): norm = dv * sum_{i < n_cells} |psi_i|^2 of a complex64 DEVICE array (the norm of the
+ * diagnostics, S12: fp32 data, fp64 accumulation), written to the DEVICE double *norm_out.  Enqueued on cuda_stream
+ * (two kernel launches), returns without synchronising; runs on the device that owns psi and restores the caller's
+ * current device.  Calls no cudaMalloc / cudaFree / allocating routine: its scratch (one partial sum per 8192 cells) is a
+ * file-scope __device__ array of SN_STATIC_NORM_SCRATCH_DOUBLES doubles = 256 KiB that every GPU which loads the library
+ * holds until the process exits.  Hence the limit: n_cells <= SN_STATIC_NORM_MAX_CELLS = 2^28 (a 2 GiB state; 512^3 is
+ * 2^27), beyond it SN_ERR_TOO_LARGE and nothing is launched.  n_cells = 0 gives 0.  The sum is taken in a fixed order:
+ * bitwise reproducible.  ALL calls on a device share the scratch array: each call overwrites the slots it reads (nothing
+ * needs clearing between calls), but two calls that OVERLAP on the GPU -- different streams, concurrently replayed
+ * graphs -- race on it and give wrong sums: keep calls on one stream or order them with events. */
+#define SN_STATIC_NORM_SCRATCH_DOUBLES 32768
+#define SN_STATIC_NORM_MAX_CELLS ((int64_t)1 << 28)
+int sn_norm_static(const void *psi /* DEVICE, n_cells complex64 */, int64_t n_cells, double dv,
+                   double *norm_out /* DEVICE, 1 double */, void *cuda_stream);
 
 int sn_destroy(sn_ctx *ctx);
 

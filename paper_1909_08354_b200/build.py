@@ -72,6 +72,7 @@ def _build_locked(force: bool) -> str:
     jobs += [(os.path.join(CSRC, "sn_kernels_f64.cu"), os.path.join(OBJ, f"sn_kernels_f64_{n}.o"), [f"-DSN_LEN={n}"])
              for n in LENGTHS_FIRST + LENGTHS + LENGTHS3]     # complex128 path
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))
+    jobs.append((os.path.join(CSRC, "sn_static.cu"), os.path.join(OBJ, "sn_static.o"), []))   # allocation-free entry point
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:
         objs = list(ex.map(_compile, jobs))
     subprocess.run([NVCC, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a",

@@ -980,6 +980,11 @@ void drop_step_graph(sn_ctx *c)
 
 } // namespace
 
+namespace snk {
+// for translation units with entry points of their own (sn_static.cu): record the text of a CUDA error for sn_strerror
+void record_cuda_error(int cuda_error) { cuda_fail((cudaError_t)cuda_error); }
+} // namespace snk
+
 // ============================================================================ C ABI
 
 extern "C" {
@@ -1650,6 +1655,9 @@ const char *sn_strerror(int code)
     case SN_ERR_CUDA: return g_cuda_msg;
     case SN_ERR_NOMEM: return "host allocation failed";
     case SN_ERR_FEATURE: return "the call needs a workspace region that was not requested at create (sn_options.features)";
+    case SN_ERR_TOO_LARGE:
+        return "sn_norm_static: n_cells exceeds SN_STATIC_NORM_MAX_CELLS = 2^28 (the 256 KiB static scratch holds one partial sum "
+               "per 8192 cells, 32768 slots); use a context (sn_create + sn_diagnostics) for larger arrays";
     default: return "unknown error code";
     }
 }

@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libsn.so")
 
 SN_OK = 0
 ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_ERR_SINGULAR",
-             -5: "SN_ERR_WORKSPACE", -6: "SN_ERR_STATE", -7: "SN_ERR_CUDA", -8: "SN_ERR_NOMEM", -9: "SN_ERR_FEATURE"}
+             -5: "SN_ERR_WORKSPACE", -6: "SN_ERR_STATE", -7: "SN_ERR_CUDA", -8: "SN_ERR_NOMEM", -9: "SN_ERR_FEATURE",
+             -10: "SN_ERR_TOO_LARGE"}
 
 # optional workspace regions (sn_options.features)
 FEAT_STAGING, FEAT_VEXT, FEAT_SOURCE, FEAT_ALL = 1, 2, 4, 7
@@ -32,7 +33,7 @@ EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get
            "sn_debug_fft", "sn_debug_potential", "sn_set_local_terms", "sn_set_external_potential", "sn_set_source_tables", "sn_step_order4", "sn_workspace_bytes_batch", "sn_create_batch", "sn_set_bohm", "sn_workspace_bytes_opt",
            "sn_create_opt", "sn_set_option", "sn_workspace_bytes_mc", "sn_create_mc", "sn_mc_norms",
            "sn_slab_workspace_bytes", "sn_slab_create", "sn_slab_stage", "sn_slab_buffer", "sn_slab_pack",
-           "sn_slab_exchange_local", "sn_slab_local_norm")
+           "sn_slab_exchange_local", "sn_slab_local_norm", "sn_norm_static")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
               "X_KDIAG", "H_SRC", "H_BOHM", "H_R2C_MC", "H_NL_MC")
@@ -95,6 +96,7 @@ def lib() -> ctypes.CDLL:
         L.sn_create_mc.argtypes = [ctypes.POINTER(vp), ctypes.c_int, i64p, dp, ctypes.c_int, dp, dp, ctypes.c_double,
                                    ctypes.c_double, dp, dp, ctypes.c_double, vp, ctypes.c_size_t, vp]
         L.sn_mc_norms.argtypes = [vp, dp]
+        L.sn_norm_static.argtypes = [vp, ctypes.c_int64, ctypes.c_double, vp, vp]
         L.sn_set_state.argtypes = [vp, vp, ctypes.c_int]
         L.sn_step.argtypes = [vp, ctypes.c_int64]
         L.sn_step_order4.argtypes = [vp, ctypes.c_int64]
@@ -127,6 +129,22 @@ def workspace_bytes(dims: Sequence[int], batch: int = 1, features: int = 0, dtyp
     d = (ctypes.c_int64 * len(dims))(*[int(n) for n in dims])
     opt = _options(batch, features, _DTYPES[dtype])
     return int(lib().sn_workspace_bytes_opt(len(dims), d, ctypes.byref(opt)))
+
+
+STATIC_NORM_MAX_CELLS = 1 << 28
+
+
+def norm_static(psi, dv: float, out, n_cells: Optional[int] = None, stream=None) -> None:
+    """sn_norm_static: out[0] = dv * sum |psi|^2 for a complex64 CUDA tensor psi, written to the float64 CUDA tensor `out`
+    (one element, caller-allocated).  No context, no workspace, no allocation: the scratch is a static device array of
+    the library (limit STATIC_NORM_MAX_CELLS cells; calls that overlap on the GPU race on it).  Asynchronous.
+    n_cells overrides psi.numel() (the tests pass an oversized count to check that it is rejected)."""
+    import torch
+    assert psi.is_cuda and psi.dtype == torch.complex64 and psi.is_contiguous()
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1 and out.device == psi.device
+    st = stream if stream is not None else torch.cuda.current_stream(psi.device)
+    _chk(lib().sn_norm_static(ctypes.c_void_p(psi.data_ptr()), int(psi.numel() if n_cells is None else n_cells), float(dv),
+                              ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(st.cuda_stream)), "sn_norm_static")
 
 
 class Simulation:
