@@ -85,6 +85,13 @@ __host__ __device__ constexpr int cpd_for(int N)
 }
 __host__ __device__ constexpr int sthreads(int N) { return cpd_for(N) * (N / ppt_for(N)); }
 __host__ __device__ constexpr int sblocks(int N) { return sthreads(N) <= 256 ? 2 : 1; }
+// axis-0 kernel: the modes without a psi transform (r2c, potential, diagnostics) fit 85 registers and run three CTAs per
+// SM; the nonlinear mode needs its 128 (at 85 it spills 420 bytes, also with phi parked in shared memory: measured with
+// -Xptxas -v), and the 12-point engine of the 3*2^a lengths one CTA per SM (240 bytes of spills at 128 registers)
+__host__ __device__ constexpr int hblocks(int N, int mode)
+{
+    return sthreads(N) <= 256 ? (mode == P_H_NLKIN ? (N % 3 == 0 ? 1 : 2) : 3) : 1;
+}
 
 // ---------------------------------------------------------------------------- strided axis
 // Tile: N rows (points of the line, row_stride elements apart) x CP adjacent columns; thread (t, j): column t,
@@ -139,7 +146,7 @@ __global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_strided(const Pass
 // the factor 1/2 is folded into the Poisson multiplier (PassArgsD::pscale).  The half spectrum stores X[k] in column
 // of the first and Y[k] in the column of the second real column, row k.
 template <int N, int CP, int MODE>
-__global__ void __launch_bounds__(sthreads(N), sblocks(N)) kd_haxis(const PassArgsD p)
+__global__ void __launch_bounds__(sthreads(N), hblocks(N, MODE)) kd_haxis(const PassArgsD p)
 {
     extern __shared__ double2 smem_d[];
     constexpr int P = ppt_for(N), T = N / P;

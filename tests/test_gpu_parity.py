@@ -214,6 +214,27 @@ STEP_CASES = [
     ("C5_512", (128, 512, 512), 128.0, 2),
 ]
 
+# C > 0 lying BETWEEN grid modes: 1/(C - k^2) changes sign inside the spectrum and is large next to C; the
+# hi/lo denominator of the Helmholtz pass keeps those modes accurate in fp32.  name, dims, L, C, steps
+POSITIVE_C_CASES = [
+    ("C2", (128, 128), 12.5, 3.3, 60),
+    ("C2", (512, 64), 25.0, 1.7, 30),          # pipelined 512-point passes
+    ("C4", (64, 64, 64), 16.0, 7.7, 30),       # 1.4e-3 (relative) from the mode k^2 = 7.711
+    ("C4", (64, 128, 256), 32.0, 2.05, 8),
+]
+
+
+@pytest.mark.parametrize("name,dims,L,C,steps", POSITIVE_C_CASES)
+def test_steps_match_oracle_with_positive_c(mods, name, dims, L, C, steps):
+    import dataclasses
+    snref, Oracle, inputs, sn = mods
+    cfg = dataclasses.replace(inputs.scaled(inputs.CONFIGS[name], dims, L=L, steps=steps), C=C)
+    got, want, sim = run_pair(mods, cfg, steps)
+    d = sim.diagnostics()
+    sim.close()
+    assert_state(got, want)
+    assert np.isfinite(d["e_total"])
+
 
 @pytest.mark.parametrize("name,dims,L,steps", STEP_CASES)
 def test_steps_match_oracle(mods, name, dims, L, steps):
