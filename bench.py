@@ -242,6 +242,8 @@ def main():
                          "precision the paper benchmarked): same step, 16 B per cell of state, float64 arithmetic")
     ap.add_argument("--dispatch", type=int, default=0, choices=[0, 1, 2],
                     help="sn_set_option(SN_OPT_DISPATCH): 0 default, 1 first-path kernels only, 2 pipelined wherever instantiated")
+    ap.add_argument("--graph-steps", type=int, default=0,
+                    help="sn_set_option(SN_OPT_GRAPH_STEPS): interior steps per replayed CUDA graph (launch-bound grids)")
     ap.add_argument("--slab", type=int, default=0,
                     help="time the slab-decomposed step (NEXT-2, DESIGN.md section 7) as this many virtual ranks on ONE GPU: "
                          "the local passes of every rank plus the all-to-all exchanges done as device-to-device copies")
@@ -340,6 +342,8 @@ def main():
         del rs, f, r2
     if args.dispatch:
         sim.set_option(sn.OPT_DISPATCH, args.dispatch)
+    if args.graph_steps:
+        sim.set_option(sn.OPT_GRAPH_STEPS, args.graph_steps)
     step = sim.step_order4 if args.order4 else sim.step
     sim.set_state(dev_in)
     step(W)                                             # untimed warm-up steps

@@ -277,6 +277,7 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 15 */, int64_t *lau
  *                   kernels (sn_kernels.cu) everywhere; 2: TMA-pipelined kernels (sn_pipe.cu) wherever instantiated. */
 #define SN_OPT_GRAPH 1
 #define SN_OPT_DISPATCH 2
+#define SN_OPT_GRAPH_STEPS 3 /* interior steps captured per replayed graph, 1 ... 64 (launch-bound grids; default: see sn_api.cu) */
 int sn_set_option(sn_ctx *ctx, int option, int value);
 
 /* In-place d-dimensional FFT of the internal state: direction +1 forward (e^{-i k x}, unscaled),

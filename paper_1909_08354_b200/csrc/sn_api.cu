@@ -281,6 +281,7 @@ struct sn_ctx {
     cudaStream_t cap_stream;
     cudaGraphExec_t step_graph;
     int graph_launches; // kernels inside the graph
+    int graph_steps;    // interior steps [N(dtau) K(dtau)] captured per graph (SN_OPT_GRAPH_STEPS)
     // optional per-launch timing (sn_profile): event pairs around every launch, summed per pass kind
     bool profiling;
     std::vector<cudaEvent_t> *ev;       // pool, pairs (start, stop)
@@ -951,8 +952,11 @@ int build_step_graph(sn_ctx *c)
     const int64_t before = c->launches;
     SN_CUDA(cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
     c->stream = c->cap_stream;
-    int rc = prepare_n(c, NL_MAIN);
-    if (rc == SN_OK) rc = kinetic_sweep(c, PH_FULL, /*with_nl=*/true, /*before_n=*/true);
+    int rc = SN_OK;
+    for (int s = 0; rc == SN_OK && s < c->graph_steps; s++) {
+        rc = prepare_n(c, NL_MAIN);
+        if (rc == SN_OK) rc = kinetic_sweep(c, PH_FULL, /*with_nl=*/true, /*before_n=*/true);
+    }
     c->stream = user;
     cudaGraph_t g = nullptr;
     const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &g);
@@ -1128,6 +1132,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
             for (int b = 0; b < mc->n; b++) c->gc[a][b] = mc->g[a * mc->n + b];
         }
     c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc && l.R == 1;
+    c->graph_steps = 1;
     c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
@@ -1310,6 +1315,8 @@ int sn_set_option(sn_ctx *c, int option, int value)
     if (!c) return SN_ERR_NULL;
     if (option == SN_OPT_GRAPH) {
         if (value != 0 && value != 1) return SN_ERR_PARAM;
+    } else if (option == SN_OPT_GRAPH_STEPS) {
+        if (value < 1 || value > 64) return SN_ERR_PARAM;
     } else if (option == SN_OPT_DISPATCH) {
         if (value < 0 || value > 2) return SN_ERR_PARAM;
     } else {
@@ -1318,7 +1325,9 @@ int sn_set_option(sn_ctx *c, int option, int value)
     DeviceGuard guard(c->device);
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
-    if (option == SN_OPT_GRAPH) {
+    if (option == SN_OPT_GRAPH_STEPS) {
+        c->graph_steps = value;
+    } else if (option == SN_OPT_GRAPH) {
         c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24) && !c->is_mc && c->lay.R == 1;
     } else {
         c->use_pipe = value != 1 && !c->f64;
@@ -1478,8 +1487,9 @@ int sn_step(sn_ctx *c, int64_t nsteps)
     int rc = kinetic_sweep(c, PH_HALF, /*with_nl=*/false, /*before_n=*/true);
     int64_t i = 1;
     if (rc == SN_OK && c->use_graph && !c->profiling && nsteps >= 4) {
-        if (!c->step_graph) rc = build_step_graph(c);
-        for (; rc == SN_OK && i < nsteps; i++) {
+        // each replay advances graph_steps interior steps; what is left over (and the closing step) runs as plain launches
+        if (!c->step_graph && i + c->graph_steps <= nsteps) rc = build_step_graph(c);
+        for (; rc == SN_OK && i + c->graph_steps <= nsteps; i += c->graph_steps) {
             SN_CUDA(cudaGraphLaunch(c->step_graph, c->stream));
             c->launches += c->graph_launches;
         }

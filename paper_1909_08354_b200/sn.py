@@ -24,7 +24,7 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # optional workspace regions (sn_options.features)
 FEAT_STAGING, FEAT_VEXT, FEAT_SOURCE, FEAT_ALL = 1, 2, 4, 7
 # sn_set_option
-OPT_GRAPH, OPT_DISPATCH = 1, 2
+OPT_GRAPH, OPT_DISPATCH, OPT_GRAPH_STEPS = 1, 2, 3
 DISPATCH_DEFAULT, DISPATCH_FIRST_PATH, DISPATCH_PIPELINED = 0, 1, 2
 
 # every symbol include/sn.h declares

@@ -479,19 +479,21 @@ def test_graph_replay_is_bitwise_the_stream_launch_path(mods):
     cfg = inputs.scaled(inputs.CONFIGS["C4"], (64, 64, 128), L=16.0, steps=12)
     psi0 = cfg.initial_state()
     out = {}
-    for mode in ("0", "1"):
+    for mode, (graph, per_graph) in {"plain": (0, 1), "graph1": (1, 1), "graph3": (1, 3), "graph5": (1, 5)}.items():
         sim = sn.Simulation.from_config(cfg)
-        sim.set_option(sn.OPT_GRAPH, 0 if mode == "1" else 1)
+        sim.set_option(sn.OPT_GRAPH, graph)
+        sim.set_option(sn.OPT_GRAPH_STEPS, per_graph)   # interior steps per replayed graph; the remainder runs as plain launches
         sim.set_state(psi0)
         n0 = sim.launch_count()
         sim.step(7)
         sim.set_dtau(0.5 * cfg.dtau)
         sim.step(5)
-        sim.step(2)                                   # below the graph threshold: plain launches in both modes
+        sim.step(2)                                   # below the graph threshold: plain launches in every mode
         out[mode] = (sim.get_state(), sim.launch_count() - n0)
         sim.close()
-    assert np.array_equal(out["0"][0], out["1"][0])
-    assert out["0"][1] == out["1"][1]                 # the launch counter counts the kernels inside the graph too
+    for mode in ("graph1", "graph3", "graph5"):
+        assert np.array_equal(out["plain"][0], out[mode][0]), mode
+        assert out["plain"][1] == out[mode][1], mode  # the launch counter counts the kernels inside the graph too
 
 
 def test_runs_on_a_side_stream(mods):
