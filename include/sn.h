@@ -261,10 +261,11 @@ int64_t sn_launch_count(const sn_ctx *ctx);
  *   8 X_KIN  contiguous-axis forward-phase-inverse 9 X_POISSON contiguous-axis forward-D/(C-k^2)-inverse
  *  10 X_KDIAG contiguous-axis kinetic-energy sum  11 H_SRC axis-0 source gamma rho + beta lap rho (eq. (12))
  *  12 H_BOHM axis-0 Bohm phase (eq. (15))       13 H_R2C_MC weighted density of coupled components + packed r2c
- *  14 H_NL_MC axis-0 c2r + nonlinear phases of coupled components */
-#define SN_NUM_PASS_KINDS 15
+ *  14 H_NL_MC axis-0 c2r + nonlinear phases of coupled components
+ *  15 R_STEPS the cluster-resident kernel: one launch = ALL steps of an sn_step call (small square 2D grids) */
+#define SN_NUM_PASS_KINDS 16
 int sn_profile(sn_ctx *ctx, int enable);
-int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 15 */, int64_t *launches_by_kind /* host, 15 */,
+int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 16 */, int64_t *launches_by_kind /* host, 16 */,
                     int reset);
 
 /* ---- test hooks (used by the acceptance tests, not by users) ---- */
@@ -278,6 +279,13 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 15 */, int64_t *lau
 #define SN_OPT_GRAPH 1
 #define SN_OPT_DISPATCH 2
 #define SN_OPT_GRAPH_STEPS 3 /* interior steps captured per replayed graph, 1 ... 64 (launch-bound grids; default: see sn_api.cu) */
+/*   SN_OPT_RESIDENT 1 (default): sn_step on a complex64 2D grid with n0 == n1 in {64, 128}, only the hot-path terms
+ *                   (no sn_set_local_terms / _external_potential / _bohm / _source_tables in effect), the default
+ *                   SN_OPT_DISPATCH and at most 32 ensemble members runs as ONE launch of the cluster-resident kernel:
+ *                   the state stays in the distributed shared memory of a cluster of 8 CTAs for all n steps of the
+ *                   call (one cluster per member); 0: the pass kernels.  Same schedule and arithmetic; the density is
+ *                   transformed as a complex field there, so the two paths agree to rounding, not bit for bit. */
+#define SN_OPT_RESIDENT 4
 int sn_set_option(sn_ctx *ctx, int option, int value);
 
 /* In-place d-dimensional FFT of the internal state: direction +1 forward (e^{-i k x}, unscaled),

@@ -17,6 +17,7 @@ LIB = os.path.join(HERE, "libsn.so")
 LENGTHS = (64, 128, 256, 512, 1024, 2048, 4096)   # pipelined + first-path kernels
 LENGTHS_FIRST = (32,)                              # first-path kernels only
 LENGTHS3 = (96, 192, 384, 768, 1536, 3072)        # 3*2^a: 12 points per thread
+LENGTHS_RESIDENT = (64, 128)                       # square 2D grids held in one cluster's shared memory
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3",
          "-Xcompiler", "-fPIC", "-diag-suppress", "128"]
@@ -71,6 +72,8 @@ def _build_locked(force: bool) -> str:
              for n in LENGTHS + LENGTHS3]
     jobs += [(os.path.join(CSRC, "sn_kernels_f64.cu"), os.path.join(OBJ, f"sn_kernels_f64_{n}.o"), [f"-DSN_LEN={n}"])
              for n in LENGTHS_FIRST + LENGTHS + LENGTHS3]     # complex128 path
+    jobs += [(os.path.join(CSRC, "sn_resident.cu"), os.path.join(OBJ, f"sn_resident_{n}.o"), [f"-DSN_LEN={n}"])
+             for n in LENGTHS_RESIDENT]                       # cluster-resident step of small 2D grids
     jobs.append((os.path.join(CSRC, "sn_api.cu"), os.path.join(OBJ, "sn_api.o"), []))
     jobs.append((os.path.join(CSRC, "sn_static.cu"), os.path.join(OBJ, "sn_static.o"), []))   # allocation-free entry point
     with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as ex:

@@ -270,6 +270,7 @@ struct sn_ctx {
     double *diag;
     int *sched;                             // tile counters of the dynamically scheduled pipelined kernels
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
+    bool use_resident; // SN_OPT_RESIDENT: small square 2D grids advance inside one cluster's shared memory (sn_resident.cu)
     bool use_pipe;  // SN_OPT_DISPATCH != 1
     bool pipe_all;  // SN_OPT_DISPATCH == 2: pipelined kernels wherever they are instantiated (tests, A/B runs)
     int sm_count;
@@ -944,6 +945,67 @@ int slab_copy_block(const Layout &l, float2 *A_r, float2 *B_s, int64_t lo, int64
     return e == cudaSuccess ? SN_OK : cuda_fail(e);
 }
 
+// ---- cluster-resident step (sn_resident.cu): the whole sn_step(n) call of a small square 2D grid in ONE launch ----
+// Served: complex64, 2D, n0 == n1 in {64, 128}, the hot-path terms only (polynomial G; no NEXT-1 term set), the default
+// dispatch (SN_OPT_DISPATCH 1 / 2 ask for the pass kernels by name), ensembles of up to RESIDENT_MAX_BATCH members
+// (one cluster per member; measured on B200, 128^2: 16 members 13 vs 25 us/step, 64 members 34 vs 29 -- a large
+// ensemble fills the machine through the pass kernels, which are the faster ones per cell).  Everything else takes the
+// pass kernels.
+constexpr int64_t RESIDENT_MAX_BATCH = 32;
+bool resident_eligible(const sn_ctx *c)
+{
+    const Layout &l = c->lay;
+    return c->use_resident && c->use_pipe && !c->pipe_all && !c->f64 && !c->is_mc && l.R == 1 && l.ndim == 2 &&
+           snk::resident_supported((int)l.n[0], (int)l.n[1]) && c->nlv[NL_MAIN].flags == 0 && !c->has_vext && !c->has_src &&
+           c->c_bohm == 0.0 && l.batch <= RESIDENT_MAX_BATCH;
+}
+
+int run_resident(sn_ctx *c, int64_t nsteps)
+{
+    const Layout &l = c->lay;
+    snk::ResidentArgs a;
+    std::memset(&a, 0, sizeof(a));
+    a.psi = c->psi;
+    a.row_stride = l.batch * l.n[1];
+    a.batch = (int)l.batch;
+    a.nsteps = nsteps;
+    a.tw = c->tw[0]; // n0 == n1: one table serves both axes
+    for (int d = 0; d < 2; d++) {
+        a.ph_full[d] = c->ph[PH_FULL][d];
+        a.ph_half[d] = c->ph[PH_HALF][d];
+    }
+    a.ksq2_1 = c->ksq2[1];
+    a.dk0 = c->kother[0];
+    a.pscale = (float)(c->D / (double)l.pcells);
+    a.nl = c->nlv[NL_MAIN];
+    a.stream = c->stream;
+    size_t ev = 0;
+    if (c->profiling) {
+        ev = c->ev_kind->size();
+        if (c->ev->size() < 2 * (ev + 1)) {
+            cudaEvent_t e0, e1;
+            SN_CUDA(cudaEventCreate(&e0));
+            SN_CUDA(cudaEventCreate(&e1));
+            c->ev->push_back(e0);
+            c->ev->push_back(e1);
+        }
+        SN_CUDA(cudaEventRecord((*c->ev)[2 * ev], c->stream));
+    }
+    int rc;
+    switch ((int)l.n[0]) {
+    case 64: rc = snk::launch_resident<64>(a); break;
+    case 128: rc = snk::launch_resident<128>(a); break;
+    default: return SN_ERR_DIMS;
+    }
+    if (rc != 0) return cuda_fail((cudaError_t)rc);
+    c->launches++;
+    if (c->profiling) {
+        SN_CUDA(cudaEventRecord((*c->ev)[2 * ev + 1], c->stream));
+        c->ev_kind->push_back(snk::P_R_STEPS);
+    }
+    return SN_OK;
+}
+
 // capture one interior step N(dtau) K(dtau) (the pass list of potential_spectrum + a full kinetic sweep)
 int build_step_graph(sn_ctx *c)
 {
@@ -1134,6 +1196,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc && l.R == 1;
     c->graph_steps = 1;
     c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
+    c->use_resident = true;
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
     int rc = SN_OK;
@@ -1319,13 +1382,17 @@ int sn_set_option(sn_ctx *c, int option, int value)
         if (value < 1 || value > 64) return SN_ERR_PARAM;
     } else if (option == SN_OPT_DISPATCH) {
         if (value < 0 || value > 2) return SN_ERR_PARAM;
+    } else if (option == SN_OPT_RESIDENT) {
+        if (value != 0 && value != 1) return SN_ERR_PARAM;
     } else {
         return SN_ERR_PARAM;
     }
     DeviceGuard guard(c->device);
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
-    if (option == SN_OPT_GRAPH_STEPS) {
+    if (option == SN_OPT_RESIDENT) {
+        c->use_resident = value == 1;
+    } else if (option == SN_OPT_GRAPH_STEPS) {
         c->graph_steps = value;
     } else if (option == SN_OPT_GRAPH) {
         c->use_graph = value == 1 && c->lay.cells <= ((int64_t)1 << 24) && !c->is_mc && c->lay.R == 1;
@@ -1483,6 +1550,7 @@ int sn_step(sn_ctx *c, int64_t nsteps)
         }
         return rc;
     }
+    if (resident_eligible(c)) return run_resident(c, nsteps); // same schedule, one launch, state held on chip
     // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2): adjacent half kinetics merged
     int rc = kinetic_sweep(c, PH_HALF, /*with_nl=*/false, /*before_n=*/true);
     int64_t i = 1;

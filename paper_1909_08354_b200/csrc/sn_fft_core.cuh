@@ -204,6 +204,11 @@ __host__ __device__ constexpr int twiddle_entries(int N)
 template <bool HILO, int NS>
 __host__ __device__ constexpr bool stage_hilo() { return HILO && NS <= SN_HILO_MAX_NS; }
 
+// The pass kernels read the tables from global memory through the read-only path; a kernel that keeps its tables in
+// shared memory (sn_resident.cu) defines SN_TW_LOAD as a plain load before including this header.
+#ifndef SN_TW_LOAD
+#define SN_TW_LOAD(p) __ldg(p)
+#endif
 template <int N, int R, int NS, int OFF, bool HILO, int P>
 __device__ __forceinline__ void load_twiddles(float4 (&w)[(P / R) * (R - 1)], int j, const float4 *__restrict__ tw)
 {
@@ -215,9 +220,9 @@ __device__ __forceinline__ void load_twiddles(float4 (&w)[(P / R) * (R - 1)], in
 #pragma unroll
         for (int r = 1; r < R; r++) {
             if (HILO) {
-                w[q * (R - 1) + r - 1] = __ldg(tw + OFF + kp + (r - 1) * NS);
+                w[q * (R - 1) + r - 1] = SN_TW_LOAD(tw + OFF + kp + (r - 1) * NS);
             } else {
-                const float2 h = __ldg(tw2 + OFF + kp + (r - 1) * NS);
+                const float2 h = SN_TW_LOAD(tw2 + OFF + kp + (r - 1) * NS);
                 w[q * (R - 1) + r - 1] = make_float4(h.x, h.y, 0.f, 0.f);
             }
         }

@@ -21,7 +21,8 @@ enum PassKind {
     P_H_SRC,       // axis 0: c2r of F[lap rho] -> s = gamma rho + beta lap rho -> packed r2c   (eq. (12), NEXT-1)
     P_H_BOHM,      // axis 0: c2r of F[lap sqrt(rho)] -> psi *= exp(-i s c_B lap sqrt(rho)/(2 sqrt(rho)))  (eq. (15))
     P_H_R2C_MC,    // axis 0, coupled components: rho = sum_c w_c |psi_c|^2 -> packed r2c
-    P_H_NL_MC      // axis 0, coupled components: c2r of phi^ -> psi_c *= exp(-i s (B_c phi + sum_c' g_cc' rho_c')) for every c
+    P_H_NL_MC,     // axis 0, coupled components: c2r of phi^ -> psi_c *= exp(-i s (B_c phi + sum_c' g_cc' rho_c')) for every c
+    P_R_STEPS      // cluster-resident kernel: ALL steps of an sn_step(n) call on a small 2D grid in one launch (sn_resident.cu)
 };
 
 // Coupled wave functions (NEXT-4b; reading Q18 of DESIGN.md): up to 4 components, stored one after the other
@@ -174,6 +175,27 @@ struct PassArgsD {
 };
 template <int N>
 int launch_pass_d(const PassArgsD &a);
+
+// ---- cluster-resident step (sn_resident.cu): small square 2D grids, complex64, hot-path terms only ----
+// The state lives in the distributed shared memory of a cluster of RES_CLUSTER CTAs for a whole sn_step(n) call.
+constexpr int RES_CLUSTER = 8;
+struct ResidentArgs {
+    float2 *psi;              // DEVICE: state, storage [n0][batch][n1]
+    long long row_stride;     // elements between consecutive rows of one member (batch * n1)
+    int batch;                // ensemble members: one cluster each
+    long long nsteps;         // Strang steps of this call (>= 1)
+    const float4 *tw;         // DEVICE: twiddle table of the (common) line length
+    const float4 *ph_full[2]; // DEVICE: kinetic phase tables per axis, s = dtau
+    const float4 *ph_half[2]; // DEVICE: s = dtau/2
+    const float2 *ksq2_1;     // DEVICE: k_1^2 per index of axis 1 as hi + lo
+    const float2 *dk0;        // DEVICE: C - k_0^2 as hi + lo per half-spectrum row and member ([n0/2+1][batch])
+    float pscale;             // D / (n0 n1)
+    NLParams nl;
+    cudaStream_t stream;
+};
+inline bool resident_supported(int n0, int n1) { return n0 == n1 && (n0 == 64 || n0 == 128); }
+template <int N>
+int launch_resident(const ResidentArgs &a);
 
 // sum |psi|^2 over n complex64 values, accumulated in double into *out (sn_mc_norms)
 int launch_norm(const float2 *psi, long long n, double *out, cudaStream_t stream);

@@ -24,7 +24,7 @@ ERR_NAMES = {-1: "SN_ERR_NULL", -2: "SN_ERR_DIMS", -3: "SN_ERR_PARAM", -4: "SN_E
 # optional workspace regions (sn_options.features)
 FEAT_STAGING, FEAT_VEXT, FEAT_SOURCE, FEAT_ALL = 1, 2, 4, 7
 # sn_set_option
-OPT_GRAPH, OPT_DISPATCH, OPT_GRAPH_STEPS = 1, 2, 3
+OPT_GRAPH, OPT_DISPATCH, OPT_GRAPH_STEPS, OPT_RESIDENT = 1, 2, 3, 4
 DISPATCH_DEFAULT, DISPATCH_FIRST_PATH, DISPATCH_PIPELINED = 0, 1, 2
 
 # every symbol include/sn.h declares
@@ -36,7 +36,7 @@ EXPORTS = ("sn_workspace_bytes", "sn_create", "sn_set_state", "sn_step", "sn_get
            "sn_slab_exchange_local", "sn_slab_local_norm", "sn_norm_static")
 
 PASS_KINDS = ("S_FFT", "S_KIN", "S_KDIAG", "H_NLKIN", "H_R2C", "H_POT", "H_DIAG", "X_FFT", "X_KIN", "X_POISSON",
-              "X_KDIAG", "H_SRC", "H_BOHM", "H_R2C_MC", "H_NL_MC")
+              "X_KDIAG", "H_SRC", "H_BOHM", "H_R2C_MC", "H_NL_MC", "R_STEPS")
 
 
 class SnDiag(ctypes.Structure):
@@ -307,7 +307,7 @@ class Simulation:
         return {k: getattr(d, k) for k, _ in SnDiag._fields_}
 
     def set_option(self, option: int, value: int) -> None:
-        """OPT_GRAPH 0/1; OPT_DISPATCH DISPATCH_DEFAULT / DISPATCH_FIRST_PATH / DISPATCH_PIPELINED (A/B runs, tests)."""
+        """OPT_GRAPH 0/1; OPT_DISPATCH DISPATCH_DEFAULT / DISPATCH_FIRST_PATH / DISPATCH_PIPELINED; OPT_RESIDENT 0/1 (A/B runs, tests)."""
         _chk(lib().sn_set_option(self._h, int(option), int(value)), "sn_set_option")
 
     def launch_count(self) -> int:
