@@ -48,6 +48,7 @@ PASS_BYTES_PER_CELL = {
     "X_POISSON": 8.0,
     "H_SRC": 24.0,     # eq. (12): read F[lap rho] (4) + psi (8) + beta, gamma (8), write F[s] (4)
     "H_BOHM": 20.0,    # eq. (15) Bohm phase: read F[lap sqrt(rho)] (4) + psi (8), write psi (8)
+    "R_STEPS": 16.0,   # cluster-resident kernel (64^2 / 128^2): ONE launch = all K steps, psi read once and written once
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
 B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update
@@ -436,6 +437,9 @@ def main():
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras and not f64 and not args.batch else None,
                 "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r02g_ncu_full_C5_512.md",
+                "note": ("R_STEPS = the cluster-resident kernel: one launch advances all K steps with the state in distributed "
+                         "shared memory, HBM sees 16 B/cell per CALL; it is latency-bound inside the cluster, so every HBM "
+                         "fraction of this line is an effective figure only") if dom == "R_STEPS" else None,
                 "algorithmic_bytes_per_launch": bpc * cells, "peak_source": peak_src,
                 "bytes_per_cell": bpc, "avg_launch_ms": dom_ms, "share_of_step": prof[dom][0] / tot,
                 "per_pass": {k: {"ms_per_launch": v[0] / v[1], "launches": v[1], "share": v[0] / tot,
