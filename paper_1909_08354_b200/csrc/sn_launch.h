@@ -111,9 +111,20 @@ struct PipeArgs {
 // geometry of the pipelined kernels, shared by the scheduler (tensor maps, tile counts) and sn_pipe.cu:
 // 8 points per thread and 512 threads for N = 2^n; 12 points per thread and 256 threads for N = 3*2^a
 __host__ __device__ constexpr int pipe_ppt(int N) { return N % 3 == 0 ? 12 : 8; }
-__host__ __device__ constexpr int pipe_threads(int N) { return N % 3 == 0 ? 256 : 512; }
+// N = 384 (BASELINE.json's sweep size): 12 warps of 168 registers (12 line pairs, 72 KB tiles, 64-byte rows) instead of 8
+// warps of ~195: H_NLKIN 0.613 -> 0.460 ms.  Measured for the other 3*2^a lengths and not taken: 192^3 0.236 -> 0.221
+// ms/step, 768^3 16.8 -> 18.2 (6 groups: 32-byte rows instead of 64), N = 96 does not fit (48 groups: 2 x 114 KB stages).
+#ifndef SN_PIPE_THREADS_384
+#define SN_PIPE_THREADS_384 384 // 256 = the round-1 geometry (A/B builds)
+#endif
+__host__ __device__ constexpr int pipe_threads(int N) { return N == 384 ? SN_PIPE_THREADS_384 : N % 3 == 0 ? 256 : 512; }
 __host__ __device__ constexpr int pipe_groups(int N) { return pipe_threads(N) / (N / pipe_ppt(N)); } // line pairs per tile
-__host__ __device__ constexpr int pipe_cpw(int N) { return pipe_groups(N) < 8 ? pipe_groups(N) : 8; }
+__host__ __device__ constexpr int pipe_cpw(int N) // largest power of two <= 8 that divides the group count
+{
+    int c = 8;
+    while (pipe_groups(N) % c) c /= 2;
+    return c;
+}
 __host__ __device__ constexpr int pipe_box_rows(int rows) // largest divisor of `rows` that is <= 256 (rows = 2^a 3^b)
 {
     int r = rows;
@@ -125,9 +136,11 @@ __host__ __device__ constexpr int pipe_box_rows(int rows) // largest divisor of 
 // length in sn_api.cu); otherwise launch_pass<N>
 inline bool pipe_supported(int N, int kind, long long ncols, long long nlines)
 {
-    // 3*2^a lengths: measured at 384^3, the 256-thread pipelined CTA (8 warps, ~195 registers) only beats the
-    // first-path kernels (2+ CTAs per SM) for the heavy axis-0 pass (0.94 vs 1.24 ms); the others stay first-path
-    if (N % 3 == 0 && kind != P_H_NLKIN) return false;
+    // 3*2^a lengths: measured at 384^3, the pipelined CTA (12 points per thread: 12 warps of 168 registers at N = 384, 8
+    // warps of ~195 elsewhere) only beats the first-path kernels (2-3 CTAs per SM) for the axis-0 passes -- H_NLKIN 0.46
+    // vs 1.24 ms, H_R2C 0.199 vs 0.222 (N = 384) -- and loses for the others (S_KIN 0.49 vs 0.31, X_KIN 0.44 vs 0.28,
+    // X_POISSON 0.21 vs 0.15, S_FFT 0.11 vs 0.09 ms): those stay first-path even under SN_OPT_DISPATCH = 2
+    if (N % 3 == 0 && kind != P_H_NLKIN && !(N == 384 && kind == P_H_R2C)) return false;
     if (N < 64) return false; // 32-point lines: first-path kernels only (no pipelined instantiation)
     switch (kind) {
     case P_S_FFT:

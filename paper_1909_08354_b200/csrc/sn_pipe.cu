@@ -50,7 +50,7 @@ struct Geo {
     static constexpr int T = N / P;                       // threads per line pair
     static constexpr int G = NTHR / T;                    // line pairs (groups) per tile
     static constexpr int TILE_BYTES = N * 2 * G * 8;      // 64 KB (N = 2^n) or 48 KB (N = 3*2^a)
-    static constexpr int CPW = G < 8 ? G : 8;             // column pairs per sub-tile row (8 for N <= 512, then 4, 2, 1)
+    static constexpr int CPW = pipe_cpw(N);               // column pairs per sub-tile row (8 for N <= 512, then 4, 2, 1; 4 at N = 384)
     static constexpr int RBY = 16 * CPW;                  // bytes of a sub-tile row: 128, 64, 32, 16
     static constexpr int SUB = G / CPW;                   // sub-tiles per tile
     static constexpr int RB = pipe_box_rows(N);           // rows per TMA box
