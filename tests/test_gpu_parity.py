@@ -482,7 +482,7 @@ def test_graph_replay_is_bitwise_the_stream_launch_path(mods):
     for mode, (graph, per_graph) in {"plain": (0, 1), "graph1": (1, 1), "graph3": (1, 3), "graph5": (1, 5)}.items():
         sim = sn.Simulation.from_config(cfg)
         sim.set_option(sn.OPT_GRAPH, graph)
-        sim.set_option(sn.OPT_GRAPH_STEPS, per_graph)   # interior steps per replayed graph; the remainder runs as plain launches
+        sim.set_option(sn.OPT_GRAPH_STEPS, per_graph)   # interior steps per replayed graph; the remainder replays a one-step graph
         sim.set_state(psi0)
         n0 = sim.launch_count()
         sim.step(7)
