@@ -950,7 +950,7 @@ int slab_copy_block(const Layout &l, float2 *A_r, float2 *B_s, int64_t lo, int64
 // ---- cluster-resident step (sn_resident.cu): the whole sn_step(n) call of a small square 2D grid in ONE launch ----
 // Served: complex64, 2D, n0 == n1 in {64, 128}, the hot-path terms only (polynomial G; no NEXT-1 term set), the default
 // dispatch (SN_OPT_DISPATCH 1 / 2 ask for the pass kernels by name), ensembles of up to RESIDENT_MAX_BATCH members
-// (one cluster per member; measured on B200, 128^2: 16 members 13 vs 25 us/step, 64 members 34 vs 29 -- a large
+// (one cluster per member; measured on B200, 128^2: 16 members 13 vs 25 us/step, 32 members 14 vs 26, 64 members 28 vs 28 -- a large
 // ensemble fills the machine through the pass kernels, which are the faster ones per cell).  Everything else takes the
 // pass kernels.
 constexpr int64_t RESIDENT_MAX_BATCH = 32;

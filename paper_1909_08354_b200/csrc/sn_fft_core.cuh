@@ -678,7 +678,21 @@ struct SmemLine {
     static constexpr int TMASK = 0;
     __host__ __device__ static constexpr int lin(int pos) { return pos ^ ((pos >> 3) & 7); }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos); }
-    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { base[i] = make_float4(a.x, a.y, b.x, b.y); }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const
+    {
+#ifdef SN_XCH_SPLIT_STORES
+        // two 64-bit stores: the packed engine's (r, i) register pairs go out as they are.  One 128-bit store needs
+        // four CONSECUTIVE registers and ptxas builds them with four MOVs per store (14 % of the instructions of a
+        // latency-bound kernel); it costs 2-way bank conflicts, which only a kernel far from the shared-memory limit
+        // can afford (sn_resident.cu).
+        // (inline PTX: written as two plain stores the compiler fuses them back into one 128-bit store)
+        const unsigned addr = (unsigned)__cvta_generic_to_shared(base + i);
+        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a.x), "f"(a.y) : "memory");
+        asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(addr), "f"(b.x), "f"(b.y) : "memory");
+#else
+        base[i] = make_float4(a.x, a.y, b.x, b.y);
+#endif
+    }
     __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
         const float4 v = base[i];

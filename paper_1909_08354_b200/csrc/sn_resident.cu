@@ -11,6 +11,10 @@
 //   "column" sweeps (along axis 0): rank r takes the column pairs [r N/8, (r+1) N/8) and reads / writes its points in
 //     place in the owners' shared memory (ld/st.shared::cluster, one float4 = both columns of a row; the row pitch of
 //     N + 2 complex puts the 8 lanes of a quarter-warp on 8 different bank groups): no transposed copy exists;
+//   a stored row keeps the two columns of a pair interleaved -- slot (row, c/2) = (re_c, re_c+1, im_c, im_c+1) -- which
+//     IS the engine's packed register layout: a column sweep's 128-bit access and a row sweep's four 32-bit accesses per
+//     point land in the register pairs directly (the first version stored complex values and spent 15 % of its
+//     instructions re-packing);
 //   between sweeps of different orientation: one hardware cluster barrier (barrier.cluster, release/acquire).
 //
 // One step (S1-S13 of SURVEY.md 8(a); eq. (1),(2), method PAPER.md:113) is THREE sweeps, the
@@ -29,6 +33,8 @@
 #include <stdint.h>
 
 #define SN_TW_LOAD(p) (*(p)) // the engine's twiddle loads: the tables live in shared memory here
+#define SN_NL_SLOW_OUTLINE   // the rare large-angle path of the nonlinear phase as a call (code size)
+#define SN_XCH_SPLIT_STORES  // exchange stores as two 64-bit stores (no register re-packing; see SmemLine::st_i)
 #include "sn_fft_core.cuh"
 #include "sn_launch.h"
 #include "sn_pointwise.cuh"
@@ -50,14 +56,15 @@ struct RGeo {
     static constexpr int NTHR = G * T;        // 32 / 128 threads at N = 64 / 128
     static constexpr int PITCH = N + 2;       // complex per stored row
     static constexpr int NTW = twiddle_entries(N);
-    // psi rows | rho rows | exchange buffers | twiddles (hi/lo + plain copy) | phases [slot][axis][N] | C - k0^2 [N] | k1^2 [N]
+    // psi rows | rho rows | exchange buffers | twiddles (hi/lo + plain copy) | phases [slot][axis][N] | C - k0^2 [N] | k1^2 [N] | multipliers
     static constexpr size_t OFF_RHO = (size_t)NL * PITCH * 8;
     static constexpr size_t OFF_XCH = 2 * OFF_RHO;
     static constexpr size_t OFF_TW = OFF_XCH + (size_t)G * N * 16;
     static constexpr size_t OFF_PH = OFF_TW + (size_t)NTW * 24;
     static constexpr size_t OFF_DK0 = OFF_PH + 4 * (size_t)N * 16;
     static constexpr size_t OFF_K1 = OFF_DK0 + (size_t)N * 8;
-    static constexpr size_t SMEM = OFF_K1 + (size_t)N * 8;
+    static constexpr size_t OFF_MUL = OFF_K1 + (size_t)N * 8; // multipliers of eq. (2) per thread: [orientation][m][thread] float2
+    static constexpr size_t SMEM = OFF_MUL + 2 * (size_t)P * NTHR * 8;
     static_assert(T == NL && T <= 32, "point j + T m of an axis-0 line lives in row j of rank m; a pair is one warp or less");
     static_assert(OFF_TW % 16 == 0 && OFF_PH % 16 == 0 && (NTW * 16) % 8 == 0, "table alignment");
 };
@@ -87,14 +94,16 @@ __device__ __forceinline__ int opaque(int v)
     return v;
 }
 
-// Where the thread's line pair lives.  cols == false: its two own rows (row0 = first row's slot of point j in this
-// rank's psi rows; the second row PITCH further).  cols == true: its column pair, point j + T m in row j of rank m
-// (slot[m], one float4 = both columns).  rho / phi^ sits at the same place in the rho rows (QB bytes further).
+// Where the thread's line pair lives.  A stored row is N/2 + 1 slots of float4 = (re_c, re_c+1, im_c, im_c+1), one per
+// column pair.  cols == false: the thread's two own rows; point p = j + T m of row r is the float at
+// r * PF + 4 (p / 2) + (p & 1) (re) and 2 further (im): row0 points at it for m = 0 of the first row, the second row is PF
+// floats further, consecutive m are 2 T floats apart (T is even).  cols == true: its column pair, point j + T m in row j
+// of rank m (slot[m], one float4).  rho / phi^ sits at the same place in the rho rows (QB bytes further).
 template <int N>
 struct Lines {
-    static constexpr int P = RGeo<N>::P, T = RGeo<N>::T, PITCH = RGeo<N>::PITCH;
+    static constexpr int P = RGeo<N>::P, T = RGeo<N>::T, PF = 2 * RGeo<N>::PITCH;
     static constexpr uint32_t QB = (uint32_t)RGeo<N>::OFF_RHO;
-    float2 *row0;
+    float *row0;
     uint32_t slot[P];
 
     template <bool RHO>
@@ -102,11 +111,15 @@ struct Lines {
     {
         if (cols) {
 #pragma unroll
-            for (int m = 0; m < P; m++) x[m] = unpack4(ld_cluster(slot[m] + (RHO ? QB : 0u)));
+            for (int m = 0; m < P; m++) {
+                const float4 v = ld_cluster(slot[m] + (RHO ? QB : 0u));
+                x[m] = cp2{make_float2(v.x, v.y), make_float2(v.z, v.w)};
+            }
         } else {
-            const float2 *a = row0 + (RHO ? QB / 8 : 0), *b = a + PITCH;
+            const float *a = row0 + (RHO ? QB / 4 : 0), *b = a + PF;
 #pragma unroll
-            for (int m = 0; m < P; m++) x[m] = pack_pair(a[T * m], b[T * m]);
+            for (int m = 0; m < P; m++)
+                x[m] = cp2{make_float2(a[2 * T * m], b[2 * T * m]), make_float2(a[2 * T * m + 2], b[2 * T * m + 2])};
         }
     }
     template <bool RHO>
@@ -114,13 +127,15 @@ struct Lines {
     {
         if (cols) {
 #pragma unroll
-            for (int m = 0; m < P; m++) st_cluster(slot[m] + (RHO ? QB : 0u), pack4(x[m]));
+            for (int m = 0; m < P; m++) st_cluster(slot[m] + (RHO ? QB : 0u), make_float4(x[m].r.x, x[m].r.y, x[m].i.x, x[m].i.y));
         } else {
-            float2 *a = row0 + (RHO ? QB / 8 : 0), *b = a + PITCH;
+            float *a = row0 + (RHO ? QB / 4 : 0), *b = a + PF;
 #pragma unroll
             for (int m = 0; m < P; m++) {
-                a[T * m] = line_a(x[m]);
-                b[T * m] = line_b(x[m]);
+                a[2 * T * m] = x[m].r.x;
+                b[2 * T * m] = x[m].r.y;
+                a[2 * T * m + 2] = x[m].i.x;
+                b[2 * T * m + 2] = x[m].i.y;
             }
         }
     }
@@ -166,12 +181,13 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     const int rank = (int)cluster.block_rank();
     const int member = blockIdx.x / R;
     extern __shared__ __align__(16) uint8_t smem_raw[];
-    float2 *psis = reinterpret_cast<float2 *>(smem_raw);                     // [NL][PITCH] this rank's rows of psi
+    float *psis = reinterpret_cast<float *>(smem_raw);                       // [NL][2 PITCH] this rank's rows of psi (slots, see Lines)
     float4 *xch = reinterpret_cast<float4 *>(smem_raw + g_::OFF_XCH);        // [G][N] exchange buffers of the line-FFT engine
     float4 *tw = reinterpret_cast<float4 *>(smem_raw + g_::OFF_TW);          // twiddles: hi/lo table, then the plain copy
     float4 *phs = reinterpret_cast<float4 *>(smem_raw + g_::OFF_PH);         // kinetic phases [full, half][axis][N]
     float2 *dk0 = reinterpret_cast<float2 *>(smem_raw + g_::OFF_DK0);        // C - k0^2 per index of axis 0 (hi + lo)
     float2 *k1s = reinterpret_cast<float2 *>(smem_raw + g_::OFF_K1);         // k1^2 per index of axis 1 (hi + lo)
+    float2 *mul = reinterpret_cast<float2 *>(smem_raw + g_::OFF_MUL);        // D/(C - k^2)/(N0 N1) of the thread's points, both orientations
     const int tid = threadIdx.x, g = tid / T, j = tid % T;
     SmemLine<T> sm{xch + g * N, 1 + g, false};
     float2 *gpsi = a.psi + (long long)member * N; // storage [n0][batch][n1]
@@ -194,7 +210,9 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     }
     for (int e = tid; e < NL * N; e += NTHR) {
         const int l = e / N, p = e % N;
-        psis[l * PITCH + p] = gpsi[(long long)(rank * NL + l) * a.row_stride + p];
+        const float2 v = gpsi[(long long)(rank * NL + l) * a.row_stride + p];
+        psis[l * 2 * PITCH + 4 * (p >> 1) + (p & 1)] = v.x;
+        psis[l * 2 * PITCH + 4 * (p >> 1) + (p & 1) + 2] = v.y;
     }
     __syncthreads();
 
@@ -204,10 +222,22 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     wrho.template load<false>(j, tw);
 
     Lines<N> ln;
-    ln.row0 = psis + 2 * g * PITCH + j;
+    ln.row0 = psis + 2 * g * 2 * PITCH + 4 * (j >> 1) + (j & 1);
     const int col = rank * NL + 2 * g; // first column of the pair (column sweeps); first row of the pair = the same number
 #pragma unroll
-    for (int m = 0; m < P; m++) ln.slot[m] = cluster_addr(psis + j * PITCH + col, m);
+    for (int m = 0; m < P; m++) ln.slot[m] = cluster_addr(psis + j * 2 * PITCH + 2 * col, m);
+
+    // multipliers of eq. (2) for the thread's 2 x 8 points, once per call: [0] column sweeps (lines = columns col, col + 1
+    // = k1; points = k0), [1] row sweeps (lines = rows col, col + 1 = k0; points = k1)
+    {
+        const float2 ka = k1s[col], kb = k1s[col + 1], da = dk0[col], db = dk0[col + 1];
+#pragma unroll
+        for (int m = 0; m < P; m++) {
+            const float2 d = dk0[j + T * m], kx = k1s[j + T * m];
+            mul[(0 * P + m) * NTHR + tid] = make_float2(helmholtz_mult(d, ka, a.pscale, 0), helmholtz_mult(d, kb, a.pscale, 0));
+            mul[(1 * P + m) * NTHR + tid] = make_float2(helmholtz_mult(da, kx, a.pscale, 0), helmholtz_mult(db, kx, a.pscale, 0));
+        }
+    }
 
     // it = -1, 0: the opening half kinetic step K(dtau/2) = K0(dtau/2) K1(dtau/2) as two K sweeps (rows, then columns
     // with the density transform of the first N); it >= 1: one Strang step = P, NK, KR.  One copy of each sweep's code.
@@ -222,37 +252,30 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
                 cp2 x[P];
                 ln.template load<true>(x, xcols);
                 fft_pair<N, +1, false>(x, jj, tw, sm, &wrho);
-                if (xcols) { // lines = columns col, col + 1 (k1); points = k0
-                    const float2 ka = k1s[col], kb = k1s[col + 1];
+                const float2 *mm = mul + (xcols ? 0 : P * NTHR) + tid;
 #pragma unroll
-                    for (int m = 0; m < P; m++) {
-                        const float2 d = dk0[jj + T * m];
-                        x[m] = cscale(x[m], helmholtz_mult(d, ka, a.pscale, 0), helmholtz_mult(d, kb, a.pscale, 0));
-                    }
-                } else { // lines = rows col, col + 1 (k0); points = k1
-                    const float2 da = dk0[col], db = dk0[col + 1];
-#pragma unroll
-                    for (int m = 0; m < P; m++) {
-                        const float2 kx = k1s[jj + T * m];
-                        x[m] = cscale(x[m], helmholtz_mult(da, kx, a.pscale, 0), helmholtz_mult(db, kx, a.pscale, 0));
-                    }
+                for (int m = 0; m < P; m++) {
+                    const float2 f = mm[m * NTHR];
+                    x[m] = cscale(x[m], f.x, f.y);
                 }
                 fft_pair<N, -1, false>(x, jj, tw, sm, &wrho);
                 ln.template store<true>(x, xcols);
             }
-            cluster.sync();
-            // NK: inverse along y -> phi; nonlinear phase; K along y
+            // NK: inverse along y -> phi; nonlinear phase; K along y.  psi has not changed since the barrier before P:
+            // its loads (remote ones every other step) are issued between the arrive and the wait of this barrier
             {
                 const int jj = opaque(j);
                 const float4 *ph = phs + ((last ? 2 : 0) + (ycols ? 0 : 1)) * N;
                 cp2 x[P], v[P];
+                cluster.barrier_arrive();
+                ln.template load<false>(v, ycols);
+                cluster.barrier_wait();
                 ln.template load<true>(x, ycols);
                 fft_pair<N, -1, false>(x, jj, tw, sm, &wrho);
-                ln.template load<false>(v, ycols);
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 phi = x[m].r; // (phi of line a, phi of line b): the imaginary parts are rounding noise
-                    nl_phase_pair<false>(pack4(v[m]), phi, a.nl, x[m].r, x[m].i);
+                    nl_phase_pair_ri<false>(v[m].r, v[m].i, phi, a.nl, x[m].r, x[m].i);
                 }
                 fft_pair<N, +1, true>(x, jj, tw, sm, &wpsi);
                 phase_mul<T, P>(x, jj, ph);
@@ -270,7 +293,8 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
 
     for (int e = tid; e < NL * N; e += NTHR) {
         const int l = e / N, p = e % N;
-        gpsi[(long long)(rank * NL + l) * a.row_stride + p] = psis[l * PITCH + p];
+        gpsi[(long long)(rank * NL + l) * a.row_stride + p] =
+            make_float2(psis[l * 2 * PITCH + 4 * (p >> 1) + (p & 1)], psis[l * 2 * PITCH + 4 * (p >> 1) + (p & 1) + 2]);
     }
 }
 
