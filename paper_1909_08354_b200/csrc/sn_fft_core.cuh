@@ -634,6 +634,25 @@ __device__ __forceinline__ void fft_pair(float2 (&a)[P], float2 (&b)[P], int j, 
 }
 
 // ---- shared-memory accessors -------------------------------------------------------------
+// One exchange position = one float4 (two register pairs of the packed engine: r = (a.re, b.re), i = (a.im, b.im); or the
+// two complex values of the scalar engine).  Written as `*p = make_float4(...)`, ptxas builds the four CONSECUTIVE
+// registers of the STS.128 with four MOVs per store (S_KIN at N = 512: 160 of 1150 instructions; the cluster-resident
+// kernel: 14 % of its instruction stream).  Written as two 64-bit stores in inline PTX it allocates the two pairs
+// adjacently and still fuses them into one STS.128 (SASS checked: same STS.128 count, MOVs gone).
+#ifndef SN_XCH_PTX_STORES
+#define SN_XCH_PTX_STORES 1 // 0: plain C++ store (A/B builds)
+#endif
+__device__ __forceinline__ void xch_store(float4 *p, float2 a, float2 b)
+{
+#if SN_XCH_PTX_STORES
+    const unsigned addr = (unsigned)__cvta_generic_to_shared(p);
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a.x), "f"(a.y) : "memory");
+    asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(addr), "f"(b.x), "f"(b.y) : "memory");
+#else
+    *p = make_float4(a.x, a.y, b.x, b.y);
+#endif
+}
+
 // One float4 per point position: (a.re, a.im, b.re, b.im).  Interface: lin(pos) = linear index of a
 // position (group constant excluded), TMASK = index bits the group constant occupies,
 // idx(pos) = lin(pos) ^ group constant, st_i / ld_i = access by index.
@@ -655,7 +674,7 @@ struct SmemTile {
         return pos ^ ((pos >> 3) & 7);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ t; }
-    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { base[i] = make_float4(a.x, a.y, b.x, b.y); }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { xch_store(base + i, a, b); }
     __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
         const float4 v = base[i];
@@ -678,21 +697,7 @@ struct SmemLine {
     static constexpr int TMASK = 0;
     __host__ __device__ static constexpr int lin(int pos) { return pos ^ ((pos >> 3) & 7); }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos); }
-    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const
-    {
-#ifdef SN_XCH_SPLIT_STORES
-        // two 64-bit stores: the packed engine's (r, i) register pairs go out as they are.  One 128-bit store needs
-        // four CONSECUTIVE registers and ptxas builds them with four MOVs per store (14 % of the instructions of a
-        // latency-bound kernel); it costs 2-way bank conflicts, which only a kernel far from the shared-memory limit
-        // can afford (sn_resident.cu).
-        // (inline PTX: written as two plain stores the compiler fuses them back into one 128-bit store)
-        const unsigned addr = (unsigned)__cvta_generic_to_shared(base + i);
-        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(a.x), "f"(a.y) : "memory");
-        asm volatile("st.shared.v2.f32 [%0+8], {%1, %2};" ::"r"(addr), "f"(b.x), "f"(b.y) : "memory");
-#else
-        base[i] = make_float4(a.x, a.y, b.x, b.y);
-#endif
-    }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { xch_store(base + i, a, b); }
     __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
         const float4 v = base[i];

@@ -91,7 +91,7 @@ struct SmemSub {
         return (r * CPW) | swz<CPW>(r);
     }
     __device__ __forceinline__ int idx(int pos) const { return lin(pos) ^ t; }
-    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { sub[i] = pack4(a, b); }
+    __device__ __forceinline__ void st_i(int i, float2 a, float2 b) const { xch_store(sub + i, a, b); }
     __device__ __forceinline__ void ld_i(int i, float2 &a, float2 &b) const
     {
         const float4 v = sub[i];

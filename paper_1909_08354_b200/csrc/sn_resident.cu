@@ -34,7 +34,6 @@
 
 #define SN_TW_LOAD(p) (*(p)) // the engine's twiddle loads: the tables live in shared memory here
 #define SN_NL_SLOW_OUTLINE   // the rare large-angle path of the nonlinear phase as a call (code size)
-#define SN_XCH_SPLIT_STORES  // exchange stores as two 64-bit stores (no register re-packing; see SmemLine::st_i)
 #include "sn_fft_core.cuh"
 #include "sn_launch.h"
 #include "sn_pointwise.cuh"
