@@ -52,10 +52,11 @@ PASS_BYTES_PER_CELL = {
 }
 B_MIN = {2: 64.0, 3: 112.0}  # SURVEY.md 8(d) minimal-pass byte count per cell-update
 B_OWN = {2: 56.0, 3: 88.0}   # bytes this design's pass list has to move per cell-update
-# ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, C5_512, from profiles/r02g_ncu_full_C5_512.md
-# (capture of commit 163e14c "NEXT-4b on the GPU"; later commits changed twiddle loads and shared-memory layout, not DRAM traffic)
-NCU_TRAFFIC_C5_512 = {"H_NLKIN": 2.633e9, "S_KIN": 2.088e9, "X_KIN": 2.088e9, "H_R2C": 1.577e9, "S_FFT": 1.019e9,
-                      "X_POISSON": 1.022e9}
+# ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, C5_512, from profiles/r02z_final_C5_512.md
+# (end-of-round capture, build of commit 3eb3bad; the same values as in profiles/r02g of commit 163e14c: the commits in
+# between changed twiddle loads, register use and shared-memory stores, not DRAM traffic)
+NCU_TRAFFIC_C5_512 = {"H_NLKIN": 2.634e9, "S_KIN": 2.089e9, "X_KIN": 2.089e9, "H_R2C": 1.577e9, "S_FFT": 1.019e9,
+                      "X_POISSON": 1.020e9}
 
 
 def load_peaks():
@@ -436,7 +437,7 @@ def main():
                 "bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak,
                 "traffic": NCU_TRAFFIC_C5_512.get(dom) if cfg.name == "C5_512" and not args.extras and not f64 and not args.batch else None,
-                "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r02g_ncu_full_C5_512.md",
+                "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r02z_final_C5_512.md",
                 "note": ("R_STEPS = the cluster-resident kernel: one launch advances all K steps with the state in distributed "
                          "shared memory, HBM sees 16 B/cell per CALL; it is latency-bound inside the cluster, so every HBM "
                          "fraction of this line is an effective figure only") if dom == "R_STEPS" else None,

@@ -284,7 +284,9 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 16 */, int64_t *lau
  *                   (no sn_set_local_terms / _external_potential / _bohm / _source_tables in effect), the default
  *                   SN_OPT_DISPATCH and at most 32 ensemble members runs as ONE launch of the cluster-resident kernel:
  *                   the state stays in the distributed shared memory of a cluster of 8 CTAs for all n steps of the
- *                   call (one cluster per member); 0: the pass kernels.  Same schedule and arithmetic; the density is
+ *                   call (one cluster per member); 0: the pass kernels.  sn_create checks once that the device can hold
+ *                   such a cluster (cudaOccupancyMaxActiveClusters); where it cannot, the option stays 0 and the pass
+ *                   kernels serve the context.  Same schedule and arithmetic; the density is
  *                   transformed as a complex field there, so the two paths agree to rounding, not bit for bit. */
 #define SN_OPT_RESIDENT 4
 int sn_set_option(sn_ctx *ctx, int option, int value);

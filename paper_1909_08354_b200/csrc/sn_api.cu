@@ -270,6 +270,7 @@ struct sn_ctx {
     double *diag;
     int *sched;                             // tile counters of the dynamically scheduled pipelined kernels
     // pipelined (TMA) passes: tensor maps of psi / half spectrum seen along axis 0 and axis 1
+    bool resident_ok;  // the device can schedule the resident kernel's cluster (checked once at create)
     bool use_resident; // SN_OPT_RESIDENT: small square 2D grids advance inside one cluster's shared memory (sn_resident.cu)
     bool use_pipe;  // SN_OPT_DISPATCH != 1
     bool pipe_all;  // SN_OPT_DISPATCH == 2: pipelined kernels wherever they are instantiated (tests, A/B runs)
@@ -1199,7 +1200,7 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
     c->use_graph = l.cells <= ((int64_t)1 << 24) && !c->is_mc && l.R == 1;
     c->graph_steps = 8; // measured on B200 (1 -> 8 steps per replay): C2 39.0 -> 36.5, 64^3 28.8 -> 27.3, 128^3 61.9 -> 59.9 us/step
     c->use_pipe = !c->f64; // the TMA-pipelined kernels are complex64 only
-    c->use_resident = true;
+    c->use_resident = c->resident_ok = false; // decided below, on the context's device
     c->pipe_all = false;
     // the device that owns the workspace is the context's device
     int rc = SN_OK;
@@ -1222,6 +1223,13 @@ static int create_impl(sn_ctx **out, int ndim, const int64_t *dims, const double
                 rc = cuda_fail(cudaGetLastError());
             else if (c->use_pipe)
                 rc = make_tensor_maps(c);
+        }
+        // the cluster-resident kernel serves the context where the grid qualifies and this device can schedule its cluster
+        if (rc == SN_OK && !c->f64 && !c->is_mc && l.R == 1 && l.ndim == 2 &&
+            snk::resident_supported((int)l.n[0], (int)l.n[1])) {
+            const int nc = l.n[0] == 64 ? snk::resident_max_clusters<64>() : snk::resident_max_clusters<128>();
+            if (nc < 0) cudaGetLastError(); // not an error of the context: the pass kernels serve it
+            c->use_resident = c->resident_ok = nc > 0;
         }
     }
     if (rc != SN_OK) {
@@ -1394,7 +1402,7 @@ int sn_set_option(sn_ctx *c, int option, int value)
     SN_CUDA(cudaStreamSynchronize(c->stream));
     drop_step_graph(c);
     if (option == SN_OPT_RESIDENT) {
-        c->use_resident = value == 1;
+        c->use_resident = value == 1 && c->resident_ok;
     } else if (option == SN_OPT_GRAPH_STEPS) {
         c->graph_steps = value;
     } else if (option == SN_OPT_GRAPH) {

@@ -209,6 +209,8 @@ struct ResidentArgs {
 inline bool resident_supported(int n0, int n1) { return n0 == n1 && (n0 == 64 || n0 == 128); }
 template <int N>
 int launch_resident(const ResidentArgs &a);
+template <int N>
+int resident_max_clusters(); // clusters the device can hold at once; <= 0: the kernel cannot run here
 
 // sum |psi|^2 over n complex64 values, accumulated in double into *out (sn_mc_norms)
 int launch_norm(const float2 *psi, long long n, double *out, cudaStream_t stream);

@@ -311,6 +311,33 @@ int launch_resident(const ResidentArgs &a)
     return (int)cudaGetLastError();
 }
 
+// clusters of this kernel the device can hold at once (0: it cannot schedule one -- e.g. a partitioned GPU whose GPC
+// slices are smaller than 8 SMs -- and the scheduler keeps the pass kernels); negative: -cudaError_t
+template <int N>
+int resident_max_clusters()
+{
+    auto kern = k_resident<N>;
+    constexpr size_t smem = RGeo<N>::SMEM;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return -(int)e;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(RES_CLUSTER, 1, 1);
+    cfg.blockDim = dim3(RGeo<N>::NTHR, 1, 1);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = RES_CLUSTER;
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    e = cudaOccupancyMaxActiveClusters(&n, kern, &cfg);
+    if (e != cudaSuccess) return -(int)e;
+    return n;
+}
+
 template int launch_resident<SN_LEN>(const ResidentArgs &a);
+template int resident_max_clusters<SN_LEN>();
 
 } // namespace snk
