@@ -131,6 +131,13 @@ def test_resident_falls_back_to_the_pass_kernels(mods):
     cleared = lambda sim: (sim.set_local_terms(0.01, 1e-9, 0.02, 0.5), sim.set_local_terms(0.0, 1e-9, 0.0, 1.0))
     _, lcl, _ = gpu_run(sn, cfg, psi0, [6], resident=1, prepare=cleared)
     assert lcl == 1                              # terms switched off again: eligible again
+    sim = sn.Simulation.from_config(cfg)
+    with pytest.raises(sn.SnError):              # the option takes 0 or 1
+        sim.set_option(sn.OPT_RESIDENT, 2)
+    sim.set_state(psi0)
+    sim.step(0)                                  # no step: no launch, state untouched
+    assert np.array_equal(sim.get_state(), psi0)
+    sim.close()
 
 
 def test_resident_runs_are_bitwise_identical(mods):
