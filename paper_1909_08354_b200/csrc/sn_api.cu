@@ -963,7 +963,7 @@ bool resident_eligible(const sn_ctx *c)
            c->c_bohm == 0.0 && l.batch <= RESIDENT_MAX_BATCH;
 }
 
-int run_resident(sn_ctx *c, int64_t nsteps)
+int run_resident(sn_ctx *c, int64_t nsteps, bool order4 = false)
 {
     const Layout &l = c->lay;
     snk::ResidentArgs a;
@@ -971,16 +971,24 @@ int run_resident(sn_ctx *c, int64_t nsteps)
     a.psi = c->psi;
     a.row_stride = l.batch * l.n[1];
     a.batch = (int)l.batch;
-    a.nsteps = nsteps;
     a.tw = c->tw[0]; // n0 == n1: one table serves both axes
-    for (int d = 0; d < 2; d++) {
-        a.ph_full[d] = c->ph[PH_FULL][d];
-        a.ph_half[d] = c->ph[PH_HALF][d];
+    // the call's program: phase slots and nonlinear-coefficient sets in the order the kernel indexes them
+    const int ph_slots[2][snk::RES_PH_SLOTS] = {{PH_FULL, PH_HALF, -1, -1}, {PH_Y_END, PH_Y_MID, PH_Y_JOIN, -1}};
+    for (int sl = 0; sl < snk::RES_PH_SLOTS; sl++)
+        for (int d = 0; d < 2; d++) a.ph[sl][d] = ph_slots[order4][sl] >= 0 ? c->ph[ph_slots[order4][sl]][d] : nullptr;
+    if (!order4) { // K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2)
+        a.nsub = nsteps; a.period = 1;
+        a.nl_of[0] = 0; a.ph_of[0] = 0; a.ph_open = a.ph_last = 1;
+        a.nl[0] = c->nlv[NL_MAIN];
+    } else { // K(w1/2) [N(w1) K((w1+w0)/2) N(w0) K((w0+w1)/2) N(w1) K(w1 or w1/2)]^n
+        a.nsub = 3 * nsteps; a.period = 3;
+        a.nl_of[0] = 0; a.nl_of[1] = 1; a.nl_of[2] = 0;
+        a.ph_of[0] = 1; a.ph_of[1] = 1; a.ph_of[2] = 2; a.ph_open = a.ph_last = 0;
+        a.nl[0] = c->nlv[NL_Y1]; a.nl[1] = c->nlv[NL_Y0];
     }
     a.ksq2_1 = c->ksq2[1];
     a.dk0 = c->kother[0];
     a.pscale = (float)(c->D / (double)l.pcells);
-    a.nl = c->nlv[NL_MAIN];
     a.stream = c->stream;
     size_t ev = 0;
     if (c->profiling) {
@@ -1597,6 +1605,7 @@ int sn_step_order4(sn_ctx *c, int64_t nsteps)
     if (!c->has_state) return SN_ERR_STATE;
     if (nsteps < 0) return SN_ERR_PARAM;
     if (nsteps == 0) return SN_OK;
+    if (resident_eligible(c)) return run_resident(c, nsteps, /*order4=*/true); // same schedule, one launch
     // one step = S2(w1 h) S2(w0 h) S2(w1 h) with S2 the Strang step; adjacent kinetic halves merged:
     // K(w1/2) [N(w1) K((w1+w0)/2) N(w0) K((w0+w1)/2) N(w1) K(w1 or w1/2)]^n
     int rc = kinetic_sweep(c, PH_Y_END, /*with_nl=*/false, /*before_n=*/true, NL_MAIN, NL_Y1);

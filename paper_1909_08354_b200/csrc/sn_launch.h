@@ -192,18 +192,24 @@ int launch_pass_d(const PassArgsD &a);
 // ---- cluster-resident step (sn_resident.cu): small square 2D grids, complex64, hot-path terms only ----
 // The state lives in the distributed shared memory of a cluster of RES_CLUSTER CTAs for a whole sn_step(n) call.
 constexpr int RES_CLUSTER = 8;
+constexpr int RES_PH_SLOTS = 4; // kinetic phase tables a call can use
 struct ResidentArgs {
     float2 *psi;              // DEVICE: state, storage [n0][batch][n1]
     long long row_stride;     // elements between consecutive rows of one member (batch * n1)
     int batch;                // ensemble members: one cluster each
-    long long nsteps;         // Strang steps of this call (>= 1)
+    // The call as a program: K(ph_open) then nsub sub-steps [N(nl[nl_of[i % period]]) K(ph_of[i % period])], the last K
+    // with ph_last instead.  Strang (sn_step): period 1, K(dtau/2) [N(dtau) K(dtau)]^(n-1) N(dtau) K(dtau/2); the
+    // fourth-order composition (sn_step_order4): period 3.
+    long long nsub;           // sub-steps of this call (>= 1)
+    int period;               // 1 or 3
+    int nl_of[3], ph_of[3];   // per position in the period: index into nl[] / into ph[] (the K after that N)
+    int ph_open, ph_last;     // phase slots of the opening and of the closing kinetic sweep
     const float4 *tw;         // DEVICE: twiddle table of the (common) line length
-    const float4 *ph_full[2]; // DEVICE: kinetic phase tables per axis, s = dtau
-    const float4 *ph_half[2]; // DEVICE: s = dtau/2
+    const float4 *ph[RES_PH_SLOTS][2]; // DEVICE: kinetic phase tables [slot][axis] (unused slots: nullptr)
     const float2 *ksq2_1;     // DEVICE: k_1^2 per index of axis 1 as hi + lo
     const float2 *dk0;        // DEVICE: C - k_0^2 as hi + lo per half-spectrum row and member ([n0/2+1][batch])
     float pscale;             // D / (n0 n1)
-    NLParams nl;
+    NLParams nl[3];
     cudaStream_t stream;
 };
 inline bool resident_supported(int n0, int n1) { return n0 == n1 && (n0 == 64 || n0 == 128); }

@@ -17,7 +17,7 @@
 //     instructions re-packing);
 //   between sweeps of different orientation: one hardware cluster barrier (barrier.cluster, release/acquire).
 //
-// One step (S1-S13 of SURVEY.md 8(a); eq. (1),(2), method PAPER.md:113) is THREE sweeps, the
+// One sub-step [N K] (S1-S13 of SURVEY.md 8(a); eq. (1),(2), method PAPER.md:113) is THREE sweeps, the
 // orientation alternating (x = the axis of the sweep, y = the other one; the kinetic factors of the two axes commute
 // and the transform of rho may start along either axis):
 //   P   forward along x -> D/(C - k^2)/(N0 N1), phi^(0) = 0 if C = 0 -> inverse along x        on rho^ (forward along y done)
@@ -60,7 +60,7 @@ struct RGeo {
     static constexpr size_t OFF_XCH = 2 * OFF_RHO;
     static constexpr size_t OFF_TW = OFF_XCH + (size_t)G * N * 16;
     static constexpr size_t OFF_PH = OFF_TW + (size_t)NTW * 24;
-    static constexpr size_t OFF_DK0 = OFF_PH + 4 * (size_t)N * 16;
+    static constexpr size_t OFF_DK0 = OFF_PH + 2 * RES_PH_SLOTS * (size_t)N * 16;
     static constexpr size_t OFF_K1 = OFF_DK0 + (size_t)N * 8;
     static constexpr size_t OFF_MUL = OFF_K1 + (size_t)N * 8; // multipliers of eq. (2) per thread: [orientation][m][thread] float2
     static constexpr size_t SMEM = OFF_MUL + 2 * (size_t)P * NTHR * 8;
@@ -170,7 +170,9 @@ __device__ __forceinline__ void sweep_kin(const Lines<N> &ln, bool cols, bool wi
     }
 }
 
-template <int N>
+// PERIOD = the program's period (1: Strang, 3: fourth-order composition) as a compile-time constant: the Strang
+// instantiation keeps constant table and coefficient indices (a run-time period costs C1 0.35 us/step)
+template <int N, int PERIOD>
 __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::NTHR, 1)
     k_resident(const __grid_constant__ ResidentArgs a)
 {
@@ -183,7 +185,7 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     float *psis = reinterpret_cast<float *>(smem_raw);                       // [NL][2 PITCH] this rank's rows of psi (slots, see Lines)
     float4 *xch = reinterpret_cast<float4 *>(smem_raw + g_::OFF_XCH);        // [G][N] exchange buffers of the line-FFT engine
     float4 *tw = reinterpret_cast<float4 *>(smem_raw + g_::OFF_TW);          // twiddles: hi/lo table, then the plain copy
-    float4 *phs = reinterpret_cast<float4 *>(smem_raw + g_::OFF_PH);         // kinetic phases [full, half][axis][N]
+    float4 *phs = reinterpret_cast<float4 *>(smem_raw + g_::OFF_PH);         // kinetic phases [slot][axis][N]
     float2 *dk0 = reinterpret_cast<float2 *>(smem_raw + g_::OFF_DK0);        // C - k0^2 per index of axis 0 (hi + lo)
     float2 *k1s = reinterpret_cast<float2 *>(smem_raw + g_::OFF_K1);         // k1^2 per index of axis 1 (hi + lo)
     float2 *mul = reinterpret_cast<float2 *>(smem_raw + g_::OFF_MUL);        // D/(C - k^2)/(N0 N1) of the thread's points, both orientations
@@ -199,10 +201,12 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
         for (int e = tid; e < NTW; e += NTHR) dst[e] = __ldg(src + e);
     }
     for (int e = tid; e < N; e += NTHR) {
-        phs[0 * N + e] = __ldg(a.ph_full[0] + e);
-        phs[1 * N + e] = __ldg(a.ph_full[1] + e);
-        phs[2 * N + e] = __ldg(a.ph_half[0] + e);
-        phs[3 * N + e] = __ldg(a.ph_half[1] + e);
+#pragma unroll
+        for (int sl = 0; sl < RES_PH_SLOTS; sl++)
+            if (a.ph[sl][0] != nullptr) {
+                phs[(2 * sl + 0) * N + e] = __ldg(a.ph[sl][0] + e);
+                phs[(2 * sl + 1) * N + e] = __ldg(a.ph[sl][1] + e);
+            }
         const int kf = e <= N / 2 ? e : N - e; // C - k0^2 is tabulated for the half spectrum's rows: [n0/2+1][batch]
         dk0[e] = __ldg(a.dk0 + (long long)kf * a.batch + member);
         k1s[e] = __ldg(a.ksq2_1 + e);
@@ -238,12 +242,14 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
         }
     }
 
-    // it = -1, 0: the opening half kinetic step K(dtau/2) = K0(dtau/2) K1(dtau/2) as two K sweeps (rows, then columns
-    // with the density transform of the first N); it >= 1: one Strang step = P, NK, KR.  One copy of each sweep's code.
+    // it = -1, 0: the opening kinetic sweep K(ph_open) = K0 K1 as two K sweeps (rows, then columns with the density
+    // transform of the first N); it >= 1: one sub-step [N K] = P, NK, KR.  One copy of each sweep's code.
     bool ycols = true; // orientation of the previous sweep = the axis rho^ has been transformed along
-    for (long long it = -1; it <= a.nsteps; it++) {
-        const bool last = it == a.nsteps;
+    for (long long it = -1; it <= a.nsub; it++) {
+        const bool last = it == a.nsub;
         const bool xcols = !ycols;
+        const int pos = PERIOD > 1 && it >= 1 ? (int)((it - 1) % PERIOD) : 0;
+        const int slot = it <= 0 ? a.ph_open : (last ? a.ph_last : a.ph_of[pos]); // phase tables of this sub-step's K
         if (it >= 1) {
             // P: forward along x -> multiplier of eq. (2) -> inverse along x
             {
@@ -264,7 +270,8 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
             // its loads (remote ones every other step) are issued between the arrive and the wait of this barrier
             {
                 const int jj = opaque(j);
-                const float4 *ph = phs + ((last ? 2 : 0) + (ycols ? 0 : 1)) * N;
+                const float4 *ph = phs + (2 * slot + (ycols ? 0 : 1)) * N;
+                const NLParams &nl = a.nl[PERIOD > 1 ? a.nl_of[pos] : 0];
                 cp2 x[P], v[P];
                 cluster.barrier_arrive();
                 ln.template load<false>(v, ycols);
@@ -274,7 +281,7 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 phi = x[m].r; // (phi of line a, phi of line b): the imaginary parts are rounding noise
-                    nl_phase_pair_ri<false>(v[m].r, v[m].i, phi, a.nl, x[m].r, x[m].i);
+                    nl_phase_pair_ri<false>(v[m].r, v[m].i, phi, nl, x[m].r, x[m].i);
                 }
                 fft_pair<N, +1, true>(x, jj, tw, sm, &wpsi);
                 phase_mul<T, P>(x, jj, ph);
@@ -284,8 +291,7 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
             cluster.sync();
         }
         // KR: K along x (+ the next step's density transform along x)
-        sweep_kin<N>(ln, xcols, it >= 0 && !last, opaque(j), tw, phs + ((it <= 0 || last ? 2 : 0) + (xcols ? 0 : 1)) * N, sm, &wpsi,
-                     &wrho);
+        sweep_kin<N>(ln, xcols, it >= 0 && !last, opaque(j), tw, phs + (2 * slot + (xcols ? 0 : 1)) * N, sm, &wpsi, &wrho);
         cluster.sync(); // (the last one also keeps every rank's shared memory alive until all remote accesses are done)
         ycols = xcols;
     }
@@ -297,18 +303,24 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     }
 }
 
-template <int N>
-int launch_resident(const ResidentArgs &a)
+template <class K>
+static int launch_resident_kernel(K kern, int threads, size_t smem, const ResidentArgs &a)
 {
-    auto kern = k_resident<N>;
-    constexpr size_t smem = RGeo<N>::SMEM;
     if (!smem_attr_done(reinterpret_cast<const void *>(kern))) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
         smem_attr_mark(reinterpret_cast<const void *>(kern));
     }
-    kern<<<RES_CLUSTER * a.batch, RGeo<N>::NTHR, smem, a.stream>>>(a);
+    kern<<<RES_CLUSTER * a.batch, threads, smem, a.stream>>>(a);
     return (int)cudaGetLastError();
+}
+
+template <int N>
+int launch_resident(const ResidentArgs &a)
+{
+    if (a.period == 1) return launch_resident_kernel(k_resident<N, 1>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
+    if (a.period == 3) return launch_resident_kernel(k_resident<N, 3>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
+    return (int)cudaErrorInvalidValue;
 }
 
 // clusters of this kernel the device can hold at once (0: it cannot schedule one -- e.g. a partitioned GPU whose GPC
@@ -316,7 +328,7 @@ int launch_resident(const ResidentArgs &a)
 template <int N>
 int resident_max_clusters()
 {
-    auto kern = k_resident<N>;
+    auto kern = k_resident<N, 1>;
     constexpr size_t smem = RGeo<N>::SMEM;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return -(int)e;

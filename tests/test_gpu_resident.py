@@ -140,6 +140,34 @@ def test_resident_falls_back_to_the_pass_kernels(mods):
     sim.close()
 
 
+@pytest.mark.parametrize("dims,steps", [((128, 128), 6), ((64, 64), 5)])
+def test_resident_order4_steps_match_oracle(mods, dims, steps):
+    """sn_step_order4 (three Strang sub-steps per step) runs through the same kernel with a period-3
+    program: against the oracle's fourth-order step, against the pass kernels, and split into two calls."""
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C2"], dims, L=12.5 * dims[0] / 64, steps=steps)
+    psi0 = cfg.initial_state()
+    out = {}
+    for res in (1, 0):
+        sim = sn.Simulation.from_config(cfg)
+        sim.set_option(sn.OPT_RESIDENT, res)
+        sim.set_state(psi0)
+        n0 = sim.launch_count()
+        sim.step_order4(steps // 2)
+        sim.step_order4(steps - steps // 2)
+        out[res] = (sim.get_state(), sim.launch_count() - n0)
+        sim.close()
+    assert out[1][1] == 2 and out[0][1] > 2 * steps
+    orc = Oracle.from_config(cfg)
+    orc.set_state(psi0.astype(np.complex128))
+    orc.step_order4(steps // 2)
+    orc.step_order4(steps - steps // 2)
+    want = orc.get_state()
+    orc.close()
+    assert_state(out[1][0], want)
+    assert rel(out[1][0], out[0][0]) < 5e-6
+
+
 def test_resident_runs_are_bitwise_identical(mods):
     Oracle, inputs, sn = mods
     cfg = inputs.CONFIGS["C1"]
