@@ -249,7 +249,8 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
         const bool last = it == a.nsub;
         const bool xcols = !ycols;
         const int pos = PERIOD > 1 && it >= 1 ? (int)((it - 1) % PERIOD) : 0;
-        const int slot = it <= 0 ? a.ph_open : (last ? a.ph_last : a.ph_of[pos]); // phase tables of this sub-step's K
+        // phase tables of this sub-step's K (Strang: slot 0 = dtau, slot 1 = dtau/2 for the opening and the closing sweep)
+        const int slot = PERIOD == 1 ? ((it <= 0 || last) ? 1 : 0) : (it <= 0 ? a.ph_open : (last ? a.ph_last : a.ph_of[pos]));
         if (it >= 1) {
             // P: forward along x -> multiplier of eq. (2) -> inverse along x
             {
