@@ -28,7 +28,9 @@
 // the pass kernels; the density / potential transforms use the plain twiddles like theirs.  Every table (twiddles,
 // kinetic phases, the k^2 tables of eq. (2)) is copied into shared memory at kernel start: the acquire side of a
 // cluster barrier invalidates L1 (SASS CCTL.IVALL), so table loads through L1 would miss after every barrier.
-// Ensembles (sn_create_batch): one cluster per member.
+// Ensembles (sn_create_batch): one cluster per member.  The local terms of eq. (16) (logarithmic / power-law G) are a
+// template variant of the nonlinear phase; contexts with an external potential, source tables or the Bohm term take
+// the pass kernels.
 #include <cooperative_groups.h>
 #include <stdint.h>
 
@@ -172,7 +174,8 @@ __device__ __forceinline__ void sweep_kin(const Lines<N> &ln, bool cols, bool wi
 
 // PERIOD = the program's period (1: Strang, 3: fourth-order composition) as a compile-time constant: the Strang
 // instantiation keeps constant table and coefficient indices (a run-time period costs C1 0.35 us/step)
-template <int N, int PERIOD>
+// EXTRA: the logarithmic / power-law terms of eq. (16) (sn_set_local_terms) are in effect.
+template <int N, int PERIOD, bool EXTRA>
 __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::NTHR, 1)
     k_resident(const __grid_constant__ ResidentArgs a)
 {
@@ -282,7 +285,7 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 phi = x[m].r; // (phi of line a, phi of line b): the imaginary parts are rounding noise
-                    nl_phase_pair_ri<false>(v[m].r, v[m].i, phi, nl, x[m].r, x[m].i);
+                    nl_phase_pair_ri<EXTRA>(v[m].r, v[m].i, phi, nl, x[m].r, x[m].i);
                 }
                 fft_pair<N, +1, true>(x, jj, tw, sm, &wpsi);
                 phase_mul<T, P>(x, jj, ph);
@@ -319,8 +322,13 @@ static int launch_resident_kernel(K kern, int threads, size_t smem, const Reside
 template <int N>
 int launch_resident(const ResidentArgs &a)
 {
-    if (a.period == 1) return launch_resident_kernel(k_resident<N, 1>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
-    if (a.period == 3) return launch_resident_kernel(k_resident<N, 3>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
+    const bool extra = (a.nl[0].flags & 1) != 0;
+    if (a.period == 1)
+        return extra ? launch_resident_kernel(k_resident<N, 1, true>, RGeo<N>::NTHR, RGeo<N>::SMEM, a)
+                     : launch_resident_kernel(k_resident<N, 1, false>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
+    if (a.period == 3)
+        return extra ? launch_resident_kernel(k_resident<N, 3, true>, RGeo<N>::NTHR, RGeo<N>::SMEM, a)
+                     : launch_resident_kernel(k_resident<N, 3, false>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);
     return (int)cudaErrorInvalidValue;
 }
 
@@ -329,7 +337,7 @@ int launch_resident(const ResidentArgs &a)
 template <int N>
 int resident_max_clusters()
 {
-    auto kern = k_resident<N, 1>;
+    auto kern = k_resident<N, 1, false>;
     constexpr size_t smem = RGeo<N>::SMEM;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return -(int)e;

@@ -113,12 +113,12 @@ def test_resident_agrees_with_pass_kernels_and_split_calls(mods, dims, batch):
 
 
 def test_resident_falls_back_to_the_pass_kernels(mods):
-    """Contexts the resident kernel does not serve take the pass kernels with unchanged results: a NEXT-1 term in
-    effect, a forced dispatch, an ensemble above its member limit, other sizes and dtypes."""
+    """Contexts the resident kernel does not serve take the pass kernels with unchanged results: the Bohm term in
+    effect, a forced dispatch, an ensemble above its member limit."""
     Oracle, inputs, sn = mods
     cfg = inputs.scaled(inputs.CONFIGS["C2"], (64, 64), L=12.5, steps=6)
     psi0 = cfg.initial_state()
-    terms = lambda sim: sim.set_local_terms(0.01, 1e-9, 0.02, 0.5)
+    terms = lambda sim: sim.set_bohm(0.05, 1e-3)
     a, la, _ = gpu_run(sn, cfg, psi0, [6], resident=1, prepare=terms)
     b, lb, _ = gpu_run(sn, cfg, psi0, [6], resident=0, prepare=terms)
     assert la == lb and la > 6 and np.array_equal(a, b)
@@ -128,9 +128,9 @@ def test_resident_falls_back_to_the_pass_kernels(mods):
     big = np.stack([psi0] * 40, axis=1)
     _, lbig, _ = gpu_run(sn, cfg, big, [6], resident=1, batch=40)
     assert lbig > 6
-    cleared = lambda sim: (sim.set_local_terms(0.01, 1e-9, 0.02, 0.5), sim.set_local_terms(0.0, 1e-9, 0.0, 1.0))
+    cleared = lambda sim: (sim.set_bohm(0.05, 1e-3), sim.set_bohm(0.0, 1e-3))
     _, lcl, _ = gpu_run(sn, cfg, psi0, [6], resident=1, prepare=cleared)
-    assert lcl == 1                              # terms switched off again: eligible again
+    assert lcl == 1                              # term switched off again: eligible again
     sim = sn.Simulation.from_config(cfg)
     with pytest.raises(sn.SnError):              # the option takes 0 or 1
         sim.set_option(sn.OPT_RESIDENT, 2)
@@ -138,6 +138,27 @@ def test_resident_falls_back_to_the_pass_kernels(mods):
     sim.step(0)                                  # no step: no launch, state untouched
     assert np.array_equal(sim.get_state(), psi0)
     sim.close()
+
+
+@pytest.mark.parametrize("terms", [(0.05, 1e-12, 0.0, 1.0), (0.0, 1e-12, 0.08, 2.0 / 3.0), (0.02, 1e-12, 0.05, 0.5)])
+def test_resident_local_terms_match_oracle(mods, terms):
+    """The logarithmic and power-law terms of eq. (16) (V_p = w ln rho, (n w/(n-1)) rho^(n-1)) run through
+    the resident kernel's nonlinear phase; against the oracle and against the pass kernels."""
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C2"], (128, 128), L=25.0, steps=40)
+    psi0 = cfg.initial_state()
+    prep = lambda sim: sim.set_local_terms(*terms)
+    a, la, _ = gpu_run(sn, cfg, psi0, [40], resident=1, prepare=prep)
+    b, lb, _ = gpu_run(sn, cfg, psi0, [40], resident=0, prepare=prep)
+    assert la == 1 and lb > 40
+    orc = Oracle.from_config(cfg)
+    orc.set_local_terms(*terms)
+    orc.set_state(psi0.astype(np.complex128))
+    orc.step(40)
+    want = orc.get_state()
+    orc.close()
+    assert_state(a, want)
+    assert rel(a, b) < 5e-6
 
 
 @pytest.mark.parametrize("dims,steps", [((128, 128), 6), ((64, 64), 5)])
