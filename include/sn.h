@@ -281,7 +281,7 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 16 */, int64_t *lau
 #define SN_OPT_GRAPH_STEPS 3 /* interior steps captured per replayed graph, 1 ... 64 (launch-bound grids; default 8; the interior
                               * steps a call leaves over replay a one-step graph, the closing step runs as plain launches) */
 /*   SN_OPT_RESIDENT 1 (default): sn_step / sn_step_order4 on a complex64 2D grid with n0 == n1 in {64, 128}, local
- *                   nonlinearities only (no sn_set_external_potential / _bohm / _source_tables in effect), the default
+ *                   nonlinearities and / or an external potential (no sn_set_bohm / _source_tables in effect), the default
  *                   SN_OPT_DISPATCH and at most 32 ensemble members runs as ONE launch of the cluster-resident kernel:
  *                   the state stays in the distributed shared memory of a cluster of 8 CTAs for all n steps of the
  *                   call (one cluster per member); 0: the pass kernels.  sn_create checks once that the device can hold

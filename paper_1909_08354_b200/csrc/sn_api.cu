@@ -950,7 +950,7 @@ int slab_copy_block(const Layout &l, float2 *A_r, float2 *B_s, int64_t lo, int64
 
 // ---- cluster-resident step (sn_resident.cu): the whole sn_step(n) call of a small square 2D grid in ONE launch ----
 // Served: complex64, 2D, n0 == n1 in {64, 128}, local nonlinearities (polynomial G and the log / power-law terms of
-// eq. (16); no external potential, source tables or Bohm term), the default
+// eq. (16), an external potential; no source tables or Bohm term), the default
 // dispatch (SN_OPT_DISPATCH 1 / 2 ask for the pass kernels by name), ensembles of up to RESIDENT_MAX_BATCH members
 // (one cluster per member; measured on B200, 128^2: 16 members 13 vs 25 us/step, 32 members 14 vs 26, 64 members 28 vs 28 -- a large
 // ensemble fills the machine through the pass kernels, which are the faster ones per cell).  Everything else takes the
@@ -960,8 +960,7 @@ bool resident_eligible(const sn_ctx *c)
 {
     const Layout &l = c->lay;
     return c->use_resident && c->use_pipe && !c->pipe_all && !c->f64 && !c->is_mc && l.R == 1 && l.ndim == 2 &&
-           snk::resident_supported((int)l.n[0], (int)l.n[1]) && !c->has_vext && !c->has_src && c->c_bohm == 0.0 &&
-           l.batch <= RESIDENT_MAX_BATCH;
+           snk::resident_supported((int)l.n[0], (int)l.n[1]) && !c->has_src && c->c_bohm == 0.0 && l.batch <= RESIDENT_MAX_BATCH;
 }
 
 int run_resident(sn_ctx *c, int64_t nsteps, bool order4 = false)
@@ -990,6 +989,9 @@ int run_resident(sn_ctx *c, int64_t nsteps, bool order4 = false)
     a.ksq2_1 = c->ksq2[1];
     a.dk0 = c->kother[0];
     a.pscale = (float)(c->D / (double)l.pcells);
+    a.vext = c->has_vext ? c->vext : nullptr;
+    for (int k = 0; k < 3; k++) // the pass kernels may leave V to the contiguous pass (v_in_xkin); here it rides on the nonlinear phase
+        if (c->has_vext) a.nl[k].flags |= 2;
     a.stream = c->stream;
     size_t ev = 0;
     if (c->profiling) {

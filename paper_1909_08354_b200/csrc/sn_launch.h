@@ -209,6 +209,7 @@ struct ResidentArgs {
     const float2 *ksq2_1;     // DEVICE: k_1^2 per index of axis 1 as hi + lo
     const float2 *dk0;        // DEVICE: C - k_0^2 as hi + lo per half-spectrum row and member ([n0/2+1][batch])
     float pscale;             // D / (n0 n1)
+    const float *vext;        // DEVICE: external potential V(x) (layout of psi, float) or nullptr  (phi_C of eq. (15))
     NLParams nl[3];
     cudaStream_t stream;
 };

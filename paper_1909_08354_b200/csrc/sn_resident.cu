@@ -29,8 +29,8 @@
 // kinetic phases, the k^2 tables of eq. (2)) is copied into shared memory at kernel start: the acquire side of a
 // cluster barrier invalidates L1 (SASS CCTL.IVALL), so table loads through L1 would miss after every barrier.
 // Ensembles (sn_create_batch): one cluster per member.  The local terms of eq. (16) (logarithmic / power-law G) are a
-// template variant of the nonlinear phase; contexts with an external potential, source tables or the Bohm term take
-// the pass kernels.
+// template variant of the nonlinear phase, and so is a fixed external potential V(x) (phi_C of eq. (15)), whose rows sit
+// in the ranks' shared memory beside psi; contexts with source tables or the Bohm term take the pass kernels.
 #include <cooperative_groups.h>
 #include <stdint.h>
 
@@ -65,7 +65,8 @@ struct RGeo {
     static constexpr size_t OFF_DK0 = OFF_PH + 2 * RES_PH_SLOTS * (size_t)N * 16;
     static constexpr size_t OFF_K1 = OFF_DK0 + (size_t)N * 8;
     static constexpr size_t OFF_MUL = OFF_K1 + (size_t)N * 8; // multipliers of eq. (2) per thread: [orientation][m][thread] float2
-    static constexpr size_t SMEM = OFF_MUL + 2 * (size_t)P * NTHR * 8;
+    static constexpr size_t OFF_V = OFF_MUL + 2 * (size_t)P * NTHR * 8; // external potential rows: [NL][PITCH] floats, column pairs adjacent
+    static constexpr size_t SMEM = OFF_V + (size_t)NL * PITCH * 4;
     static_assert(T == NL && T <= 32, "point j + T m of an axis-0 line lives in row j of rank m; a pair is one warp or less");
     static_assert(OFF_TW % 16 == 0 && OFF_PH % 16 == 0 && (NTW * 16) % 8 == 0, "table alignment");
 };
@@ -174,7 +175,8 @@ __device__ __forceinline__ void sweep_kin(const Lines<N> &ln, bool cols, bool wi
 
 // PERIOD = the program's period (1: Strang, 3: fourth-order composition) as a compile-time constant: the Strang
 // instantiation keeps constant table and coefficient indices (a run-time period costs C1 0.35 us/step)
-// EXTRA: the logarithmic / power-law terms of eq. (16) (sn_set_local_terms) are in effect.
+// EXTRA: the logarithmic / power-law terms of eq. (16) (sn_set_local_terms) and / or an external potential
+// (sn_set_external_potential) are in effect.
 template <int N, int PERIOD, bool EXTRA>
 __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::NTHR, 1)
     k_resident(const __grid_constant__ ResidentArgs a)
@@ -192,6 +194,7 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     float2 *dk0 = reinterpret_cast<float2 *>(smem_raw + g_::OFF_DK0);        // C - k0^2 per index of axis 0 (hi + lo)
     float2 *k1s = reinterpret_cast<float2 *>(smem_raw + g_::OFF_K1);         // k1^2 per index of axis 1 (hi + lo)
     float2 *mul = reinterpret_cast<float2 *>(smem_raw + g_::OFF_MUL);        // D/(C - k^2)/(N0 N1) of the thread's points, both orientations
+    float *vrows = reinterpret_cast<float *>(smem_raw + g_::OFF_V);          // this rank's rows of the external potential
     const int tid = threadIdx.x, g = tid / T, j = tid % T;
     SmemLine<T> sm{xch + g * N, 1 + g, false};
     float2 *gpsi = a.psi + (long long)member * N; // storage [n0][batch][n1]
@@ -214,6 +217,11 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
         dk0[e] = __ldg(a.dk0 + (long long)kf * a.batch + member);
         k1s[e] = __ldg(a.ksq2_1 + e);
     }
+    if (EXTRA && a.vext != nullptr)
+        for (int e = tid; e < NL * N; e += NTHR) {
+            const int l = e / N, p = e % N;
+            vrows[l * PITCH + p] = __ldg(a.vext + (long long)member * N + (long long)(rank * NL + l) * a.row_stride + p);
+        }
     for (int e = tid; e < NL * N; e += NTHR) {
         const int l = e / N, p = e % N;
         const float2 v = gpsi[(long long)(rank * NL + l) * a.row_stride + p];
@@ -232,6 +240,11 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
     const int col = rank * NL + 2 * g; // first column of the pair (column sweeps); first row of the pair = the same number
 #pragma unroll
     for (int m = 0; m < P; m++) ln.slot[m] = cluster_addr(psis + j * 2 * PITCH + 2 * col, m);
+
+    uint32_t vslot[P]; // external potential of the column pair: (V_col, V_col+1) in row j of rank m
+#pragma unroll
+    for (int m = 0; m < P; m++) vslot[m] = EXTRA ? cluster_addr(vrows + j * PITCH + col, m) : 0u;
+    const float *vrow0 = vrows + 2 * g * PITCH + j; // the row pair's values at point j (rows PITCH apart, points T apart)
 
     // multipliers of eq. (2) for the thread's 2 x 8 points, once per call: [0] column sweeps (lines = columns col, col + 1
     // = k1; points = k0), [1] row sweeps (lines = rows col, col + 1 = k0; points = k1)
@@ -285,7 +298,12 @@ __global__ void __cluster_dims__(RES_CLUSTER, 1, 1) __launch_bounds__(RGeo<N>::N
 #pragma unroll
                 for (int m = 0; m < P; m++) {
                     const float2 phi = x[m].r; // (phi of line a, phi of line b): the imaginary parts are rounding noise
-                    nl_phase_pair_ri<EXTRA>(v[m].r, v[m].i, phi, nl, x[m].r, x[m].i);
+                    float2 ve = make_float2(0.f, 0.f);
+                    if (EXTRA && (nl.flags & 2)) {
+                        if (ycols) asm volatile("ld.shared::cluster.v2.f32 {%0, %1}, [%2];" : "=f"(ve.x), "=f"(ve.y) : "r"(vslot[m]) : "memory");
+                        else ve = make_float2(vrow0[T * m], vrow0[PITCH + T * m]);
+                    }
+                    nl_phase_pair_ri<EXTRA>(v[m].r, v[m].i, phi, nl, x[m].r, x[m].i, ve);
                 }
                 fft_pair<N, +1, true>(x, jj, tw, sm, &wpsi);
                 phase_mul<T, P>(x, jj, ph);
@@ -322,7 +340,7 @@ static int launch_resident_kernel(K kern, int threads, size_t smem, const Reside
 template <int N>
 int launch_resident(const ResidentArgs &a)
 {
-    const bool extra = (a.nl[0].flags & 1) != 0;
+    const bool extra = a.nl[0].flags != 0; // log / power-law terms and / or an external potential
     if (a.period == 1)
         return extra ? launch_resident_kernel(k_resident<N, 1, true>, RGeo<N>::NTHR, RGeo<N>::SMEM, a)
                      : launch_resident_kernel(k_resident<N, 1, false>, RGeo<N>::NTHR, RGeo<N>::SMEM, a);

@@ -31,8 +31,8 @@ def oracle_run(Oracle, cfg, psi0, steps):
     return want
 
 
-def gpu_run(sn, cfg, psi0, calls, resident=1, batch=None, prepare=None):
-    sim = sn.Simulation.from_config(cfg, batch=batch)
+def gpu_run(sn, cfg, psi0, calls, resident=1, batch=None, prepare=None, features=0):
+    sim = sn.Simulation.from_config(cfg, batch=batch, features=features)
     sim.set_option(sn.OPT_RESIDENT, resident)
     if prepare:
         prepare(sim)
@@ -155,6 +155,45 @@ def test_resident_local_terms_match_oracle(mods, terms):
     orc.set_local_terms(*terms)
     orc.set_state(psi0.astype(np.complex128))
     orc.step(40)
+    want = orc.get_state()
+    orc.close()
+    assert_state(a, want)
+    assert rel(a, b) < 5e-6
+
+
+@pytest.mark.parametrize("dims,order4", [((128, 128), False), ((64, 64), False), ((128, 128), True)])
+def test_resident_external_potential_matches_oracle(mods, dims, order4):
+    """A fixed external potential V(x) (phi_C of eq. (15); softened at the origin, reading Q16) together
+    with the local terms: its rows sit in the ranks' shared memory and its phase rides on the nonlinear phase."""
+    Oracle, inputs, sn = mods
+    L = 25.0 * dims[0] / 128
+    cfg = inputs.scaled(inputs.CONFIGS["C2"], dims, L=L, steps=30)
+    psi0 = cfg.initial_state()
+    X = np.meshgrid(*[inputs.coords(n, L) for n in dims], indexing="ij")
+    r = np.sqrt(sum(x * x for x in X) + 1.0)
+    V = (-1.0 / r + 0.05 * X[0] - 0.02 * X[1]).astype(np.float32)   # not symmetric under transposition
+    steps = 6 if order4 else 30
+    def prep(sim):
+        sim.set_local_terms(0.02, 1e-12, 0.05, 0.5)
+        sim.set_external_potential(V)
+    def run(res):
+        sim = sn.Simulation.from_config(cfg, features=sn.FEAT_VEXT)
+        sim.set_option(sn.OPT_RESIDENT, res)
+        prep(sim)
+        sim.set_state(psi0)
+        n0 = sim.launch_count()
+        (sim.step_order4 if order4 else sim.step)(steps)
+        out = (sim.get_state(), sim.launch_count() - n0)
+        sim.close()
+        return out
+    a, la = run(1)
+    b, lb = run(0)
+    assert la == 1 and lb > steps
+    orc = Oracle.from_config(cfg)
+    orc.set_local_terms(0.02, 1e-12, 0.05, 0.5)
+    orc.set_external_potential(V.astype(np.float64))
+    orc.set_state(psi0.astype(np.complex128))
+    (orc.step_order4 if order4 else orc.step)(steps)
     want = orc.get_state()
     orc.close()
     assert_state(a, want)
