@@ -282,7 +282,8 @@ int sn_profile_read(sn_ctx *ctx, double *ms_by_kind /* host, 16 */, int64_t *lau
                               * steps a call leaves over replay a one-step graph, the closing step runs as plain launches) */
 /*   SN_OPT_RESIDENT 1 (default): sn_step / sn_step_order4 on a complex64 2D grid with n0 == n1 in {64, 128}, local
  *                   nonlinearities and / or an external potential (no sn_set_bohm / _source_tables in effect), the default
- *                   SN_OPT_DISPATCH and at most 32 ensemble members runs as ONE launch of the cluster-resident kernel:
+ *                   SN_OPT_DISPATCH and at most 32 (128^2) / 256 (64^2) ensemble members runs as ONE launch of the
+ *                   cluster-resident kernel:
  *                   the state stays in the distributed shared memory of a cluster of 8 CTAs for all n steps of the
  *                   call (one cluster per member); 0: the pass kernels.  sn_create checks once that the device can hold
  *                   such a cluster (cudaOccupancyMaxActiveClusters); where it cannot, the option stays 0 and the pass

@@ -955,12 +955,19 @@ int slab_copy_block(const Layout &l, float2 *A_r, float2 *B_s, int64_t lo, int64
 // (one cluster per member; measured on B200, 128^2: 16 members 13 vs 25 us/step, 32 members 14 vs 26, 64 members 28 vs 28 -- a large
 // ensemble fills the machine through the pass kernels, which are the faster ones per cell).  Everything else takes the
 // pass kernels.
+// member limits, measured on B200 (us/step resident vs pass kernels): 128^2: 16 members 13 vs 25, 32 members 14 vs 26, 64
+// members 28 vs 28; 64^2 (32-thread CTAs, 25 KB of shared memory: many more clusters at once): 64 members 6.5 vs 19.2, 148
+// members 13.5 vs 19.7, 296 members 21.9 vs 23.6, 1024 members 70 vs 54
+#ifndef SN_RES_MAXB64
+#define SN_RES_MAXB64 256
+#endif
 constexpr int64_t RESIDENT_MAX_BATCH = 32;
 bool resident_eligible(const sn_ctx *c)
 {
     const Layout &l = c->lay;
     return c->use_resident && c->use_pipe && !c->pipe_all && !c->f64 && !c->is_mc && l.R == 1 && l.ndim == 2 &&
-           snk::resident_supported((int)l.n[0], (int)l.n[1]) && !c->has_src && c->c_bohm == 0.0 && l.batch <= RESIDENT_MAX_BATCH;
+           snk::resident_supported((int)l.n[0], (int)l.n[1]) && !c->has_src && c->c_bohm == 0.0 &&
+           l.batch <= (l.n[0] == 64 ? (int64_t)SN_RES_MAXB64 : RESIDENT_MAX_BATCH);
 }
 
 int run_resident(sn_ctx *c, int64_t nsteps, bool order4 = false)

@@ -125,8 +125,8 @@ def test_resident_falls_back_to_the_pass_kernels(mods):
     forced = lambda sim: sim.set_option(sn.OPT_DISPATCH, sn.DISPATCH_FIRST_PATH)
     _, lf, _ = gpu_run(sn, cfg, psi0, [6], resident=1, prepare=forced)
     assert lf > 6
-    big = np.stack([psi0] * 40, axis=1)
-    _, lbig, _ = gpu_run(sn, cfg, big, [6], resident=1, batch=40)
+    big = np.stack([psi0] * 300, axis=1)          # above the member limit of the 64^2 kernel (256; 32 at 128^2)
+    _, lbig, _ = gpu_run(sn, cfg, big, [6], resident=1, batch=300)
     assert lbig > 6
     cleared = lambda sim: (sim.set_bohm(0.05, 1e-3), sim.set_bohm(0.0, 1e-3))
     _, lcl, _ = gpu_run(sn, cfg, psi0, [6], resident=1, prepare=cleared)
