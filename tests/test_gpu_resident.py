@@ -228,6 +228,22 @@ def test_resident_order4_steps_match_oracle(mods, dims, steps):
     assert rel(out[1][0], out[0][0]) < 5e-6
 
 
+@pytest.mark.parametrize("dims,batch", [((128, 128), 32), ((64, 64), 256)])
+def test_resident_full_ensembles_are_bitwise_the_single_system(mods, dims, batch):
+    """The largest ensembles the kernel serves: every cluster of the machine busy at once, rough states (blobs + white
+    noise).  Every member must equal the single-system run bit for bit, in every repetition: a race between clusters, or
+    between the remote accesses of one cluster and its barriers, would show as a differing member."""
+    Oracle, inputs, sn = mods
+    cfg = inputs.scaled(inputs.CONFIGS["C2"], dims, L=12.5 * dims[0] / 64, steps=60)
+    one = (0.5 * cfg.initial_state() + 0.2 * inputs.white_noise(dims, 3)).astype(np.complex64)
+    ref, l1, _ = gpu_run(sn, cfg, one, [60])
+    psi0 = np.stack([one] * batch, axis=1).astype(np.complex64)
+    for rep in range(3):
+        out, lb, _ = gpu_run(sn, cfg, psi0, [60], batch=batch)
+        assert l1 == 1 and lb == 1
+        assert all(np.array_equal(out[:, b], ref) for b in range(batch)), rep
+
+
 def test_resident_runs_are_bitwise_identical(mods):
     Oracle, inputs, sn = mods
     cfg = inputs.CONFIGS["C1"]
