@@ -492,7 +492,8 @@ int run_pass_raw(sn_ctx *c, int N, PassArgs &a)
         // which kinds gain from the pipeline depends on the line length (measured): the heavy axis-0
         // pass always; the others at N = 512 and N >= 2048 (N <= 256 and N = 1024: two first-path CTAs per SM win)
         const bool worth = a.kind == snk::P_H_NLKIN || c->pipe_all || N == 512 || N >= 2048 ||
-                           (N == 384 && a.kind == snk::P_H_R2C) ||
+                           (a.kind == snk::P_H_R2C && (N == 256 || N == 384 || N == 1024)) || // measured per length: the
+                           (a.kind == snk::P_S_FFT && N == 256) ||                             // light axis-0 / axis-1 passes too
                            (a.kind == snk::P_X_KIN && a.vext != nullptr); // V rides on the pipelined contiguous pass
         if (maps && worth && snk::pipe_supported(N, a.kind, a.ncols, a.nlines)) {
             snk::PipeArgs pa;
